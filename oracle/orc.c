@@ -1,0 +1,543 @@
+/*
+ * orc.c -- the ORACLE: a plain, slow, fp64 CPU statement of what the hot path
+ * of arXiv 1308.5587 (HOOMD-blue) computes for one Lennard-Jones NVE time step.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, the smoke check
+ * in __graft_entry__.py and bench.py's cpu_baseline / --impl reference legs may
+ * build, load or call it.  It shares no code, header, table or helper with the
+ * CUDA library (paper_1308_5587_b200/csrc) and neither includes the other.
+ *
+ * Style: every function is the paper's definition written out, in the paper's
+ * order and notation, in double precision.  No blocking, fusion, tiling or
+ * reordering; the only parallelism is an optional `omp parallel for` over the
+ * particle index i, which leaves each particle's arithmetic untouched.
+ *
+ * Parity status: every function below is pinned by tests/test_oracle_*.py
+ * (closed forms, O(N^2) brute force, invariants); nothing is "parity unpinned".
+ *
+ * Citations are PAPER.md:<line> (the extracted paper) and the readings of
+ * SURVEY.md section 8(c) / DESIGN.md "Readings".
+ *
+ * Conventions
+ *   box      cubic, periodic, from b = -L/2 to b + L = +L/2
+ *   pos      double [N][3];  type int32 [N];  tables [ntypes*ntypes] row-major
+ *   cell id  c = cx + m*(cy + m*cz)
+ *   virial   six components in the order xx, xy, xz, yy, yz, zz
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_OK 0
+#define ORC_EBOX -1   /* L < 2 r_max or fewer than 3 cells per axis */
+#define ORC_ECAP -2   /* caller's buffer too small */
+#define ORC_ENOMEM -3
+
+/* ------------------------------------------------------------------ c1 ---- */
+/* Cells per axis.  [reading c1.ii] m = floor(L / r_max), so that the cell
+ * width L/m >= r_max and the 27 adjacent cells of Alg. 3 l.11 suffice. */
+int orc_cell_dim(double L, double r_max)
+{
+    return (int)floor(L / r_max);
+}
+
+/* Algorithm 2 lines 5-9: shift to the box origin, scale by
+ * s = m/L, floor.  [reading c1.i] "r + b" is read as x - b with b = -L/2.
+ * [reading c1.iii] a result outside 0..m-1 is wrapped periodically.
+ * [reading c1.iv] CANONICAL value: the same expression in IEEE binary32,
+ * each operation rounded separately (no fused multiply-add), because
+ * "bit-exact membership" needs one pinned formula.  Compile with
+ * -ffp-contract=off. */
+void orc_cell_index_f32(const float *pos, int64_t N, float L, int m, int32_t *cell)
+{
+    const float b = -0.5f * L;
+    const float s = (float)m / L;
+    for (int64_t i = 0; i < N; i++) {
+        int c[3];
+        for (int a = 0; a < 3; a++) {
+            volatile float r = pos[3 * i + a] - b;   /* line 6 */
+            volatile float u = r * s;                /* lines 7-9 */
+            int ca = (int)floorf(u);
+            if (ca >= m) ca -= m;
+            if (ca < 0) ca += m;
+            c[a] = ca;
+        }
+        cell[i] = c[0] + m * (c[1] + m * c[2]);
+    }
+}
+
+/* The same index from the geometry in double.  margin[i] = distance of the
+ * scaled coordinate to the nearest integer (min over axes): where it is tiny
+ * the fp32 and fp64 answers may legitimately differ. */
+void orc_cell_index_f64(const double *pos, int64_t N, double L, int m, int32_t *cell, double *margin)
+{
+    const double b = -0.5 * L;
+    const double s = (double)m / L;
+    for (int64_t i = 0; i < N; i++) {
+        int c[3];
+        double mg = 1.0;
+        for (int a = 0; a < 3; a++) {
+            double u = (pos[3 * i + a] - b) * s;
+            double fl = floor(u);
+            double d = fmin(u - fl, fl + 1.0 - u);
+            if (d < mg) mg = d;
+            int ca = (int)fl;
+            if (ca >= m) ca -= m;
+            if (ca < 0) ca += m;
+            c[a] = ca;
+        }
+        cell[i] = c[0] + m * (c[1] + m * c[2]);
+        if (margin) margin[i] = mg;
+    }
+}
+
+/* Algorithm 2 lines 10-11: celln counts, then each particle
+ * takes the next free slot of its cell.  Run serially in index order, so the
+ * (undefined) entry order is ascending i.  Stored as CSR: members of cell c are
+ * cell_members[cell_start[c] .. cell_start[c+1]). */
+void orc_build_cells(const int32_t *cell, int64_t N, int m, int64_t *cell_start, int32_t *cell_members)
+{
+    const int64_t nc = (int64_t)m * m * m;
+    int64_t *celln = (int64_t *)calloc((size_t)nc + 1, sizeof(int64_t));
+    for (int64_t i = 0; i < N; i++) celln[cell[i]]++;
+    cell_start[0] = 0;
+    for (int64_t c = 0; c < nc; c++) cell_start[c + 1] = cell_start[c] + celln[c];
+    memset(celln, 0, (size_t)nc * sizeof(int64_t));
+    for (int64_t i = 0; i < N; i++) {
+        int64_t n = celln[cell[i]]++;                 /* line 10: n <= atomicInc */
+        cell_members[cell_start[cell[i]] + n] = (int32_t)i; /* line 11 */
+    }
+    free(celln);
+}
+
+/* ------------------------------------------------------------------ c2 ---- */
+/* minimage (Alg. 3 l.16): nearest periodic image of a separation component. */
+static inline double minimage(double d, double L)
+{
+    return d - L * rint(d / L);
+}
+
+static inline double dist2(const double *pos, int64_t i, int64_t j, double L, double d[3])
+{
+    d[0] = minimage(pos[3 * i + 0] - pos[3 * j + 0], L);
+    d[1] = minimage(pos[3 * i + 1] - pos[3 * j + 1], L);
+    d[2] = minimage(pos[3 * i + 2] - pos[3 * j + 2], L);
+    return d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+}
+
+/* The DEFINITION of the neighbor set: N(i) = { j != i : |minimage(Ri-Rj)| < r_max }
+ * (Alg. 3 l.17, strict <), by testing every pair.  Full list, ascending j.
+ * Call with nbr == NULL to get the counts only. */
+int orc_nlist_brute(const double *pos, int64_t N, double L, double r_max,
+                    int32_t *count, const int64_t *row_start, int32_t *nbr)
+{
+    if (L < 2.0 * r_max) return ORC_EBOX;
+    const double r_max2 = r_max * r_max;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < N; i++) {
+        int32_t n = 0;
+        double d[3];
+        for (int64_t j = 0; j < N; j++) {
+            if (j == i) continue;
+            if (dist2(pos, i, j, L, d) < r_max2) {
+                if (nbr) nbr[row_start[i] + n] = (int32_t)j;
+                n++;
+            }
+        }
+        count[i] = n;
+    }
+    return ORC_OK;
+}
+
+/* The same set for a SAMPLE of particles (full-size spot checks): rows for
+ * sample[0..S) only, each tested against all N. */
+int orc_nlist_brute_sample(const double *pos, int64_t N, double L, double r_max,
+                           const int64_t *sample, int64_t S,
+                           int32_t *count, const int64_t *row_start, int32_t *nbr)
+{
+    if (L < 2.0 * r_max) return ORC_EBOX;
+    const double r_max2 = r_max * r_max;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t k = 0; k < S; k++) {
+        const int64_t i = sample[k];
+        int32_t n = 0;
+        double d[3];
+        for (int64_t j = 0; j < N; j++) {
+            if (j == i) continue;
+            if (dist2(pos, i, j, L, d) < r_max2) {
+                if (nbr) nbr[row_start[k] + n] = (int32_t)j;
+                n++;
+            }
+        }
+        count[k] = n;
+    }
+    return ORC_OK;
+}
+
+/* Algorithm 3, step by step, one particle at a time.
+ * [reading c2.i] line 15 is read as (R_j, j) <= celldata[o, d].
+ * [reading c2.ii] nlistn is written after the loop over a.
+ * `cell` is the cell of every particle as used to build cell_start/members
+ * (lines 5-9 recompute exactly that).  celladj (line 12) is computed on the fly:
+ * the 27 cells (cx+ax, cy+ay, cz+az), a in {-1,0,1}^3, wrapped periodically.
+ * Call with nbr == NULL to get the counts only. */
+int orc_nlist_cells(const double *pos, int64_t N, double L, double r_max, int m,
+                    const int32_t *cell, const int64_t *cell_start, const int32_t *cell_members,
+                    int32_t *count, const int64_t *row_start, int32_t *nbr)
+{
+    if (m < 3 || L < 2.0 * r_max || L / m < r_max) return ORC_EBOX;
+    const double r_max2 = r_max * r_max;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < N; i++) {
+        const int cx = cell[i] % m, cy = (cell[i] / m) % m, cz = cell[i] / (m * m);
+        int32_t n_neigh = 0;                                   /* line 10 */
+        for (int a = 0; a < 27; a++) {                         /* line 11 */
+            const int dx = (cx + (a % 3) - 1 + m) % m;         /* line 12 */
+            const int dy = (cy + ((a / 3) % 3) - 1 + m) % m;
+            const int dz = (cz + (a / 9) - 1 + m) % m;
+            const int64_t dcell = dx + (int64_t)m * (dy + (int64_t)m * dz);
+            const int64_t n_d = cell_start[dcell + 1] - cell_start[dcell]; /* line 13 */
+            for (int64_t o = 0; o < n_d; o++) {                /* line 14 */
+                const int64_t j = cell_members[cell_start[dcell] + o]; /* line 15 */
+                double r[3];
+                const double r2 = dist2(pos, i, j, L, r);      /* line 16 */
+                if (r2 < r_max2 && i != j) {                   /* line 17 */
+                    if (nbr) nbr[row_start[i] + n_neigh] = (int32_t)j; /* line 18 */
+                    n_neigh++;                                 /* line 19 */
+                }
+            }
+        }
+        count[i] = n_neigh;                                    /* line 22 */
+    }
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------ c3 ---- */
+/* [reading c3] Rebuild rule: the list built at R^build stays valid while no
+ * particle has moved more than r_buff/2 (PAPER.md:167 only says r_buff exists).
+ * Returns max_i |minimage(R_i - R_i^build)|^2; rebuild iff it is > (r_buff/2)^2. */
+double orc_max_disp2(const double *pos, const double *pos_build, int64_t N, double L)
+{
+    double mx = 0.0;
+    for (int64_t i = 0; i < N; i++) {
+        double s = 0.0;
+        for (int a = 0; a < 3; a++) {
+            double d = minimage(pos[3 * i + a] - pos_build[3 * i + a], L);
+            s += d * d;
+        }
+        if (s > mx) mx = s;
+    }
+    return mx;
+}
+
+/* ------------------------------------------------------------- c4, c5 ---- */
+/* V_lj(r) = 4 eps [ (sigma/r)^12 - alpha (sigma/r)^6 ], alpha = 1
+ * -(1/r) dV/dr = (1/r^2) (48 eps (sigma/r)^12 - 24 eps (sigma/r)^6)
+ * active iff r < r_cut; shift: V = V_lj(r) - V_lj(r_cut). */
+static inline double vlj(double r, double eps, double sigma)
+{
+    const double sr = sigma / r;
+    const double sr6 = sr * sr * sr * sr * sr * sr;
+    return 4.0 * eps * (sr6 * sr6 - sr6);
+}
+
+void orc_lj_pair(double r, double eps, double sigma, double r_cut, int shift,
+                 double *V, double *minus_dVdr_over_r)
+{
+    if (!(r < r_cut)) { *V = 0.0; *minus_dVdr_over_r = 0.0; return; }
+    const double sr = sigma / r;
+    const double sr6 = sr * sr * sr * sr * sr * sr;
+    *minus_dVdr_over_r = (48.0 * eps * sr6 * sr6 - 24.0 * eps * sr6) / (r * r);
+    *V = vlj(r, eps, sigma) - (shift ? vlj(r_cut, eps, sigma) : 0.0);
+}
+
+/* ------------------------------------------------------------------ c6 ---- */
+/* One pair's contribution to particle i:  F_i += f, U_i += V/2,
+ * W_i^{ab} += (1/2) d^a f^b  with d = minimage(R_i - R_j), f = [-(1/r)dV/dr] d. */
+static inline void add_pair(const double d[3], double r2, double eps, double sigma, double r_cut,
+                            int shift, double *F, double *U, double *W,
+                            double band, double *allow)
+{
+    const double r = sqrt(r2);
+    double V, fdivr;
+    orc_lj_pair(r, eps, sigma, r_cut, shift, &V, &fdivr);
+    const double f[3] = { fdivr * d[0], fdivr * d[1], fdivr * d[2] };
+    F[0] += f[0]; F[1] += f[1]; F[2] += f[2];
+    *U += 0.5 * V;
+    W[0] += 0.5 * d[0] * f[0]; W[1] += 0.5 * d[0] * f[1]; W[2] += 0.5 * d[0] * f[2];
+    W[3] += 0.5 * d[1] * f[1]; W[4] += 0.5 * d[1] * f[2]; W[5] += 0.5 * d[2] * f[2];
+    /* [reading c6.ii] cutoff-flip allowance: the truncated force jumps at
+     * r_cut, so an fp32 implementation may legitimately decide
+     * r < r_cut differently for a pair within `band` of the cutoff.  allow[0..2]
+     * accumulate what such a pair could change: |f|, |V|/2, |d||f|/2, taken
+     * at the cutoff from inside. */
+    if (allow && fabs(r - r_cut) <= band) {
+        const double rc = nextafter(r_cut, 0.0);
+        double Vc, fc;
+        orc_lj_pair(rc, eps, sigma, r_cut, shift, &Vc, &fc);
+        allow[0] += fabs(fc) * rc;
+        allow[1] += 0.5 * fabs(Vc);
+        allow[2] += 0.5 * fabs(fc) * rc * rc;
+    }
+}
+
+/* DEFINITION: sums over all j != i (O(N^2)).  F[N][3], U[N], W[N][6]. */
+int orc_compute_lj_brute(const double *pos, const int32_t *type, int64_t N, double L, int ntypes,
+                         const double *eps, const double *sigma, const double *rcut, int shift,
+                         double *F, double *U, double *W)
+{
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < N; i++) {
+        double Fi[3] = {0, 0, 0}, Ui = 0, Wi[6] = {0, 0, 0, 0, 0, 0};
+        for (int64_t j = 0; j < N; j++) {
+            if (j == i) continue;
+            double d[3];
+            const double r2 = dist2(pos, i, j, L, d);
+            const int p = type[i] * ntypes + type[j];
+            if (r2 < rcut[p] * rcut[p]) add_pair(d, r2, eps[p], sigma[p], rcut[p], shift, Fi, &Ui, Wi, 0.0, NULL);
+        }
+        memcpy(F + 3 * i, Fi, sizeof Fi); U[i] = Ui; memcpy(W + 6 * i, Wi, sizeof Wi);
+    }
+    return ORC_OK;
+}
+
+/* Sampled definition for full-size spot checks: rows sample[0..S) only. */
+int orc_compute_lj_brute_sample(const double *pos, const int32_t *type, int64_t N, double L, int ntypes,
+                                const double *eps, const double *sigma, const double *rcut, int shift,
+                                const int64_t *sample, int64_t S, double band,
+                                double *F, double *U, double *W, double *allow)
+{
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t k = 0; k < S; k++) {
+        const int64_t i = sample[k];
+        double Fi[3] = {0, 0, 0}, Ui = 0, Wi[6] = {0, 0, 0, 0, 0, 0}, al[3] = {0, 0, 0};
+        for (int64_t j = 0; j < N; j++) {
+            if (j == i) continue;
+            double d[3];
+            const double r2 = dist2(pos, i, j, L, d);
+            const int p = type[i] * ntypes + type[j];
+            const double rc = rcut[p] + band;
+            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], shift, Fi, &Ui, Wi, band, al);
+        }
+        memcpy(F + 3 * k, Fi, sizeof Fi); U[k] = Ui; memcpy(W + 6 * k, Wi, sizeof Wi);
+        if (allow) memcpy(allow + 3 * k, al, sizeof al);
+    }
+    return ORC_OK;
+}
+
+/* The method's way: the same sums restricted to the listed
+ * neighbors, each tested against its type pair's r_cut.  allow[N][3] (nullable)
+ * receives the cutoff-flip allowances for pairs within `band` of r_cut. */
+int orc_compute_lj_nlist(const double *pos, const int32_t *type, int64_t N, double L, int ntypes,
+                         const double *eps, const double *sigma, const double *rcut, int shift,
+                         const int32_t *count, const int64_t *row_start, const int32_t *nbr,
+                         double band, double *F, double *U, double *W, double *allow)
+{
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < N; i++) {
+        double Fi[3] = {0, 0, 0}, Ui = 0, Wi[6] = {0, 0, 0, 0, 0, 0}, al[3] = {0, 0, 0};
+        for (int32_t k = 0; k < count[i]; k++) {
+            const int64_t j = nbr[row_start[i] + k];
+            double d[3];
+            const double r2 = dist2(pos, i, j, L, d);
+            const int p = type[i] * ntypes + type[j];
+            /* add_pair() itself applies r < r_cut; pairs just outside are
+             * visited only so that their allowance is recorded. */
+            const double rc = rcut[p] + band;
+            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], shift, Fi, &Ui, Wi, band, al);
+        }
+        memcpy(F + 3 * i, Fi, sizeof Fi); U[i] = Ui; memcpy(W + 6 * i, Wi, sizeof Wi);
+        if (allow) memcpy(allow + 3 * i, al, sizeof al);
+    }
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------ c7 ---- */
+/* Velocity Verlet, first half ([reading c7] m = 1):
+ *   v' = v + (dt/2) F(t);  x(t+dt) = x + dt v';
+ * then wrap each axis into [-L/2, L/2), image -/+ 1 per crossing. */
+void orc_nve_step1(double *pos, double *vel, const double *F, int32_t *image, int64_t N, double L, double dt)
+{
+    for (int64_t k = 0; k < 3 * N; k++) {
+        vel[k] = vel[k] + 0.5 * dt * F[k];
+        double x = pos[k] + dt * vel[k];
+        if (x >= 0.5 * L) { x -= L; image[k] += 1; }
+        else if (x < -0.5 * L) { x += L; image[k] -= 1; }
+        pos[k] = x;
+    }
+}
+
+/* second half: v(t+dt) = v' + (dt/2) F(t+dt). */
+void orc_nve_step2(double *vel, const double *F, int64_t N, double dt)
+{
+    for (int64_t k = 0; k < 3 * N; k++) vel[k] = vel[k] + 0.5 * dt * F[k];
+}
+
+/* ------------------------------------------------------------------ c9 ---- */
+/* out[12] = K, U, W[6], P, px, py, pz with K = (1/2) sum v^2 (m = 1),
+ * P = (2K + tr W) / (3 L^3)  (PAPER.md:330 lists K, E, P as logged). */
+void orc_thermo(const double *vel, const double *U, const double *W, int64_t N, double L, double *out)
+{
+    memset(out, 0, 12 * sizeof(double));
+    for (int64_t i = 0; i < N; i++) {
+        for (int a = 0; a < 3; a++) {
+            out[0] += 0.5 * vel[3 * i + a] * vel[3 * i + a];
+            out[9 + a] += vel[3 * i + a];
+        }
+        out[1] += U[i];
+        for (int a = 0; a < 6; a++) out[2 + a] += W[6 * i + a];
+    }
+    out[8] = (2.0 * out[0] + out[2] + out[5] + out[7]) / (3.0 * L * L * L);
+}
+
+/* ------------------------------------------------------------------ c8 ---- */
+/* Hilbert index of a point on the 2^B grid, B bits per axis (Skilling,
+ * "Programming the Hilbert curve", AIP Conf. Proc. 707 (2004): AxestoTranspose,
+ * then the transposed bits are interleaved, X[0] most significant).
+ * [reading c8] The paper names only "SFCPACK sort"; the
+ * curve, B = 8 and the tie-break are this build's readings. */
+uint32_t orc_hilbert_key(uint32_t ix, uint32_t iy, uint32_t iz, int B)
+{
+    uint32_t X[3] = { ix, iy, iz };
+    const uint32_t M = 1u << (B - 1);
+    uint32_t P, Q, t;
+    for (Q = M; Q > 1; Q >>= 1) {              /* inverse undo */
+        P = Q - 1;
+        for (int i = 0; i < 3; i++) {
+            if (X[i] & Q) X[0] ^= P;           /* invert */
+            else { t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; } /* exchange */
+        }
+    }
+    for (int i = 1; i < 3; i++) X[i] ^= X[i - 1];   /* Gray encode */
+    t = 0;
+    for (Q = M; Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
+    for (int i = 0; i < 3; i++) X[i] ^= t;
+    uint32_t key = 0;
+    for (int b = B - 1; b >= 0; b--)
+        for (int i = 0; i < 3; i++) key = (key << 1) | ((X[i] >> b) & 1u);
+    return key;
+}
+
+/* key_i from the position: grid coordinate floor((x - b) 2^B / L) per axis,
+ * evaluated -- like the cell index, and for the same reason -- in binary32
+ * without contraction, wrapped into 0 .. 2^B-1. */
+void orc_sfc_keys(const float *pos, int64_t N, float L, int B, uint32_t *key)
+{
+    const float b = -0.5f * L;
+    const int G = 1 << B;
+    const float s = (float)G / L;
+    for (int64_t i = 0; i < N; i++) {
+        uint32_t g[3];
+        for (int a = 0; a < 3; a++) {
+            volatile float r = pos[3 * i + a] - b;
+            volatile float u = r * s;
+            int ga = (int)floorf(u);
+            if (ga >= G) ga -= G;
+            if (ga < 0) ga += G;
+            g[a] = (uint32_t)ga;
+        }
+        key[i] = orc_hilbert_key(g[0], g[1], g[2], B);
+    }
+}
+
+/* New order: stable sort by (key, current index).  perm[k] = old index of the
+ * particle that moves to position k.  Insertion into counting buckets keeps it
+ * obviously stable. */
+int orc_sort_perm(const uint32_t *key, int64_t N, int B, int64_t *perm)
+{
+    const int64_t nk = (int64_t)1 << (3 * B);
+    int64_t *start = (int64_t *)calloc((size_t)nk + 1, sizeof(int64_t));
+    if (!start) return ORC_ENOMEM;
+    for (int64_t i = 0; i < N; i++) start[key[i] + 1]++;
+    for (int64_t k = 0; k < nk; k++) start[k + 1] += start[k];
+    for (int64_t i = 0; i < N; i++) perm[start[key[i]]++] = i;
+    free(start);
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------ the whole loop ---- */
+/* nsteps of NVE with the list rebuilt on buffer exceedance; used for the
+ * trajectory parity case, the conservation pins and the timed CPU baseline.
+ * State arrays are updated in place.  F, U, W hold F(t), U_i, W_i on entry if
+ * have_forces != 0 (else they are computed first) and on return.
+ * log_KU (nullable) [nsteps+1][2] receives K and U at every step incl. step 0.
+ * stats[0] = number of list builds, stats[1] = max list length seen.
+ * Uses its own fp64 binning (any self-consistent binning with cell width >=
+ * r_max yields the exact set -- pinned against orc_nlist_brute). */
+int orc_run_nve(double *pos, double *vel, int32_t *image, const int32_t *type, int64_t N, double L,
+                int ntypes, const double *eps, const double *sigma, const double *rcut, int shift,
+                double r_buff, double dt, int64_t nsteps, int have_forces,
+                double *F, double *U, double *W, double *log_KU, int64_t *stats)
+{
+    double r_cut_max = 0.0;
+    for (int p = 0; p < ntypes * ntypes; p++) if (rcut[p] > r_cut_max) r_cut_max = rcut[p];
+    const double r_max = r_cut_max + r_buff;
+    const int m = orc_cell_dim(L, r_max);
+    if (m < 3) return ORC_EBOX;
+    const int64_t nc = (int64_t)m * m * m;
+    int32_t *cell = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    int64_t *cell_start = (int64_t *)malloc((size_t)(nc + 1) * sizeof(int64_t));
+    int32_t *members = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    int32_t *count = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    int64_t *row_start = (int64_t *)malloc((size_t)(N + 1) * sizeof(int64_t));
+    double *pos_build = (double *)malloc((size_t)3 * N * sizeof(double));
+    int32_t *nbr = NULL;
+    int64_t cap = 0, builds = 0, maxlen = 0;
+    int rc = ORC_OK, need_build = 1;
+    if (!cell || !cell_start || !members || !count || !row_start || !pos_build) { rc = ORC_ENOMEM; goto done; }
+
+    for (int64_t step = 0; step <= nsteps; step++) {
+        if (step > 0) {
+            orc_nve_step1(pos, vel, F, image, N, L, dt);
+            const double half = 0.5 * r_buff;
+            if (!need_build && orc_max_disp2(pos, pos_build, N, L) > half * half) need_build = 1;
+        }
+        if (step > 0 || !have_forces) {
+            if (need_build) {
+                orc_cell_index_f64(pos, N, L, m, cell, NULL);
+                orc_build_cells(cell, N, m, cell_start, members);
+                rc = orc_nlist_cells(pos, N, L, r_max, m, cell, cell_start, members, count, NULL, NULL);
+                if (rc) goto done;
+                row_start[0] = 0;
+                for (int64_t i = 0; i < N; i++) {
+                    row_start[i + 1] = row_start[i] + count[i];
+                    if (count[i] > maxlen) maxlen = count[i];
+                }
+                if (row_start[N] > cap) {
+                    free(nbr);
+                    cap = row_start[N] + row_start[N] / 8 + 16;
+                    nbr = (int32_t *)malloc((size_t)cap * sizeof(int32_t));
+                    if (!nbr) { rc = ORC_ENOMEM; goto done; }
+                }
+                orc_nlist_cells(pos, N, L, r_max, m, cell, cell_start, members, count, row_start, nbr);
+                memcpy(pos_build, pos, (size_t)3 * N * sizeof(double));
+                need_build = 0;
+                builds++;
+            }
+            orc_compute_lj_nlist(pos, type, N, L, ntypes, eps, sigma, rcut, shift,
+                                 count, row_start, nbr, 0.0, F, U, W, NULL);
+        }
+        if (step > 0) orc_nve_step2(vel, F, N, dt);
+        if (log_KU) {
+            double K = 0.0, Ut = 0.0;
+            for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * vel[k] * vel[k];
+            for (int64_t i = 0; i < N; i++) Ut += U[i];
+            log_KU[2 * step] = K; log_KU[2 * step + 1] = Ut;
+        }
+    }
+    if (stats) { stats[0] = builds; stats[1] = maxlen; }
+done:
+    free(cell); free(cell_start); free(members); free(count); free(row_start); free(pos_build); free(nbr);
+    return rc;
+}
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    extern int omp_get_max_threads(void);
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,461 @@
+"""Pins of the oracle (oracle/orc.c) to things other than itself: closed forms,
+O(N^2) brute force, invariants, the paper's Table 2.  CPU only.
+
+Each test names the oracle part it pins and the
+mistake it is meant to catch.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from paper_1308_5587_b200 import workloads as wl
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rows(name):
+    with open(os.path.join(GOLDEN, name)) as f:
+        return [ln.split() for ln in f if ln.strip() and not ln.startswith("#")]
+
+
+def _small_params(orc, w):
+    return orc.Params.of(w)
+
+
+# ----------------------------------------------------------------- c4, c5 ----
+def test_lj_pair_closed_forms(orc):
+    """c4: hand-worked rational values (golden/lj_closed_form.txt).  F(r) = f * r."""
+    for rn, rd, vn, vd, fn, fd in _rows("lj_closed_form.txt"):
+        r = Fraction(int(rn), int(rd))
+        V, fdivr = orc.lj_pair(float(r), 1.0, 1.0, 10.0, 0)
+        assert V == pytest.approx(float(Fraction(int(vn), int(vd))), rel=1e-13, abs=1e-13)
+        assert fdivr * float(r) == pytest.approx(float(Fraction(int(fn), int(fd))), rel=1e-13)
+
+
+def test_lj_minimum_and_scaling(orc):
+    """c4: minimum at 2^(1/6) sigma with depth -eps; eps scales V and F linearly,
+    sigma scales lengths (catches swapped eps/sigma, wrong exponent)."""
+    for eps, sigma in [(1.0, 1.0), (1.5, 0.8), (0.5, 0.88)]:
+        rmin = 2.0 ** (1.0 / 6.0) * sigma
+        V, f = orc.lj_pair(rmin, eps, sigma, 10.0, 0)
+        assert V == pytest.approx(-eps, rel=1e-12)
+        assert abs(f) < 1e-11
+        V1, f1 = orc.lj_pair(1.3, 1.0, 1.0, 10.0, 0)
+        V2, f2 = orc.lj_pair(1.3 * sigma, eps, sigma, 10.0, 0)
+        assert V2 == pytest.approx(eps * V1, rel=1e-12)
+        assert f2 == pytest.approx(eps * f1 / sigma ** 2, rel=1e-12)
+
+
+def test_force_is_minus_gradient(orc):
+    """c4: -(1/r) dV/dr against a central difference of V."""
+    for r in np.linspace(0.9, 2.9, 41):
+        h = 1e-6
+        Vp, _ = orc.lj_pair(r + h, 1.0, 1.0, 10.0, 0)
+        Vm, _ = orc.lj_pair(r - h, 1.0, 1.0, 10.0, 0)
+        _, fdivr = orc.lj_pair(r, 1.0, 1.0, 10.0, 0)
+        assert fdivr * r == pytest.approx(-(Vp - Vm) / (2 * h), rel=1e-7, abs=1e-8)
+
+
+def test_shift_and_cutoff(orc):
+    """c5: V(r_cut-) -> 0 in shift mode, force unchanged by the shift, zero at and
+    beyond r_cut; literature values of V_lj(r_cut)."""
+    assert orc.lj_pair(3.0 - 1e-12, 1, 1, 10.0, 0)[0] == pytest.approx(-5.479441744e-3, rel=1e-9)
+    assert orc.lj_pair(2.5 - 1e-12, 1, 1, 10.0, 0)[0] == pytest.approx(-1.631689114e-2, rel=1e-9)
+    for rc in (3.0, 2.5, 2.0 ** (1 / 6)):
+        Vs, fs = orc.lj_pair(0.9 * rc, 1, 1, rc, 1)
+        Vn, fn = orc.lj_pair(0.9 * rc, 1, 1, rc, 0)
+        Vc, _ = orc.lj_pair(rc - 1e-13, 1, 1, rc, 0)
+        assert fs == fn
+        assert Vs == pytest.approx(Vn - Vc, rel=1e-9, abs=1e-12)
+        assert abs(orc.lj_pair(rc - 1e-13, 1, 1, rc, 1)[0]) < 1e-10
+        assert orc.lj_pair(rc, 1, 1, rc, 1) == (0.0, 0.0)
+        assert orc.lj_pair(rc * 1.01, 1, 1, rc, 0) == (0.0, 0.0)
+    # WCA: purely repulsive, V >= 0 everywhere inside the cutoff
+    rc = 2.0 ** (1 / 6)
+    for r in np.linspace(0.8, rc - 1e-9, 50):
+        V, f = orc.lj_pair(r, 1, 1, rc, 1)
+        assert V >= 0 and f >= 0
+    # Kob-Andersen shifts (eps_ab * V_lj(2.5 sigma)/eps): PAPER.md:314 with per-pair tables
+    for eps, sig in [(1.0, 1.0), (1.5, 0.8), (0.5, 0.88)]:
+        Vc, _ = orc.lj_pair(2.5 * sig - 1e-13, eps, sig, 10.0, 0)
+        assert Vc == pytest.approx(eps * -1.631689114e-2, rel=1e-8)
+
+
+# ----------------------------------------------------------------- c1 -------
+@pytest.mark.parametrize("name,N", [("lj_1k", 1000), ("lj_64k", 8000), ("wca_256k", 4096), ("ka_1m", 8000)])
+def test_cell_index_invariants(orc, name, N):
+    """c1: every particle once, inside its cell's bounds; fp32 canonical value
+    equals the fp64 geometric one away from faces."""
+    w = wl.scaled(wl.CONFIGS[name], N)
+    s = wl.make_state(w)
+    m = orc.cell_dim(s.L, w.r_max)
+    assert m >= 3 and s.L / m >= w.r_max and s.L / (m + 1) < w.r_max
+    c32 = orc.cell_index_f32(s.pos, s.L, m)
+    c64, margin = orc.cell_index_f64(s.pos.astype(np.float64), s.L, m)
+    far = margin > 2.0 ** -18
+    assert np.array_equal(c32[far], c64[far])
+    assert np.mean(far) > 0.99
+    start, members = orc.build_cells(c32, m)
+    assert start[0] == 0 and start[-1] == N
+    assert np.array_equal(np.sort(members), np.arange(N))
+    # geometric containment, independent of the formula's form
+    width = s.L / m
+    for c in np.unique(c32)[:50]:
+        ids = members[start[c]:start[c + 1]]
+        cx, cy, cz = c % m, (c // m) % m, c // (m * m)
+        lo = np.array([cx, cy, cz]) * width - s.L / 2
+        p = s.pos[ids].astype(np.float64)
+        assert np.all(p >= lo - 1e-4) and np.all(p < lo + width + 1e-4)
+
+
+def test_cell_index_wraps_at_upper_face(orc):
+    """c1.iii: a coordinate that scales to exactly m wraps to cell 0, not m."""
+    L = np.float32(13.782)
+    m = 4
+    x = np.nextafter(np.float32(L / 2), np.float32(0))
+    pos = np.array([[x, 0, 0], [-L / 2, 0, 0]], dtype=np.float32)
+    c = orc.cell_index_f32(pos, L, m)
+    assert np.all((c % m >= 0) & (c % m < m))
+    assert c[1] % m == 0
+
+
+# ----------------------------------------------------------------- c2 -------
+def _as_sets(count, row_start, nbr):
+    return [set(nbr[row_start[i]:row_start[i] + count[i]].tolist()) for i in range(len(count))]
+
+
+@pytest.mark.parametrize("name,N", [("lj_1k", 1000), ("lj_64k", 1728), ("wca_256k", 1331), ("ka_1m", 2000)])
+def test_cell_nlist_equals_brute_force(orc, name, N):
+    """c2: Algorithm 3 reaches exactly the O(N^2) definition (all five density /
+    cutoff combinations appear in these four fluids + lj_1m == lj_64k's fluid)."""
+    w = wl.scaled(wl.CONFIGS[name], N)
+    s = wl.make_state(w)
+    pos = s.pos.astype(np.float64)
+    cb, rb, nb = orc.nlist_brute(pos, s.L, w.r_max)
+    m = orc.cell_dim(s.L, w.r_max)
+    for cell in (None, orc.cell_index_f32(s.pos, s.L, m)):
+        cc, rc, nc = orc.nlist_cells(pos, s.L, w.r_max, m, cell)
+        assert np.array_equal(cb, cc)
+        assert _as_sets(cb, rb, nb) == _as_sets(cc, rc, nc)
+
+
+def test_nlist_faces_corners_and_symmetry(orc):
+    """c2: particles exactly on faces / edges / corners and pairs that interact
+    across one, two and three periodic faces; full list, symmetric, no self, no
+    duplicates."""
+    L = float(np.float32(12.0))
+    r_max = 3.4
+    h = L / 2
+    pts = [[-h, -h, -h], [h - 0.5, h - 0.5, h - 0.5],          # across three faces
+           [-h, 0.0, 0.0], [h - 1.0, 0.2, 0.1],                # across one face
+           [-h + 0.1, -h + 0.2, 1.0], [h - 0.3, h - 0.4, 1.5], # across two faces
+           [0.0, 0.0, 0.0], [3.3, 0.0, 0.0], [0.0, 3.5, 0.0]]  # inside / outside r_max
+    rng = np.random.default_rng(7)
+    pts = np.array(pts + ((rng.random((400, 3)) - 0.5) * L).tolist())
+    pts = np.float32(pts).astype(np.float64)
+    cb, rb, nb = orc.nlist_brute(pts, L, r_max)
+    cc, rc, nc = orc.nlist_cells(pts, L, r_max)
+    sb, sc = _as_sets(cb, rb, nb), _as_sets(cc, rc, nc)
+    assert sb == sc
+    assert 1 in sb[0] and 3 in sb[2] and 5 in sb[4] and 7 in sb[6] and 8 not in sb[6]
+    for i, s in enumerate(sb):
+        assert i not in s and len(s) == cb[i]
+        for j in s:
+            assert i in sb[j]
+
+
+def test_nlist_mean_length_uniform_gas(orc):
+    """c2: mean list length of an ideal gas = (4/3) pi r_max^3 rho (N-1)/N
+    (catches a wrong radius, a half list, a missed image)."""
+    N, rho, r_max = 6000, 0.382, 3.4
+    s = wl.uniform_random_state(N, (N / rho) ** (1 / 3), 1.0, seed=3)
+    c, _, _ = orc.nlist_cells(s.pos.astype(np.float64), s.L, r_max)
+    expect = 4 / 3 * math.pi * r_max ** 3 * (N - 1) / s.L ** 3
+    assert c.mean() == pytest.approx(expect, rel=0.01)
+
+
+def test_nlist_rejects_small_box(orc):
+    pos = np.zeros((4, 3))
+    with pytest.raises(RuntimeError):
+        orc.nlist_cells(pos, 6.0, 3.4, m=1, cell=np.zeros(4, dtype=np.int32))
+
+
+# ----------------------------------------------------------------- c6 -------
+def test_two_particles_by_hand(orc):
+    """c6: one pair at r = 2 along x across the periodic face.  F_0 = f * d with
+    d = minimage(R_0 - R_1); U_i = V/2 each; W_xx = d_x f_x / 2 each."""
+    L = 10.0
+    pos = np.array([[4.5, 0, 0], [-3.5, 0, 0]])  # separation 8 -> image distance 2, d_0 = -2
+    typ = np.zeros(2, dtype=np.int32)
+    p = orc.Params(1, [1.0], [1.0], [3.0], 0)
+    F, U, W = orc.compute_lj_brute(pos, typ, L, p)
+    Fmag = -93 / 512                       # -dV/dr at r = 2 (attractive)
+    assert F[0] == pytest.approx([-2 * Fmag / 2, 0, 0], abs=1e-14)   # pulled towards +x image
+    assert F[0, 0] > 0 and F[1, 0] == pytest.approx(-F[0, 0], abs=1e-15)
+    assert U == pytest.approx([-63 / 2048, -63 / 2048], rel=1e-13)
+    assert W[0, 0] == pytest.approx(0.5 * 2 * Fmag, rel=1e-13) and np.allclose(W[:, 1:], 0)
+
+
+def test_six_particles_translation_invariance(orc):
+    """c6 (the paper's unit-test recipe): six particles, some pairs
+    across the boundary, several (eps, sigma, r_cut).  Forces, energies and
+    virials must not change when the whole system is translated (and re-wrapped)
+    so that other pairs straddle the faces."""
+    L = 9.0
+    base = np.array([[0.1, 0.2, 0.3], [1.2, 0.1, 0.4], [0.3, 1.4, 0.2], [1.0, 1.1, 1.3], [-0.9, 0.4, 0.8], [0.5, -0.8, 1.9]])
+    typ = np.array([0, 1, 0, 1, 0, 1], dtype=np.int32)
+    for eps, sig, rc in [((1, 1.5, 1.5, 0.5), (1, 0.8, 0.8, 0.88), (2.5, 2.0, 2.0, 2.2)),
+                         ((2, 1, 1, 3), (1.1, 0.9, 0.9, 1.0), (3.0, 3.0, 3.0, 3.0))]:
+        p = orc.Params(2, eps, sig, rc, 1)
+        ref = orc.compute_lj_brute(base, typ, L, p)
+        assert np.abs(ref[0]).max() > 1.0
+        for t in ([4.3, 0, 0], [4.3, -4.2, 0], [4.0, 4.1, -4.4], [-3.9, 3.7, 4.45]):
+            moved = base + np.array(t)
+            moved -= L * np.floor((moved + L / 2) / L)
+            got = orc.compute_lj_brute(moved, typ, L, p)
+            for a, b in zip(ref, got):
+                assert np.allclose(a, b, rtol=1e-11, atol=1e-12)
+
+
+def _pair_sum_numpy(pos, typ, L, p):
+    """Independent total energy: sum over i<j pairs, vectorised."""
+    N = len(pos)
+    i, j = np.triu_indices(N, 1)
+    d = pos[i] - pos[j]
+    d -= L * np.round(d / L)
+    r = np.sqrt((d * d).sum(1))
+    k = typ[i] * p.ntypes + typ[j]
+    eps, sig, rc = p.eps[k], p.sigma[k], p.rcut[k]
+    v = lambda x: 4 * eps * ((sig / x) ** 12 - (sig / x) ** 6)
+    V = np.where(r < rc, v(r) - (v(rc) if p.shift else 0.0), 0.0)
+    return V.sum()
+
+
+@pytest.mark.parametrize("name,N", [("lj_1k", 1000), ("ka_1m", 1500), ("wca_256k", 1331)])
+def test_force_sums_newton_energy_virial(orc, name, N):
+    """c6: list-based sums == brute-force sums; Newton III (net force 1e-10
+    relative, north_star); sum U_i == pair sum; tr W == -dU/dlambda under uniform
+    scaling (catches a dropped 1/2, a sign, a transposed virial index)."""
+    w = wl.scaled(wl.CONFIGS[name], N)
+    s = wl.make_state(w)
+    pos = s.pos.astype(np.float64)
+    p = orc.Params.of(w)
+    Fb, Ub, Wb = orc.compute_lj_brute(pos, s.type, s.L, p)
+    c, r, n = orc.nlist_cells(pos, s.L, w.r_max)
+    Fl, Ul, Wl, _ = orc.compute_lj_nlist(pos, s.type, s.L, p, c, r, n)
+    assert np.allclose(Fb, Fl, rtol=1e-12, atol=1e-12)
+    assert np.allclose(Ub, Ul, rtol=1e-12, atol=1e-13) and np.allclose(Wb, Wl, rtol=1e-12, atol=1e-12)
+    assert np.linalg.norm(Fb.sum(0)) / np.abs(Fb).sum() < 1e-10
+    assert Ub.sum() == pytest.approx(_pair_sum_numpy(pos, s.type, s.L, p), rel=1e-11)
+    h = 1e-6
+    Up = orc.compute_lj_brute(pos * (1 + h), s.type, s.L * (1 + h), p)[1].sum()
+    Um = orc.compute_lj_brute(pos * (1 - h), s.type, s.L * (1 - h), p)[1].sum()
+    trW = Wb[:, 0].sum() + Wb[:, 3].sum() + Wb[:, 5].sum()
+    assert trW == pytest.approx(-(Up - Um) / (2 * h), rel=2e-5)
+    # off-diagonal components: W_xy of the system == sum over pairs d_x f_y / ... symmetric tensor
+    i, j = np.triu_indices(N, 1)
+    d = pos[i] - pos[j]
+    d -= s.L * np.round(d / s.L)
+    # rotate the configuration by 90 degrees about z: (x,y,z)->(y,-x,z) maps W_xy -> -W_xy, W_xx <-> W_yy
+    rot = np.stack([pos[:, 1], -pos[:, 0], pos[:, 2]], axis=1)
+    rot -= s.L * np.floor((rot + s.L / 2) / s.L)
+    Wr = orc.compute_lj_brute(rot, s.type, s.L, p)[2]
+    assert np.allclose(Wr[:, 0], Wb[:, 3], atol=1e-9) and np.allclose(Wr[:, 1], -Wb[:, 1], atol=1e-9)
+    assert np.allclose(Wr[:, 2], Wb[:, 4], atol=1e-9) and np.allclose(Wr[:, 4], -Wb[:, 2], atol=1e-9)
+
+
+def test_cutoff_flip_allowance(orc):
+    """c6.ii: a pair placed 1e-6 inside / outside r_cut shows up in the allowance
+    with the size of the force jump |f(r_cut)| = 0.01094 at r_cut = 3."""
+    L = 20.0
+    p = orc.Params(1, [1.0], [1.0], [3.0], 1)
+    for dr in (-1e-6, 1e-6):
+        pos = np.array([[0, 0, 0], [3.0 + dr, 0, 0]])
+        c, r, n = orc.nlist_brute(pos, L, 3.4)
+        F, U, W, A = orc.compute_lj_nlist(pos, np.zeros(2, dtype=np.int32), L, p, c, r, n, band=1e-5)
+        assert A[0, 0] == pytest.approx(0.01094, rel=2e-3)
+        assert (abs(F[0, 0]) > 0.0109) == (dr < 0)
+
+
+# ----------------------------------------------------------------- c3, c7 ---
+def test_rebuild_rule_keeps_list_complete(orc):
+    """c3: driving the pieces by hand with the r_buff/2 rule, at EVERY step every
+    pair with d < r_cut is in the current list (checked by brute force)."""
+    w = wl.scaled(wl.CONFIGS["lj_1k"], 512)
+    s = wl.make_state(w)
+    p = orc.Params.of(w)
+    pos, vel, img = s.pos.astype(np.float64), s.vel.astype(np.float64) * 3.0, s.image.copy()
+    dt, builds = 0.005, 0
+    lst = orc.nlist_cells(pos, s.L, w.r_max)
+    pos_build = pos.copy()
+    F = orc.compute_lj_nlist(pos, s.type, s.L, p, *lst)[0]
+    for step in range(60):
+        orc.nve_step1(pos, vel, F, img, s.L, dt)
+        if orc.max_disp2(pos, pos_build, s.L) > (w.r_buff / 2) ** 2:
+            lst = orc.nlist_cells(pos, s.L, w.r_max)
+            pos_build = pos.copy()
+            builds += 1
+        need = _as_sets(*orc.nlist_brute(pos, s.L, w.r_cut_max))
+        have = _as_sets(*lst)
+        assert all(a <= b for a, b in zip(need, have))
+        F = orc.compute_lj_nlist(pos, s.type, s.L, p, *lst)[0]
+        orc.nve_step2(vel, F, dt)
+    assert 2 <= builds < 60
+
+
+def test_run_nve_matches_hand_driven_loop(orc):
+    """orc_run_nve is the same loop as the pieces called one by one."""
+    w = wl.CONFIGS["lj_1k"]
+    s = wl.make_state(w)
+    p = orc.Params.of(w)
+    out = orc.run_nve(s.pos, s.vel, s.image, s.type, s.L, p, w.r_buff, w.dt, 10, log=True)
+    pos, vel, img = s.pos.astype(np.float64), s.vel.astype(np.float64), s.image.copy()
+    F = orc.compute_lj_brute(pos, s.type, s.L, p)[0]
+    for _ in range(10):
+        orc.nve_step1(pos, vel, F, img, s.L, w.dt)
+        F, U, W = orc.compute_lj_brute(pos, s.type, s.L, p)
+        orc.nve_step2(vel, F, w.dt)
+    assert np.allclose(out["pos"], pos, atol=1e-12) and np.allclose(out["vel"], vel, atol=1e-12)
+    assert np.allclose(out["F"], F, atol=1e-10) and np.array_equal(out["image"], img)
+    assert out["KU"][-1, 1] == pytest.approx(U.sum(), rel=1e-12)
+
+
+def test_velocity_verlet_reversible_and_momentum(orc):
+    """c7: k steps, v -> -v, k steps returns to the start (to round-off); total
+    momentum conserved to round-off (Table 2 DP column: 1e-19 drift)."""
+    w = wl.scaled(wl.CONFIGS["lj_1k"], 729)
+    s = wl.make_state(w)
+    p = orc.Params.of(w)
+    a = orc.run_nve(s.pos, s.vel, s.image, s.type, s.L, p, w.r_buff, w.dt, 40)
+    b = orc.run_nve(a["pos"], -a["vel"], a["image"], s.type, s.L, p, w.r_buff, w.dt, 40)
+    back = b["pos"] + b["image"] * s.L
+    assert np.allclose(back, s.pos.astype(np.float64), atol=1e-9)
+    assert np.allclose(-b["vel"], s.vel.astype(np.float64), atol=1e-9)
+    p0 = s.vel.astype(np.float64).sum(0)
+    assert np.allclose(a["vel"].sum(0), p0, atol=1e-11)
+
+
+def test_wrap_and_image_flags(orc):
+    """c7: wrap into [-L/2, L/2) with image +-1; x + image*L is continuous."""
+    L, dt = 10.0, 0.5
+    pos = np.array([[4.9, -4.9, 0.0], [4.99, 4.99, -4.99]])
+    vel = np.array([[1.0, -1.0, 0.0], [0.04, -0.04, -0.04]])
+    img = np.zeros((2, 3), dtype=np.int32)
+    un0 = pos.copy()
+    F = np.zeros((2, 3))
+    orc.nve_step1(pos, vel, F, img, L, dt)
+    assert np.all(pos >= -L / 2) and np.all(pos < L / 2)
+    assert img.tolist() == [[1, -1, 0], [1, 0, -1]]
+    assert np.allclose(pos + img * L, un0 + dt * vel, atol=1e-14)
+    assert pos[1, 0] == pytest.approx(-4.99, abs=1e-12)    # 5.01 -> -4.99
+
+
+def test_energy_fluctuation_scales_as_dt_squared(orc):
+    """c7 (Fig. 4a): velocity Verlet is second order -- halving dt
+    cuts the energy fluctuation ~4x."""
+    w = wl.scaled(wl.CONFIGS["lj_1k"], 1000)
+    s = wl.make_state(w)
+    p = orc.Params(1, [1.0], [1.0], [3.0], 1)
+    warm = orc.run_nve(s.pos, s.vel, s.image, s.type, s.L, p, w.r_buff, 0.005, 400)
+    fl = []
+    for dt in (0.008, 0.004):
+        o = orc.run_nve(warm["pos"], warm["vel"], warm["image"], s.type, s.L, p, w.r_buff, dt, int(round(1.6 / dt)), log=True)
+        E = o["KU"].sum(1)
+        fl.append(E.std())
+    assert 2.8 < fl[0] / fl[1] < 5.5
+
+
+def test_table2_energy_fluctuation_magnitude(orc):
+    """c7 + c4-c6 together against the paper's printed number (Table 2,
+    PAPER.md:383-396): |dE/E| = 2.0(1)e-5 for N=5000, rho=0.4, r_cut=2.5 shifted,
+    T=1, dt=0.005 from an EQUILIBRATED state.  Our start is a jittered lattice
+    brought to T~1 by crude velocity rescaling in this test (the paper used 1e6
+    NVT steps), so this is an order-of-magnitude pin: within a factor 1.5 (measured here: 2.11e-5)."""
+    ref = float(_rows("table2_nve.txt")[0][1])
+    N, rho, dt = 5000, 0.4, 0.005
+    w = wl.Workload("table2", N, rho, 1.0, 1, (1.0,), (1.0,), (2.5,), 0.4, dt, 0, 1, 0)
+    s = wl.make_state(w)
+    p = orc.Params.of(w)
+    pos, vel, img = s.pos, s.vel.astype(np.float64), s.image
+    for _ in range(12):                      # melt + thermalise: 12 x 150 steps, rescale to T = 1
+        o = orc.run_nve(pos, vel, img, s.type, s.L, p, 0.4, dt, 150)
+        pos, vel, img = o["pos"], o["vel"], o["image"]
+        T = (vel ** 2).sum() / (3 * N)
+        vel = vel * math.sqrt(1.0 / T)
+    o = orc.run_nve(pos, vel, img, s.type, s.L, p, 0.4, dt, 300)
+    o = orc.run_nve(o["pos"], o["vel"], o["image"], s.type, s.L, p, 0.4, dt, 2000, log=True)  # 10 tau
+    E = o["KU"].sum(1)
+    T = 2 * o["KU"][:, 0].mean() / (3 * N)
+    assert 0.9 < T < 1.1
+    dE = E.std() / abs(E.mean())
+    assert ref / 1.5 < dE < ref * 1.5, dE
+
+
+# ----------------------------------------------------------------- c8 -------
+@pytest.mark.parametrize("B", [1, 2, 3, 4])
+def test_hilbert_is_a_bijection_with_adjacent_steps(orc, B):
+    """c8: exhaustive on the 2^B grid: every index 0..8^B-1 once; consecutive
+    indices are face-adjacent grid cells (the defining property of the curve)."""
+    G = 1 << B
+    keys = {}
+    for x in range(G):
+        for y in range(G):
+            for z in range(G):
+                keys[orc.hilbert_key(x, y, z, B)] = (x, y, z)
+    assert sorted(keys) == list(range(G ** 3))
+    for k in range(G ** 3 - 1):
+        a, b = keys[k], keys[k + 1]
+        assert sum(abs(u - v) for u, v in zip(a, b)) == 1
+
+
+def test_sfc_sort_permutation(orc):
+    """c8: valid permutation, keys non-decreasing, ties keep index order."""
+    s = wl.make_state(wl.scaled(wl.CONFIGS["lj_64k"], 8000))
+    key = orc.sfc_keys(s.pos, s.L, 8)
+    assert key.max() < 1 << 24
+    perm = orc.sort_perm(key, 8)
+    assert np.array_equal(np.sort(perm), np.arange(8000))
+    ks = key[perm]
+    assert np.all(np.diff(ks.astype(np.int64)) >= 0)
+    same = np.diff(ks.astype(np.int64)) == 0
+    assert np.all(np.diff(perm)[same] > 0)
+    assert np.array_equal(perm, np.argsort(key, kind="stable"))
+    # locality: mean distance between consecutive particles is a few sigma, not L/2
+    d = s.pos[perm][1:] - s.pos[perm][:-1]
+    d -= s.L * np.round(d / s.L)
+    assert np.sqrt((d * d).sum(1)).mean() < 2.5
+
+
+# ----------------------------------------------------------------- c9 -------
+def test_thermo(orc):
+    """c9: K, U, W, P, p by direct numpy sums; ideal-gas limit P V = (2/3) K."""
+    rng = np.random.default_rng(5)
+    N, L = 300, 7.0
+    vel, U, W = rng.normal(size=(N, 3)), rng.normal(size=N), rng.normal(size=(N, 6))
+    t = orc.thermo(vel, U, W, L)
+    assert t["K"] == pytest.approx(0.5 * (vel ** 2).sum(), rel=1e-13)
+    assert t["U"] == pytest.approx(U.sum(), rel=1e-12, abs=1e-12)
+    assert [t["px"], t["py"], t["pz"]] == pytest.approx(vel.sum(0).tolist(), abs=1e-12)
+    assert t["Wyz"] == pytest.approx(W[:, 4].sum(), abs=1e-12)
+    t0 = orc.thermo(vel, U, np.zeros((N, 6)), L)
+    assert t0["P"] * L ** 3 == pytest.approx(2 / 3 * t0["K"], rel=1e-13)
+    assert t["P"] == pytest.approx((2 * t["K"] + W[:, [0, 3, 5]].sum()) / (3 * L ** 3), rel=1e-12)
+
+
+# ------------------------------------------------------------ generator -----
+def test_workload_generator_shapes():
+    for name in ("lj_1k", "wca_256k"):
+        w = wl.CONFIGS[name] if name == "lj_1k" else wl.scaled(wl.CONFIGS[name], 4000)
+        s = wl.make_state(w)
+        assert s.pos.dtype == np.float32 and s.pos.shape == (w.N, 3)
+        assert np.all(s.pos >= -s.L / 2) and np.all(s.pos < s.L / 2)
+        assert abs(s.vel.astype(np.float64).sum(0)).max() < 1e-3
+        assert (s.vel.astype(np.float64) ** 2).mean() == pytest.approx(w.T, rel=0.08)
+        s2 = wl.make_state(w)
+        assert np.array_equal(s.pos, s2.pos) and np.array_equal(s.vel, s2.vel)
+    ka = wl.make_state(wl.scaled(wl.CONFIGS["ka_1m"], 5000))
+    assert (ka.type == 0).sum() == 4000 and (ka.type == 1).sum() == 1000
+    assert wl.CONFIGS["lj_64k"].L == pytest.approx(55.128, abs=2e-3)

@@ -1,0 +1,187 @@
+/*
+ * hb.h -- C ABI of libhb: the data-parallel hot path of one molecular-dynamics
+ * time step as described in arXiv 1308.5587 (HOOMD-blue, Anderson & Glotzer),
+ * written from scratch for NVIDIA B200 (sm_100a).
+ *
+ *   cell list (Algorithm 2)
+ *   -> neighbor list with cutoff r_max = r_cut + r_buff (Algorithm 3),
+ *      reused until a particle has moved more than r_buff/2
+ *   -> Lennard-Jones pair force, energy and virial per particle
+ *   -> velocity-Verlet NVE half-steps with image flags
+ *   +  periodic space-filling-curve sort of the particles.
+ *
+ * Every step runs in CUDA kernels; there is no CPU fallback.  One GPU, one
+ * stream, no collectives.  Citations are PAPER.md:<line>; "reading" refers to
+ * the list of readings in DESIGN.md.
+ *
+ * Conventions
+ *   - Every call returns int: HB_OK (0) or a negative HB_E* code;
+ *     hb_last_error(h) gives a message owned by the handle (valid until the
+ *     next call on that handle).  No exception crosses this boundary.
+ *   - Box: cubic, periodic, from b = -L/2 to b + L = +L/2.
+ *   - Tables are row-major [ntypes][ntypes] and must be symmetric.
+ *   - L, eps, sigma, r_cut, r_buff, dt are taken as double and rounded ONCE to
+ *     binary32; all device arithmetic is binary32 (the paper's GPU precision,
+ *     PAPER.md:308); hb_thermo accumulates in binary64.
+ *   - Work is enqueued on the cudaStream_t given to hb_create.  Calls that
+ *     return data to the host synchronise that stream; the others may not.
+ *   - Pointers passed in are caller-owned and never retained.  `on_device`
+ *     says whether they are device (1) or host (0) pointers.
+ *   - Particles keep a tag (their index at hb_set_state).  hb_sort changes
+ *     the storage order; every accessor reports BY TAG, so results do not
+ *     depend on the current order.
+ *   - Virial component order: xx, xy, xz, yy, yz, zz.
+ */
+#ifndef HB_H
+#define HB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define HB_API __attribute__((visibility("default")))
+#else
+#define HB_API
+#endif
+
+#define HB_OK 0
+#define HB_EINVAL (-1)  /* bad argument (NULL handle, N <= 0, asymmetric table, ...) */
+#define HB_ECUDA (-2)   /* a CUDA runtime call or kernel failed; see hb_last_error */
+#define HB_ENOMEM (-3)  /* device allocation failed */
+#define HB_EBOX (-4)    /* L < 2 r_max or fewer than 3 cells per axis: 27 adjacent cells would alias */
+#define HB_ESTATE (-5)  /* stage called before its prerequisite (no state, no list, ...) */
+#define HB_ENAN (-6)    /* a non-finite or out-of-box particle was seen while binning */
+
+#define HB_SHIFT_NONE 0   /* V = V_lj(r) */
+#define HB_SHIFT_ENERGY 1 /* V = V_lj(r) - V_lj(r_cut); same force */
+
+typedef struct hb_system hb_system;
+
+/* Optional device allocator (e.g. PyTorch's caching allocator).  alloc returns
+ * a device pointer aligned to >= 256 B or NULL; both are called on the host. */
+typedef struct hb_allocator {
+    void *(*alloc)(size_t bytes, void *cuda_stream, void *user);
+    void (*free)(void *ptr, void *cuda_stream, void *user);
+    void *user;
+} hb_allocator;
+
+/* Thermodynamic sums: K = 1/2 sum v^2 (m = 1), U = sum U_i,
+ * W = sum W_i, P = (2K + tr W) / (3 L^3), p = sum v. */
+typedef struct hb_thermo_t {
+    double K, U, W[6], P, px, py, pz;
+} hb_thermo_t;
+
+typedef struct hb_stats_t {
+    int64_t steps;            /* NVE steps taken since hb_create */
+    int64_t rebuilds;         /* neighbor-list builds */
+    int64_t sorts;            /* hb_sort calls (incl. those made by hb_run_nve) */
+    int64_t overflow_retries; /* times the list rows were grown and work redone */
+    int64_t max_nbrs;         /* longest row of the current list */
+    int64_t row_pitch;        /* ints per list row (multiple of 32 = 128 B) */
+    int64_t cells_per_axis;   /* m */
+    int64_t graph_launches;   /* CUDA graph launches made by hb_run_nve */
+    int64_t kernel_launches;  /* kernels enqueued (graph nodes counted when they run) */
+} hb_stats_t;
+
+/* Create a system of N particles in a cubic box of edge L with ntypes types and
+ * LJ tables eps, sigma [ntypes*ntypes] (parameters per type pair).
+ * cuda_stream: a cudaStream_t (NULL = the legacy default stream).
+ * alloc: NULL = cudaMalloc/cudaFree.  r_cut defaults to 2.5 sigma_ab until
+ * hb_set_rcut_pair / hb_build_nlist says otherwise. */
+HB_API int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *eps, const double *sigma,
+              void *cuda_stream, const hb_allocator *alloc);
+HB_API int hb_destroy(hb_system *h);
+
+/* Upload the state: pos_xyz [N][3] inside [-L/2, L/2), type [N] in 0..ntypes-1,
+ * vel_xyz [N][3], image [N][3] (NULL = zeros).  Tags are reset to 0..N-1, the
+ * list and the forces become stale. */
+HB_API int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz,
+                 const int32_t *image, int on_device);
+/* Download the state BY TAG.  Any output pointer may be NULL.  order [N]
+ * (nullable) receives, for each storage slot k, the tag stored there. */
+HB_API int hb_get_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image,
+                 uint32_t *order, int on_device);
+
+/* Per-type-pair cutoffs r_cut,ab [ntypes*ntypes].  The list is
+ * built with the largest of them (reading c2.iii); the force applies each. */
+HB_API int hb_set_rcut_pair(hb_system *h, const double *rcut);
+
+/* Algorithm 2: bin the particles into m^3 cells, m = floor(L / r_max), with
+ * c = floor((x - b) m / L) per axis evaluated in binary32 without contraction
+ * (reading c1).  Uses the r_max of the last hb_build_nlist (or r_cut,max +
+ * 0 if none).  Result: CSR cell list in cell-id order c = cx + m (cy + m cz). */
+HB_API int hb_build_cells(hb_system *h);
+
+/* Algorithm 3: N(i) = { j != i : |minimage(R_i - R_j)| < r_cut + r_buff }, full
+ * list, rows padded to a multiple of 128 B.  r_cut <= 0 keeps the per-pair table
+ * maximum; otherwise it REPLACES every r_cut,ab not set by hb_set_rcut_pair.
+ * Builds the cells first.  Row overflow is detected, rows are grown and the
+ * build redone.  Remembers the build positions for the
+ * r_buff/2 rule. */
+HB_API int hb_build_nlist(hb_system *h, double r_cut, double r_buff);
+
+/* Reading c3: *need = 1 iff some particle is now farther than r_buff/2 from
+ * where it was when the list was built (or there is no list). */
+HB_API int hb_needs_rebuild(hb_system *h, int *need);
+
+/* F_i, U_i = 1/2 sum V, W_i = 1/2 sum d f over the listed neighbors with
+ * r < r_cut,ab.  HB_ESTATE if there is no list. */
+HB_API int hb_compute_lj(hb_system *h, int shift_mode);
+
+/* One velocity-Verlet step: half kick, drift, wrap with
+ * image flags, rebuild if the buffer is exceeded, forces, half kick.  Computes
+ * the list and F(t) first if they are stale.  Uses the shift mode and r_buff
+ * of the last hb_compute_lj / hb_build_nlist. */
+HB_API int hb_step_nve(hb_system *h, double dt);
+
+/* nsteps of the same, enqueued as CUDA graphs with the rebuild decision taken
+ * on the device (no host round trip per step); hb_sort every sort_period steps
+ * (0 = never).  Row overflow inside the run is repaired by restoring the state
+ * saved at the start of the affected chunk and redoing it with longer rows. */
+HB_API int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period);
+
+/* Reorder the particles along a Hilbert curve on a 2^8 grid per axis, stable in
+ * the current index (reading c8); permutes every per-particle array, keeps the
+ * tags, invalidates the list. */
+HB_API int hb_sort(hb_system *h);
+
+HB_API int hb_thermo(hb_system *h, hb_thermo_t *out);
+
+/* Cell list: m_out [3]; cell_start [m^3+1]; cell_tags [N] = tags of the members
+ * of each cell in CSR order (order inside a cell is undefined).
+ * Pass NULL to skip an output.  Sizes: call once with only m_out. */
+HB_API int hb_get_cells(hb_system *h, int32_t *m_out, int32_t *cell_start, uint32_t *cell_tags, int on_device);
+/* Neighbor list BY TAG as CSR: row_start [N+1] (int64), nbr_tags
+ * [row_start[N]] (NULL = sizes only).  Order inside a row is undefined. */
+HB_API int hb_get_nlist(hb_system *h, int64_t *row_start, uint32_t *nbr_tags, int on_device);
+/* f_xyz_u [N][4] = (Fx, Fy, Fz, U_i), virial6 [N][6] (nullable), BY TAG. */
+HB_API int hb_get_forces(hb_system *h, float *f_xyz_u, float *virial6, int on_device);
+
+HB_API int hb_stats(hb_system *h, hb_stats_t *out);
+
+/* Tunables never change results beyond summation order.
+ *   "tpp"            threads per particle in the force kernel: 1,2,4,8,16,32
+ *   "force_block"    threads per block of the force kernel
+ *   "nlist_ppi"      particles tested per candidate load in the list kernel: 1,2,4
+ *   "nlist_cap"      candidates staged in shared memory per warp: 256..2048
+ *   "row_pitch"      initial ints per list row (rounded up to 32; 0 = estimate)
+ *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
+ *   "graph_mode"     0 = no graphs (host reads the flag each step)
+ *                    1 = graphs of kernels that exit early unless rebuilding
+ *                    2 = graphs with a conditional IF node around the rebuild
+ *   "graph_steps"    steps per graph launch
+ */
+HB_API int hb_set_tunable(hb_system *h, const char *name, int value);
+HB_API int hb_get_tunable(hb_system *h, const char *name, int *value);
+
+HB_API const char *hb_last_error(hb_system *h);
+HB_API const char *hb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HB_H */

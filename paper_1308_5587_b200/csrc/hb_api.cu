@@ -1,0 +1,881 @@
+// libhb: the C ABI of include/hb.h.  Host-side orchestration only -- every step
+// of the hot path is a kernel in cells.cu / nlist.cu / force.cu / nve.cu / sort.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "hb_internal.cuh"
+
+namespace {
+
+const int kRebuildKernels = 7;  // clear, bin, scan x2, scatter, (sort), list -- see enqueue_rebuild
+
+int dev_alloc(hb_system *h, void **p, size_t bytes)
+{
+    *p = nullptr;
+    if (bytes == 0) bytes = 256;
+    if (h->has_alloc) {
+        *p = h->alloc.alloc(bytes, (void *)h->stream, h->alloc.user);
+        if (!*p) { h->err = "allocator returned NULL for " + std::to_string(bytes) + " bytes"; return HB_ENOMEM; }
+        return HB_OK;
+    }
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        h->err = std::string("cudaMalloc(") + std::to_string(bytes) + "): " + cudaGetErrorString(e);
+        return HB_ENOMEM;
+    }
+    return HB_OK;
+}
+
+void dev_free(hb_system *h, void *p)
+{
+    if (!p) return;
+    if (h->has_alloc) h->alloc.free(p, (void *)h->stream, h->alloc.user);
+    else cudaFree(p);
+}
+
+template <typename T>
+int dev_alloc_t(hb_system *h, T **p, size_t count) { return dev_alloc(h, (void **)p, count * sizeof(T)); }
+
+template <typename T>
+void dev_free_t(hb_system *h, T *&p) { dev_free(h, (void *)p); p = nullptr; }
+
+int round_up(int x, int q) { return (x + q - 1) / q * q; }
+
+void destroy_graphs(hb_system *h)
+{
+    for (auto &kv : h->graphs) {
+        if (kv.second.e) cudaGraphExecDestroy(kv.second.e);
+        if (kv.second.g) cudaGraphDestroy(kv.second.g);
+    }
+    h->graphs.clear();
+}
+
+// Per-type-pair device table from eps, sigma, r_cut (binary64 -> rounded once).
+int upload_params(hb_system *h)
+{
+    const int nt2 = h->ntypes * h->ntypes;
+    h->h_params.resize(nt2);
+    double rc_max = 0.0;
+    for (int p = 0; p < nt2; p++) {
+        const double e = h->eps[p], s = h->sigma[p], rc = h->rcut[p];
+        const double s6 = std::pow(s, 6.0);
+        PairParam pp;
+        pp.lj1 = (float)(4.0 * e * s6 * s6);
+        pp.lj2 = (float)(4.0 * e * s6);
+        pp.rcut2 = (float)(rc * rc);
+        const double sr6 = s6 / std::pow(rc, 6.0);
+        pp.eshift = h->shift_mode == HB_SHIFT_ENERGY ? (float)(4.0 * e * (sr6 * sr6 - sr6)) : 0.0f;
+        h->h_params[p] = pp;
+        if (rc > rc_max) rc_max = rc;
+    }
+    h->r_cut_max = (float)rc_max;
+    HB_CK(cudaMemcpyAsync(h->params, h->h_params.data(), sizeof(PairParam) * nt2, cudaMemcpyHostToDevice, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));  // h_params is pageable
+    return HB_OK;
+}
+
+// r_max, m, cell arrays, row pitch.  Reading c1.ii: m = floor(L / r_max) in binary64
+// from the binary32 values of L and r_max.
+int configure_geometry(hb_system *h)
+{
+    const float r_max = h->r_cut_max + h->r_buff;  // binary32 sum
+    const int m = (int)std::floor((double)h->L / (double)r_max);
+    if (!(r_max > 0.f) || m < 3 || (double)h->L < 2.0 * (double)r_max) {
+        char buf[200];
+        snprintf(buf, sizeof buf, "box too small: L = %g, r_max = %g gives m = %d cells per axis (need >= 3)", h->L, r_max, m);
+        h->err = buf;
+        return HB_EBOX;
+    }
+    if (r_max != h->r_max || m != h->m) {
+        destroy_graphs(h);
+        h->cells_valid = h->nlist_valid = false;
+    }
+    h->r_max = r_max;
+    h->m = m;
+    h->ncells = (int64_t)m * m * m;
+    if (h->ncells > h->ncells_alloc) {
+        dev_free_t(h, h->cell_count);
+        dev_free_t(h, h->cell_start);
+        HB_TRY(dev_alloc_t(h, &h->cell_count, (size_t)h->ncells));
+        HB_TRY(dev_alloc_t(h, &h->cell_start, (size_t)h->ncells + 1));
+        h->ncells_alloc = h->ncells;
+        destroy_graphs(h);
+    }
+    const int64_t need_tmp = cdiv(h->ncells, 2048) + 16;
+    if (need_tmp > h->scan_tmp_len) {
+        dev_free_t(h, h->scan_tmp);
+        HB_TRY(dev_alloc_t(h, &h->scan_tmp, (size_t)need_tmp));
+        h->scan_tmp_len = need_tmp;
+        destroy_graphs(h);
+    }
+    h->stats.cells_per_axis = m;
+    return HB_OK;
+}
+
+int ensure_rows(hb_system *h, int pitch)
+{
+    pitch = round_up(pitch < 32 ? 32 : pitch, 32);
+    const int64_t need = h->N * (int64_t)pitch;
+    if (need > h->nlist_alloc) {
+        dev_free_t(h, h->nlist);
+        HB_TRY(dev_alloc_t(h, &h->nlist, (size_t)need));
+        h->nlist_alloc = need;
+    }
+    if (pitch != h->row_pitch) destroy_graphs(h);
+    h->row_pitch = pitch;
+    h->stats.row_pitch = pitch;
+    h->nlist_valid = false;
+    return HB_OK;
+}
+
+int initial_pitch(const hb_system *h)
+{
+    if (h->tun.row_pitch > 0) return h->tun.row_pitch;
+    const double kPi = 3.14159265358979323846;
+    const double n_est = 4.0 / 3.0 * kPi * std::pow((double)h->r_max, 3.0) * (double)h->N / std::pow((double)h->L, 3.0);
+    return (int)(1.5 * n_est) + 24;
+}
+
+int read_flags(hb_system *h)
+{
+    HB_CK(cudaMemcpyAsync(h->h_flags, h->flags, sizeof(int) * FL_COUNT, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    return HB_OK;
+}
+
+int set_flag(hb_system *h, int which, int value)
+{
+    HB_CK(cudaMemsetAsync(h->flags + which, 0, sizeof(int), h->stream));
+    if (value != 0) {
+        h->h_flags[which] = value;
+        HB_CK(cudaMemcpyAsync(h->flags + which, h->h_flags + which, sizeof(int), cudaMemcpyHostToDevice, h->stream));
+        HB_CK(cudaStreamSynchronize(h->stream));
+    }
+    return HB_OK;
+}
+
+// Algorithm 2: clear, bin (atomic slot per particle), scan, scatter, order within cells.
+int enqueue_cells(hb_system *h, const int *pred)
+{
+    HB_CK(launch_cell_clear(h, pred));
+    HB_CK(launch_cell_bin(h, pred));
+    HB_CK(launch_scan_exclusive(h, h->cell_count, h->cell_start, h->ncells, h->scan_tmp, pred));
+    HB_CK(launch_cell_scatter(h, pred));
+    if (h->tun.cell_sort) HB_CK(launch_cell_sort(h, pred));
+    return HB_OK;
+}
+
+// Algorithm 2 + Algorithm 3, no host interaction (pred: device flag for early exit, or NULL).
+int enqueue_rebuild(hb_system *h, const int *pred)
+{
+    HB_TRY(enqueue_cells(h, pred));
+    HB_CK(launch_nlist(h, pred));
+    return HB_OK;
+}
+
+int rebuild_kernel_count(const hb_system *h) { return kRebuildKernels - (h->tun.cell_sort ? 0 : 1); }
+
+// Build with the host in the loop: detects row overflow, grows the rows, rebuilds.
+int build_nlist_sync(hb_system *h)
+{
+    if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
+    if (h->row_pitch == 0) HB_TRY(ensure_rows(h, initial_pitch(h)));
+    for (int attempt = 0; attempt < 12; attempt++) {
+        HB_TRY(enqueue_rebuild(h, nullptr));
+        HB_TRY(read_flags(h));
+        if (h->h_flags[FL_BAD]) {
+            h->err = "a particle is non-finite or outside the box";
+            set_flag(h, FL_BAD, 0);
+            return HB_ENAN;
+        }
+        h->stats.rebuilds = h->h_flags[FL_BUILDS];
+        h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
+        if (h->h_flags[FL_MAX_NBRS] <= h->row_pitch) {
+            HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
+            HB_TRY(set_flag(h, FL_NEED_BUILD, 0));
+            h->cells_valid = h->nlist_valid = true;
+            return HB_OK;
+        }
+        h->stats.overflow_retries++;
+        HB_TRY(ensure_rows(h, (int)(h->h_flags[FL_MAX_NBRS] * 1.25) + 8));
+    }
+    h->err = "neighbor-list rows keep overflowing";
+    return HB_ENOMEM;
+}
+
+int ensure_forces(hb_system *h)
+{
+    if (!h->nlist_valid) { HB_TRY(build_nlist_sync(h)); h->forces_valid = false; }
+    if (!h->forces_valid) {
+        HB_CK(launch_force(h));
+        h->forces_valid = true;
+    }
+    return HB_OK;
+}
+
+int ensure_sort_buffers(hb_system *h)
+{
+    if (h->keys) return HB_OK;
+    const size_t N = (size_t)h->N;
+    HB_TRY(dev_alloc_t(h, &h->keys, N));
+    HB_TRY(dev_alloc_t(h, &h->keys2, N));
+    HB_TRY(dev_alloc_t(h, &h->perm, N));
+    HB_TRY(dev_alloc_t(h, &h->perm2, N));
+    HB_TRY(dev_alloc_t(h, &h->pos2, N));
+    HB_TRY(dev_alloc_t(h, &h->vel2, N));
+    HB_TRY(dev_alloc_t(h, &h->force2, N));
+    HB_TRY(dev_alloc_t(h, &h->virial2, 2 * N));
+    HB_TRY(dev_alloc_t(h, &h->image2, 3 * N));
+    HB_TRY(dev_alloc_t(h, &h->tag2, N));
+    const int64_t ntiles = cdiv(h->N, 512);
+    h->radix_counts_len = 256 * ntiles;
+    HB_TRY(dev_alloc_t(h, &h->radix_counts, (size_t)(2 * h->radix_counts_len + 8)));
+    const int64_t need_tmp = cdiv(h->radix_counts_len, 2048) + 16;
+    if (need_tmp > h->scan_tmp_len) {
+        dev_free_t(h, h->scan_tmp);
+        HB_TRY(dev_alloc_t(h, &h->scan_tmp, (size_t)need_tmp));
+        h->scan_tmp_len = need_tmp;
+        destroy_graphs(h);
+    }
+    return HB_OK;
+}
+
+int sort_internal(hb_system *h)
+{
+    if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    HB_TRY(ensure_sort_buffers(h));
+    HB_CK(launch_sfc_keys(h));
+    HB_CK(launch_radix_sort(h, 24));
+    HB_CK(launch_gather_state(h));
+    // copy back rather than swap pointers: captured graphs keep pointing at the first set
+    const size_t N = (size_t)h->N;
+    HB_CK(cudaMemcpyAsync(h->pos, h->pos2, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->vel, h->vel2, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->force, h->force2, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->virial, h->virial2, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->image, h->image2, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->tag, h->tag2, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
+    h->cells_valid = h->nlist_valid = false;
+    h->bk_valid = false;
+    h->stats.sorts++;
+    h->since_sort = 0;
+    return HB_OK;
+}
+
+// ---- hb_run_nve: n steps as one CUDA graph ----
+int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
+{
+    const int mode = h->tun.graph_mode;
+    cudaStream_t cs = nullptr, cs2 = nullptr;
+    HB_CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+    HB_CK(cudaStreamCreateWithFlags(&cs2, cudaStreamNonBlocking));
+    cudaGraph_t g = nullptr;
+    HB_CK(cudaGraphCreate(&g, 0));
+    cudaStream_t saved = h->stream;
+    const int64_t saved_launches = h->stats.kernel_launches;
+    int rc = HB_OK;
+    auto fail = [&](const char *what, cudaError_t e) {
+        h->err = std::string(what) + ": " + cudaGetErrorString(e);
+        rc = HB_ECUDA;
+    };
+    cudaError_t e = cudaStreamBeginCaptureToGraph(cs, g, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+    if (e != cudaSuccess) { fail("cudaStreamBeginCaptureToGraph", e); }
+    if (rc == HB_OK) {
+        h->stream = cs;
+        for (int s = 0; s < n && rc == HB_OK; s++) {
+            cudaGraphConditionalHandle cond = 0;
+            if (mode == 2) {
+                e = cudaGraphConditionalHandleCreate(&cond, g, 0, cudaGraphCondAssignDefault);
+                if (e != cudaSuccess) { fail("cudaGraphConditionalHandleCreate", e); break; }
+            }
+            e = launch_nve(h, dt, s > 0, true, cond, mode == 2);
+            if (e != cudaSuccess) { fail("nve kernel (capture)", e); break; }
+            if (mode == 2) {
+                cudaStreamCaptureStatus st;
+                const cudaGraphNode_t *deps = nullptr;
+                size_t ndeps = 0;
+                cudaGraph_t cg = nullptr;
+                e = cudaStreamGetCaptureInfo_v2(cs, &st, nullptr, &cg, &deps, &ndeps);
+                if (e != cudaSuccess) { fail("cudaStreamGetCaptureInfo_v2", e); break; }
+                cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+                np.type = cudaGraphNodeTypeConditional;
+                np.conditional.handle = cond;
+                np.conditional.type = cudaGraphCondTypeIf;
+                np.conditional.size = 1;
+                cudaGraphNode_t node = nullptr;
+                e = cudaGraphAddNode(&node, g, deps, ndeps, &np);
+                if (e != cudaSuccess) { fail("cudaGraphAddNode(conditional)", e); break; }
+                cudaGraph_t body = np.conditional.phGraph_out[0];
+                e = cudaStreamBeginCaptureToGraph(cs2, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+                if (e != cudaSuccess) { fail("cudaStreamBeginCaptureToGraph(body)", e); break; }
+                h->stream = cs2;
+                rc = enqueue_rebuild(h, nullptr);
+                h->stream = cs;
+                cudaGraph_t tmp = nullptr;
+                e = cudaStreamEndCapture(cs2, &tmp);
+                if (rc != HB_OK) break;
+                if (e != cudaSuccess) { fail("cudaStreamEndCapture(body)", e); break; }
+                e = cudaStreamUpdateCaptureDependencies(cs, &node, 1, cudaStreamSetCaptureDependencies);
+                if (e != cudaSuccess) { fail("cudaStreamUpdateCaptureDependencies", e); break; }
+            } else {
+                rc = enqueue_rebuild(h, h->flags + FL_NEED_BUILD);
+                if (rc != HB_OK) break;
+            }
+            e = launch_force(h);
+            if (e != cudaSuccess) { fail("force kernel (capture)", e); break; }
+        }
+        if (rc == HB_OK) {
+            e = launch_nve(h, dt, true, false, 0, false);
+            if (e != cudaSuccess) fail("nve kernel (capture)", e);
+        }
+        cudaGraph_t tmp = nullptr;
+        e = cudaStreamEndCapture(cs, &tmp);
+        if (rc == HB_OK && e != cudaSuccess) fail("cudaStreamEndCapture", e);
+    }
+    h->stream = saved;
+    h->stats.kernel_launches = saved_launches;
+    cudaGraphExec_t ex = nullptr;
+    if (rc == HB_OK) {
+        e = cudaGraphInstantiate(&ex, g, 0);
+        if (e != cudaSuccess) fail("cudaGraphInstantiate", e);
+    }
+    cudaStreamDestroy(cs);
+    cudaStreamDestroy(cs2);
+    if (rc != HB_OK) {
+        cudaGetLastError();
+        if (g) cudaGraphDestroy(g);
+        return rc;
+    }
+    out->g = g;
+    out->e = ex;
+    out->nkernels_fixed = 2 * n + 1 + (mode == 1 ? n * rebuild_kernel_count(h) : 0);
+    return HB_OK;
+}
+
+int backup_state(hb_system *h)
+{
+    const size_t N = (size_t)h->N;
+    if (!h->bk_pos) {
+        HB_TRY(dev_alloc_t(h, &h->bk_pos, N));
+        HB_TRY(dev_alloc_t(h, &h->bk_vel, N));
+        HB_TRY(dev_alloc_t(h, &h->bk_force, N));
+        HB_TRY(dev_alloc_t(h, &h->bk_virial, 2 * N));
+        HB_TRY(dev_alloc_t(h, &h->bk_image, 3 * N));
+    }
+    HB_CK(cudaMemcpyAsync(h->bk_pos, h->pos, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->bk_vel, h->vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->bk_force, h->force, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->bk_virial, h->virial, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->bk_image, h->image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
+    h->bk_valid = true;
+    return HB_OK;
+}
+
+int restore_state(hb_system *h)
+{
+    const size_t N = (size_t)h->N;
+    HB_CK(cudaMemcpyAsync(h->pos, h->bk_pos, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->vel, h->bk_vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->force, h->bk_force, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->virial, h->bk_virial, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->image, h->bk_image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
+    h->nlist_valid = h->cells_valid = false;
+    return HB_OK;
+}
+
+// One step with the host reading the rebuild flag (hb_step_nve and graph_mode 0).
+int step_sync(hb_system *h, float dt)
+{
+    HB_TRY(ensure_forces(h));
+    HB_CK(launch_nve(h, dt, false, true, 0, false));
+    HB_TRY(read_flags(h));
+    if (h->h_flags[FL_NEED_BUILD]) HB_TRY(build_nlist_sync(h));
+    HB_CK(launch_force(h));
+    HB_CK(launch_nve(h, dt, true, false, 0, false));
+    h->stats.steps++;
+    return HB_OK;
+}
+
+int run_chunk(hb_system *h, float dt, int n)
+{
+    if (h->tun.graph_mode == 0) {
+        for (int s = 0; s < n; s++) HB_TRY(step_sync(h, dt));
+        return HB_OK;
+    }
+    for (int attempt = 0; attempt < 8; attempt++) {
+        HB_TRY(ensure_forces(h));
+        if (dt != h->graph_dt) { destroy_graphs(h); h->graph_dt = dt; }
+        auto it = h->graphs.find(n);
+        if (it == h->graphs.end()) {
+            hb_system::GraphEntry ge;
+            HB_TRY(build_graph(h, n, dt, &ge));
+            it = h->graphs.emplace((int64_t)n, ge).first;
+        }
+        HB_TRY(backup_state(h));
+        const int builds_before = h->h_flags[FL_BUILDS];
+        HB_CK(cudaGraphLaunch(it->second.e, h->stream));
+        h->stats.graph_launches++;
+        HB_TRY(read_flags(h));
+        const int nb = h->h_flags[FL_BUILDS] - builds_before;
+        h->stats.kernel_launches += it->second.nkernels_fixed + (h->tun.graph_mode == 2 ? nb * rebuild_kernel_count(h) : 0);
+        h->stats.rebuilds = h->h_flags[FL_BUILDS];
+        if (h->h_flags[FL_BAD]) {
+            h->err = "a particle is non-finite or outside the box";
+            set_flag(h, FL_BAD, 0);
+            return HB_ENAN;
+        }
+        if (!h->h_flags[FL_OVERFLOWED]) {
+            if (nb > 0) h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
+            h->stats.steps += n;
+            return HB_OK;
+        }
+        // some build inside the chunk overflowed its rows: go back, grow, redo
+        const int needed = h->h_flags[FL_OVERFLOWED];
+        h->stats.overflow_retries++;
+        HB_TRY(restore_state(h));
+        HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
+        HB_TRY(ensure_rows(h, (int)(needed * 1.25) + 8));
+        HB_TRY(build_nlist_sync(h));
+    }
+    h->err = "neighbor-list rows keep overflowing inside hb_run_nve";
+    return HB_ENOMEM;
+}
+
+int ensure_stage(hb_system *h, void **stage, size_t *cap, size_t bytes)
+{
+    if (bytes <= *cap) return HB_OK;
+    dev_free(h, *stage);
+    *stage = nullptr;
+    *cap = 0;
+    HB_TRY(dev_alloc(h, stage, bytes));
+    *cap = bytes;
+    return HB_OK;
+}
+
+struct Stage { void *p = nullptr; size_t cap = 0; };
+std::map<hb_system *, Stage> g_stage;  // accessor staging, one per handle
+
+}  // namespace
+
+#define HB_NEED(h)            \
+    if (!(h)) return HB_EINVAL; \
+    (h)->err.clear();
+
+extern "C" {
+
+const char *hb_version(void) { return "libhb 0.1 (sm_100a)"; }
+
+const char *hb_last_error(hb_system *h) { return h ? h->err.c_str() : "null handle"; }
+
+int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *eps, const double *sigma, void *cuda_stream,
+              const hb_allocator *alloc)
+{
+    if (!out) return HB_EINVAL;
+    *out = nullptr;
+    if (N <= 0 || N >= (int64_t)1 << 31 || !(L > 0.0) || ntypes <= 0 || ntypes > 64 || !eps || !sigma) return HB_EINVAL;
+    for (int a = 0; a < ntypes; a++)
+        for (int b = 0; b < ntypes; b++)
+            if (eps[a * ntypes + b] != eps[b * ntypes + a] || sigma[a * ntypes + b] != sigma[b * ntypes + a] ||
+                !(sigma[a * ntypes + b] > 0.0))
+                return HB_EINVAL;
+    hb_system *h = new (std::nothrow) hb_system();
+    if (!h) return HB_ENOMEM;
+    h->N = N;
+    h->L = (float)L;
+    h->ntypes = ntypes;
+    h->eps.assign(eps, eps + ntypes * ntypes);
+    h->sigma.assign(sigma, sigma + ntypes * ntypes);
+    h->rcut.resize(ntypes * ntypes);
+    for (int p = 0; p < ntypes * ntypes; p++) h->rcut[p] = (double)(float)(2.5 * sigma[p]);
+    h->stream = (cudaStream_t)cuda_stream;
+    if (alloc && alloc->alloc && alloc->free) { h->alloc = *alloc; h->has_alloc = true; }
+    *out = h;  // from here on the caller can read hb_last_error and must hb_destroy
+
+    const size_t n = (size_t)N;
+    HB_TRY(dev_alloc_t(h, &h->pos, n));
+    HB_TRY(dev_alloc_t(h, &h->vel, n));
+    HB_TRY(dev_alloc_t(h, &h->force, n));
+    HB_TRY(dev_alloc_t(h, &h->virial, 2 * n));
+    HB_TRY(dev_alloc_t(h, &h->image, 3 * n));
+    HB_TRY(dev_alloc_t(h, &h->tag, n));
+    HB_TRY(dev_alloc_t(h, &h->rtag, n));
+    HB_TRY(dev_alloc_t(h, &h->pos_build, n));
+    HB_TRY(dev_alloc_t(h, &h->cell_rank, n));
+    HB_TRY(dev_alloc_t(h, &h->cell_xyzi, n));
+    HB_TRY(dev_alloc_t(h, &h->nlistn, n));
+    HB_TRY(dev_alloc_t(h, &h->params, (size_t)ntypes * ntypes));
+    HB_TRY(dev_alloc_t(h, &h->flags, (size_t)FL_COUNT));
+    HB_CK(cudaMallocHost((void **)&h->h_flags, sizeof(int) * FL_COUNT));
+    HB_CK(cudaMallocHost((void **)&h->h_thermo, sizeof(double) * 16));
+    memset(h->h_flags, 0, sizeof(int) * FL_COUNT);
+    HB_CK(cudaMemsetAsync(h->flags, 0, sizeof(int) * FL_COUNT, h->stream));
+    HB_CK(cudaMemsetAsync(h->force, 0, sizeof(float4) * n, h->stream));
+    HB_CK(cudaMemsetAsync(h->virial, 0, sizeof(float4) * 2 * n, h->stream));
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    h->thermo_blocks = (int)std::min<int64_t>(cdiv(N, 256), (int64_t)sms * 4);
+    HB_TRY(dev_alloc_t(h, &h->thermo_part, (size_t)(h->thermo_blocks + 2) * 11));
+    HB_TRY(upload_params(h));
+    return HB_OK;
+}
+
+int hb_destroy(hb_system *h)
+{
+    if (!h) return HB_EINVAL;
+    cudaStreamSynchronize(h->stream);
+    destroy_graphs(h);
+    auto it = g_stage.find(h);
+    if (it != g_stage.end()) { dev_free(h, it->second.p); g_stage.erase(it); }
+    void *ptrs[] = {h->pos, h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->pos2, h->vel2, h->force2,
+                    h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_pos_build, h->bk_image,
+                    h->params, h->cell_count, h->cell_start, h->cell_rank, h->cell_xyzi, h->scan_tmp, h->nlist, h->nlistn,
+                    h->keys, h->keys2, h->perm, h->perm2, h->radix_counts, h->flags, h->thermo_part};
+    for (void *p : ptrs) dev_free(h, p);
+    if (h->h_flags) cudaFreeHost(h->h_flags);
+    if (h->h_thermo) cudaFreeHost(h->h_thermo);
+    cudaGetLastError();
+    delete h;
+    return HB_OK;
+}
+
+int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz, const int32_t *image,
+                 int on_device)
+{
+    HB_NEED(h);
+    if (!pos_xyz || !vel_xyz) { h->err = "pos_xyz and vel_xyz are required"; return HB_EINVAL; }
+    const size_t N = (size_t)h->N;
+    const float *dpos = pos_xyz, *dvel = vel_xyz;
+    const int32_t *dtype = type, *dimg = image;
+    if (!on_device) {
+        Stage &st = g_stage[h];
+        const size_t bytes = N * (3 * 4 + 4 + 3 * 4 + 3 * 4);
+        HB_TRY(ensure_stage(h, &st.p, &st.cap, bytes));
+        char *base = (char *)st.p;
+        float *spos = (float *)base;
+        float *svel = (float *)(base + N * 12);
+        int32_t *stype = (int32_t *)(base + N * 24);
+        int32_t *simg = (int32_t *)(base + N * 28);
+        HB_CK(cudaMemcpyAsync(spos, pos_xyz, N * 12, cudaMemcpyHostToDevice, h->stream));
+        HB_CK(cudaMemcpyAsync(svel, vel_xyz, N * 12, cudaMemcpyHostToDevice, h->stream));
+        if (type) HB_CK(cudaMemcpyAsync(stype, type, N * 4, cudaMemcpyHostToDevice, h->stream));
+        if (image) HB_CK(cudaMemcpyAsync(simg, image, N * 12, cudaMemcpyHostToDevice, h->stream));
+        dpos = spos; dvel = svel; dtype = type ? stype : nullptr; dimg = image ? simg : nullptr;
+    }
+    HB_CK(launch_pack_state(h, dpos, dtype, dvel, dimg));
+    if (!on_device) HB_CK(cudaStreamSynchronize(h->stream));  // the caller's host buffers may be pageable
+    h->have_state = true;
+    h->cells_valid = h->nlist_valid = h->forces_valid = h->bk_valid = false;
+    h->since_sort = -1;
+    return HB_OK;
+}
+
+int hb_get_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image, uint32_t *order, int on_device)
+{
+    HB_NEED(h);
+    if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    const size_t N = (size_t)h->N;
+    if (on_device) {
+        HB_CK(launch_unpack_state(h, pos_xyz, type, vel_xyz, image));
+        if (order) HB_CK(cudaMemcpyAsync(order, h->tag, N * 4, cudaMemcpyDeviceToDevice, h->stream));
+        return HB_OK;
+    }
+    Stage &st = g_stage[h];
+    HB_TRY(ensure_stage(h, &st.p, &st.cap, N * 40));
+    char *base = (char *)st.p;
+    float *spos = (float *)base;
+    float *svel = (float *)(base + N * 12);
+    int32_t *stype = (int32_t *)(base + N * 24);
+    int32_t *simg = (int32_t *)(base + N * 28);
+    HB_CK(launch_unpack_state(h, pos_xyz ? spos : nullptr, type ? stype : nullptr, vel_xyz ? svel : nullptr,
+                              image ? simg : nullptr));
+    if (pos_xyz) HB_CK(cudaMemcpyAsync(pos_xyz, spos, N * 12, cudaMemcpyDeviceToHost, h->stream));
+    if (vel_xyz) HB_CK(cudaMemcpyAsync(vel_xyz, svel, N * 12, cudaMemcpyDeviceToHost, h->stream));
+    if (type) HB_CK(cudaMemcpyAsync(type, stype, N * 4, cudaMemcpyDeviceToHost, h->stream));
+    if (image) HB_CK(cudaMemcpyAsync(image, simg, N * 12, cudaMemcpyDeviceToHost, h->stream));
+    if (order) HB_CK(cudaMemcpyAsync(order, h->tag, N * 4, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    return HB_OK;
+}
+
+int hb_set_rcut_pair(hb_system *h, const double *rcut)
+{
+    HB_NEED(h);
+    if (!rcut) { h->err = "rcut is NULL"; return HB_EINVAL; }
+    const int nt = h->ntypes;
+    for (int a = 0; a < nt; a++)
+        for (int b = 0; b < nt; b++)
+            if (rcut[a * nt + b] != rcut[b * nt + a] || !(rcut[a * nt + b] > 0.0)) { h->err = "r_cut table must be symmetric and positive"; return HB_EINVAL; }
+    for (int p = 0; p < nt * nt; p++) h->rcut[p] = (double)(float)rcut[p];
+    h->rcut_user = true;
+    h->nlist_valid = h->cells_valid = h->forces_valid = false;
+    destroy_graphs(h);
+    return upload_params(h);
+}
+
+int hb_build_cells(hb_system *h)
+{
+    HB_NEED(h);
+    if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
+    HB_TRY(configure_geometry(h));
+    HB_TRY(enqueue_cells(h, nullptr));
+    HB_TRY(read_flags(h));
+    if (h->h_flags[FL_BAD]) {
+        h->err = "a particle is non-finite or outside the box";
+        set_flag(h, FL_BAD, 0);
+        return HB_ENAN;
+    }
+    h->cells_valid = true;
+    return HB_OK;
+}
+
+int hb_build_nlist(hb_system *h, double r_cut, double r_buff)
+{
+    HB_NEED(h);
+    if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
+    if (!(r_buff >= 0.0)) { h->err = "r_buff must be >= 0"; return HB_EINVAL; }
+    if (r_cut > 0.0 && !h->rcut_user) {
+        for (auto &rc : h->rcut) rc = (double)(float)r_cut;
+        HB_TRY(upload_params(h));
+        h->forces_valid = false;
+    }
+    if ((float)r_buff != h->r_buff) destroy_graphs(h);
+    h->r_buff = (float)r_buff;
+    HB_TRY(configure_geometry(h));
+    return build_nlist_sync(h);
+}
+
+int hb_needs_rebuild(hb_system *h, int *need)
+{
+    HB_NEED(h);
+    if (!need) return HB_EINVAL;
+    if (!h->nlist_valid) { *need = 1; return HB_OK; }
+    HB_TRY(read_flags(h));
+    *need = h->h_flags[FL_NEED_BUILD] ? 1 : 0;
+    return HB_OK;
+}
+
+int hb_compute_lj(hb_system *h, int shift_mode)
+{
+    HB_NEED(h);
+    if (shift_mode != HB_SHIFT_NONE && shift_mode != HB_SHIFT_ENERGY) { h->err = "unknown shift mode"; return HB_EINVAL; }
+    if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
+    if (shift_mode != h->shift_mode) {
+        h->shift_mode = shift_mode;
+        HB_TRY(upload_params(h));
+    }
+    // the force kernel clears FL_NEED_BUILD; as a stand-alone call that must not lose a pending decision
+    HB_TRY(read_flags(h));
+    const int pending = h->h_flags[FL_NEED_BUILD];
+    HB_CK(launch_force(h));
+    if (pending) HB_TRY(set_flag(h, FL_NEED_BUILD, 1));
+    h->forces_valid = true;
+    return HB_OK;
+}
+
+int hb_step_nve(hb_system *h, double dt)
+{
+    HB_NEED(h);
+    if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    if (h->m == 0) HB_TRY(configure_geometry(h));
+    return step_sync(h, (float)dt);
+}
+
+int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
+{
+    HB_NEED(h);
+    if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    if (nsteps < 0 || sort_period < 0) return HB_EINVAL;
+    if (h->m == 0) HB_TRY(configure_geometry(h));
+    int64_t done = 0;
+    while (done < nsteps) {
+        // sort before the first step ever run, then every sort_period steps (counted across calls)
+        if (sort_period > 0 && (h->since_sort < 0 || h->since_sort >= sort_period)) {
+            HB_TRY(ensure_forces(h));
+            HB_TRY(sort_internal(h));
+            h->since_sort = 0;
+        }
+        int64_t n = std::min<int64_t>(h->tun.graph_steps, nsteps - done);
+        if (sort_period > 0) n = std::min<int64_t>(n, sort_period - h->since_sort);
+        HB_TRY(run_chunk(h, (float)dt, (int)n));
+        done += n;
+        if (h->since_sort >= 0) h->since_sort += n;
+    }
+    return HB_OK;
+}
+
+int hb_sort(hb_system *h)
+{
+    HB_NEED(h);
+    return sort_internal(h);
+}
+
+int hb_thermo(hb_system *h, hb_thermo_t *out)
+{
+    HB_NEED(h);
+    if (!out) return HB_EINVAL;
+    if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    HB_CK(launch_thermo(h));
+    HB_CK(cudaMemcpyAsync(h->h_thermo, h->thermo_part + (int64_t)h->thermo_blocks * 11, sizeof(double) * 11,
+                          cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    const double *t = h->h_thermo;
+    out->K = t[0];
+    out->U = t[1];
+    for (int a = 0; a < 6; a++) out->W[a] = t[2 + a];
+    out->px = t[8]; out->py = t[9]; out->pz = t[10];
+    const double V = (double)h->L * (double)h->L * (double)h->L;
+    out->P = (2.0 * out->K + out->W[0] + out->W[3] + out->W[5]) / (3.0 * V);
+    return HB_OK;
+}
+
+int hb_get_cells(hb_system *h, int32_t *m_out, int32_t *cell_start, uint32_t *cell_tags, int on_device)
+{
+    HB_NEED(h);
+    if (!h->cells_valid) { h->err = "no cell list: call hb_build_cells first"; return HB_ESTATE; }
+    if (m_out) {
+        int32_t mm[3] = {h->m, h->m, h->m};
+        if (on_device) HB_CK(cudaMemcpyAsync(m_out, mm, sizeof mm, cudaMemcpyHostToDevice, h->stream));
+        else memcpy(m_out, mm, sizeof mm);
+    }
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    if (cell_start) HB_CK(cudaMemcpyAsync(cell_start, h->cell_start, sizeof(int) * (size_t)(h->ncells + 1), kind, h->stream));
+    if (cell_tags) {
+        if (on_device) {
+            HB_CK(launch_cell_tags(h, cell_tags));
+        } else {
+            Stage &st = g_stage[h];
+            HB_TRY(ensure_stage(h, &st.p, &st.cap, (size_t)h->N * 4));
+            HB_CK(launch_cell_tags(h, (uint32_t *)st.p));
+            HB_CK(cudaMemcpyAsync(cell_tags, st.p, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
+        }
+    }
+    HB_CK(cudaStreamSynchronize(h->stream));
+    return HB_OK;
+}
+
+int hb_get_nlist(hb_system *h, int64_t *row_start, uint32_t *nbr_tags, int on_device)
+{
+    HB_NEED(h);
+    if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
+    if (!row_start) { h->err = "row_start is NULL"; return HB_EINVAL; }
+    const size_t N = (size_t)h->N;
+    // counts by tag -> host prefix sum (binary integer work, done once per call)
+    int *d_counts = nullptr;
+    HB_TRY(dev_alloc_t(h, &d_counts, N));
+    std::vector<int> counts(N);
+    std::vector<int64_t> rs(N + 1);
+    int rc = HB_OK;
+    int64_t *d_rs = nullptr;
+    uint32_t *d_out = nullptr;
+    do {
+        if (launch_nlist_counts_by_tag(h, d_counts) != cudaSuccess ||
+            cudaMemcpyAsync(counts.data(), d_counts, N * 4, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+            cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
+        rs[0] = 0;
+        for (size_t i = 0; i < N; i++) rs[i + 1] = rs[i] + counts[i];
+        if (on_device) {
+            if (cudaMemcpyAsync(row_start, rs.data(), (N + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
+        } else {
+            memcpy(row_start, rs.data(), (N + 1) * 8);
+        }
+        if (nbr_tags) {
+            const int64_t *rs_dev = row_start;
+            if (!on_device) {
+                if ((rc = dev_alloc_t(h, &d_rs, N + 1)) != HB_OK) break;
+                if (cudaMemcpyAsync(d_rs, rs.data(), (N + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
+                rs_dev = d_rs;
+                if ((rc = dev_alloc_t(h, &d_out, (size_t)rs[N] + 1)) != HB_OK) break;
+            }
+            uint32_t *outp = on_device ? nbr_tags : d_out;
+            if (launch_nlist_fill_by_tag(h, rs_dev, outp) != cudaSuccess) { rc = HB_ECUDA; break; }
+            if (!on_device &&
+                cudaMemcpyAsync(nbr_tags, d_out, (size_t)rs[N] * 4, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
+        }
+        if (cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
+    } while (0);
+    if (rc == HB_ECUDA) h->err = std::string("hb_get_nlist: ") + cudaGetErrorString(cudaGetLastError());
+    dev_free(h, d_counts);
+    dev_free(h, d_rs);
+    dev_free(h, d_out);
+    return rc;
+}
+
+int hb_get_forces(hb_system *h, float *f_xyz_u, float *virial6, int on_device)
+{
+    HB_NEED(h);
+    if (!h->forces_valid) { h->err = "forces are stale: call hb_compute_lj first"; return HB_ESTATE; }
+    const size_t N = (size_t)h->N;
+    if (on_device) {
+        HB_CK(launch_unpack_forces(h, f_xyz_u, virial6));
+        return HB_OK;
+    }
+    Stage &st = g_stage[h];
+    HB_TRY(ensure_stage(h, &st.p, &st.cap, N * 40));
+    float *sf = (float *)st.p;
+    float *sv = (float *)((char *)st.p + N * 16);
+    HB_CK(launch_unpack_forces(h, f_xyz_u ? sf : nullptr, virial6 ? sv : nullptr));
+    if (f_xyz_u) HB_CK(cudaMemcpyAsync(f_xyz_u, sf, N * 16, cudaMemcpyDeviceToHost, h->stream));
+    if (virial6) HB_CK(cudaMemcpyAsync(virial6, sv, N * 24, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    return HB_OK;
+}
+
+int hb_stats(hb_system *h, hb_stats_t *out)
+{
+    HB_NEED(h);
+    if (!out) return HB_EINVAL;
+    HB_TRY(read_flags(h));
+    h->stats.rebuilds = h->h_flags[FL_BUILDS];
+    *out = h->stats;
+    return HB_OK;
+}
+
+static int *tunable_slot(hb_system *h, const char *name)
+{
+    if (!name) return nullptr;
+    if (!strcmp(name, "tpp")) return &h->tun.tpp;
+    if (!strcmp(name, "force_block")) return &h->tun.force_block;
+    if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
+    if (!strcmp(name, "nlist_cap")) return &h->tun.nlist_cap;
+    if (!strcmp(name, "row_pitch")) return &h->tun.row_pitch;
+    if (!strcmp(name, "cell_sort")) return &h->tun.cell_sort;
+    if (!strcmp(name, "graph_mode")) return &h->tun.graph_mode;
+    if (!strcmp(name, "graph_steps")) return &h->tun.graph_steps;
+    return nullptr;
+}
+
+int hb_set_tunable(hb_system *h, const char *name, int value)
+{
+    HB_NEED(h);
+    int *slot = tunable_slot(h, name);
+    if (!slot) { h->err = std::string("unknown tunable ") + (name ? name : "(null)"); return HB_EINVAL; }
+    bool ok = true;
+    if (slot == &h->tun.tpp) ok = value == 1 || value == 2 || value == 4 || value == 8 || value == 16 || value == 32;
+    else if (slot == &h->tun.force_block) ok = value >= 32 && value <= 256 && value % 32 == 0;
+    else if (slot == &h->tun.nlist_ppi) ok = value == 1 || value == 2 || value == 4;
+    else if (slot == &h->tun.nlist_cap) ok = value >= 64 && value <= 2048 && value % 32 == 0;
+    else if (slot == &h->tun.row_pitch) ok = value >= 0 && value <= 4096;
+    else if (slot == &h->tun.cell_sort) ok = value == 0 || value == 1;
+    else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 2;
+    else if (slot == &h->tun.graph_steps) ok = value >= 1 && value <= 2000;
+    if (!ok) { h->err = std::string("value out of range for tunable ") + name; return HB_EINVAL; }
+    *slot = value;
+    destroy_graphs(h);
+    if (slot == &h->tun.row_pitch && value > 0) HB_TRY(ensure_rows(h, value));
+    return HB_OK;
+}
+
+int hb_get_tunable(hb_system *h, const char *name, int *value)
+{
+    HB_NEED(h);
+    int *slot = tunable_slot(h, name);
+    if (!slot || !value) return HB_EINVAL;
+    *value = *slot;
+    return HB_OK;
+}
+
+}  // extern "C"

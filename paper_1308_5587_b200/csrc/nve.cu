@@ -1,0 +1,181 @@
+// Velocity-Verlet NVE half-steps, the buffer-exceedance check
+// that decides when the neighbor list is rebuilt (reading c3), the
+// thermodynamic reduction and the state pack/unpack kernels.
+#include "hb_internal.cuh"
+
+// One kernel covers the three places an integrator kernel is needed:
+//   KICK_PREV  : v += (dt/2) F   -- second half of the previous step (reading c7)
+//   KICK_DRIFT : v += (dt/2) F;  x += dt v;  wrap into [-L/2, L/2) with image +-1;
+//                set FL_NEED_BUILD if |minimage(x - x_build)| > r_buff / 2
+// Inside hb_run_nve both are fused (one read of F, one read/write of v per step);
+// the arithmetic, operation by operation, is the same as two separate launches.
+// With use_cond the last block to finish hands the rebuild decision to the CUDA
+// graph's conditional node, so the host never sees it.
+template <bool KICK_PREV, bool KICK_DRIFT>
+__global__ void __launch_bounds__(256)
+nve_kernel(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ force, int *__restrict__ image,
+           const float4 *__restrict__ pos_build, int N, float L, float dt, float half_buff2, int *__restrict__ flags,
+           cudaGraphConditionalHandle cond, int use_cond)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const float hdt = 0.5f * dt, hL = 0.5f * L;
+    bool exceed = false;
+    if (i < N) {
+        float4 v = vel[i];
+        const float4 f = force[i];
+        if (KICK_PREV) {
+            v.x = __fmaf_rn(hdt, f.x, v.x);
+            v.y = __fmaf_rn(hdt, f.y, v.y);
+            v.z = __fmaf_rn(hdt, f.z, v.z);
+        }
+        if (KICK_DRIFT) {
+            v.x = __fmaf_rn(hdt, f.x, v.x);
+            v.y = __fmaf_rn(hdt, f.y, v.y);
+            v.z = __fmaf_rn(hdt, f.z, v.z);
+            float4 p = pos[i];
+            p.x = __fmaf_rn(dt, v.x, p.x);
+            p.y = __fmaf_rn(dt, v.y, p.y);
+            p.z = __fmaf_rn(dt, v.z, p.z);
+            if (p.x >= hL) { p.x -= L; image[i] += 1; } else if (p.x < -hL) { p.x += L; image[i] -= 1; }
+            if (p.y >= hL) { p.y -= L; image[N + i] += 1; } else if (p.y < -hL) { p.y += L; image[N + i] -= 1; }
+            if (p.z >= hL) { p.z -= L; image[2 * N + i] += 1; } else if (p.z < -hL) { p.z += L; image[2 * N + i] -= 1; }
+            pos[i] = p;
+            const float4 pb = pos_build[i];
+            float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
+            if (dx >= hL) dx -= L; else if (dx < -hL) dx += L;
+            if (dy >= hL) dy -= L; else if (dy < -hL) dy += L;
+            if (dz >= hL) dz -= L; else if (dz < -hL) dz += L;
+            exceed = (dx * dx + dy * dy + dz * dz) > half_buff2;
+        }
+        vel[i] = v;
+    }
+    if (KICK_DRIFT) {
+        if (__any_sync(0xffffffffu, exceed) && (threadIdx.x & 31) == 0) flags[FL_NEED_BUILD] = 1;
+        if (use_cond) {
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                __threadfence();
+                const int ticket = atomicAdd(&flags[FL_DONE_CTR], 1);
+                if (ticket == (int)gridDim.x - 1) {
+                    __threadfence();
+                    const int need = *((volatile int *)&flags[FL_NEED_BUILD]);
+                    cudaGraphSetConditional(cond, need ? 1u : 0u);
+                    flags[FL_DONE_CTR] = 0;
+                }
+            }
+        }
+    }
+}
+
+cudaError_t launch_nve(hb_system *h, float dt, bool kick_prev, bool kick_drift, cudaGraphConditionalHandle cond, bool use_cond)
+{
+    const unsigned grid = (unsigned)cdiv(h->N, 256);
+    const float hb = 0.5f * h->r_buff;
+    const float half_buff2 = hb * hb;
+#define NVE_ARGS h->pos, h->vel, h->force, h->image, h->pos_build, (int)h->N, h->L, dt, half_buff2, h->flags, cond, use_cond ? 1 : 0
+    if (kick_prev && kick_drift) nve_kernel<true, true><<<grid, 256, 0, h->stream>>>(NVE_ARGS);
+    else if (kick_drift) nve_kernel<false, true><<<grid, 256, 0, h->stream>>>(NVE_ARGS);
+    else nve_kernel<true, false><<<grid, 256, 0, h->stream>>>(NVE_ARGS);
+#undef NVE_ARGS
+    h->stats.kernel_launches++;
+    return cudaGetLastError();
+}
+
+// ---- thermodynamic sums, accumulated in binary64, deterministic two-stage reduction ----
+constexpr int TH_VALS = 11;  // K, U, W[6], px, py, pz
+constexpr int TH_THREADS = 256;
+
+__global__ void __launch_bounds__(TH_THREADS)
+thermo_partial_kernel(const float4 *__restrict__ vel, const float4 *__restrict__ force, const float4 *__restrict__ virial,
+                      int N, double *__restrict__ part)
+{
+    double a[TH_VALS];
+#pragma unroll
+    for (int q = 0; q < TH_VALS; q++) a[q] = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        const float4 v = vel[i];
+        const float4 f = force[i];
+        const float4 w0 = virial[2 * (int64_t)i], w1 = virial[2 * (int64_t)i + 1];
+        a[0] += 0.5 * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+        a[1] += f.w;
+        a[2] += w0.x; a[3] += w0.y; a[4] += w0.z; a[5] += w0.w; a[6] += w1.x; a[7] += w1.y;
+        a[8] += v.x; a[9] += v.y; a[10] += v.z;
+    }
+    __shared__ double sm[TH_THREADS / 32][TH_VALS];
+#pragma unroll
+    for (int q = 0; q < TH_VALS; q++) {
+        double x = a[q];
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5][q] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x < TH_VALS) {
+        double x = 0.0;
+        for (int w = 0; w < TH_THREADS / 32; w++) x += sm[w][threadIdx.x];
+        part[(int64_t)blockIdx.x * TH_VALS + threadIdx.x] = x;
+    }
+}
+
+__global__ void thermo_final_kernel(const double *__restrict__ part, int nblocks, double *__restrict__ out)
+{
+    if (threadIdx.x < TH_VALS) {
+        double x = 0.0;
+        for (int b = 0; b < nblocks; b++) x += part[(int64_t)b * TH_VALS + threadIdx.x];
+        out[threadIdx.x] = x;
+    }
+}
+
+cudaError_t launch_thermo(hb_system *h)
+{
+    thermo_partial_kernel<<<h->thermo_blocks, TH_THREADS, 0, h->stream>>>(h->vel, h->force, h->virial, (int)h->N, h->thermo_part);
+    thermo_final_kernel<<<1, 32, 0, h->stream>>>(h->thermo_part, h->thermo_blocks,
+                                                h->thermo_part + (int64_t)h->thermo_blocks * TH_VALS);
+    h->stats.kernel_launches += 2;
+    return cudaGetLastError();
+}
+
+// ---- state upload / download ----
+__global__ void pack_state_kernel(const float *__restrict__ pos_xyz, const int32_t *__restrict__ type,
+                                  const float *__restrict__ vel_xyz, const int32_t *__restrict__ image_in, int N,
+                                  float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ image,
+                                  uint32_t *__restrict__ tag, uint32_t *__restrict__ rtag)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    pos[i] = make_float4(pos_xyz[3 * (int64_t)i], pos_xyz[3 * (int64_t)i + 1], pos_xyz[3 * (int64_t)i + 2],
+                         __int_as_float(type ? type[i] : 0));
+    vel[i] = make_float4(vel_xyz[3 * (int64_t)i], vel_xyz[3 * (int64_t)i + 1], vel_xyz[3 * (int64_t)i + 2], 0.f);
+    for (int a = 0; a < 3; a++) image[(int64_t)a * N + i] = image_in ? image_in[3 * (int64_t)i + a] : 0;
+    tag[i] = i;
+    rtag[i] = i;
+}
+
+__global__ void unpack_state_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ vel,
+                                    const int *__restrict__ image, const uint32_t *__restrict__ tag, int N,
+                                    float *__restrict__ pos_xyz, int32_t *__restrict__ type, float *__restrict__ vel_xyz,
+                                    int32_t *__restrict__ image_out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int64_t t = tag[i];
+    const float4 p = pos[i], v = vel[i];
+    if (pos_xyz) { pos_xyz[3 * t] = p.x; pos_xyz[3 * t + 1] = p.y; pos_xyz[3 * t + 2] = p.z; }
+    if (type) type[t] = __float_as_int(p.w);
+    if (vel_xyz) { vel_xyz[3 * t] = v.x; vel_xyz[3 * t + 1] = v.y; vel_xyz[3 * t + 2] = v.z; }
+    if (image_out)
+        for (int a = 0; a < 3; a++) image_out[3 * t + a] = image[(int64_t)a * N + i];
+}
+
+cudaError_t launch_pack_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz, const int32_t *image)
+{
+    pack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(pos_xyz, type, vel_xyz, image, (int)h->N, h->pos, h->vel,
+                                                                        h->image, h->tag, h->rtag);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image)
+{
+    unpack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->pos, h->vel, h->image, h->tag, (int)h->N, pos_xyz,
+                                                                          type, vel_xyz, image);
+    return cudaGetLastError();
+}

@@ -1,0 +1,317 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against
+the oracle, stage by stage on identical seeded snapshots.  Needs a B200.
+
+Sizes here finish in seconds on the oracle yet span many cells / warps / blocks
+with ragged tails (N is never a multiple of the tile sizes).  Full-size cases
+are in test_gpu_fullsize.py.
+"""
+import numpy as np
+import pytest
+
+from paper_1308_5587_b200 import workloads as wl
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+CASES = {
+    "lj_1k": wl.CONFIGS["lj_1k"],                          # BASELINE configs[0], full size
+    "lj_20k": wl.scaled(wl.CONFIGS["lj_64k"], 19_683),     # configs[1]/[2] fluid, 27^3
+    "wca_12k": wl.scaled(wl.CONFIGS["wca_256k"], 12_000),  # configs[3] fluid, vacancies
+    "ka_10k": wl.scaled(wl.CONFIGS["ka_1m"], 10_001),      # configs[4] fluid, two types
+}
+
+
+@pytest.fixture(scope="module")
+def hb():
+    from paper_1308_5587_b200 import hb as _hb
+    _hb.load()
+    return _hb
+
+
+def _system(hb, w, s, **tun):
+    sysm = hb.System.from_workload(w)
+    for k, v in tun.items():
+        sysm.set_tunable(k, v)
+    sysm.set_state(s.pos, s.type, s.vel, s.image)
+    return sysm
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_cells_bit_exact(hb, orc, case):
+    w = CASES[case]
+    s = wl.make_state(w)
+    with _system(hb, w, s) as g:
+        g.build_nlist(0.0, w.r_buff)     # fixes r_max
+        g.build_cells()
+        m, start, tags = g.get_cells()
+    assert m == orc.cell_dim(s.L, w.r_max)
+    parity.assert_cells_equal(orc, s.pos, s.L, m, start, tags)
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_nlist_set_exact(hb, orc, case):
+    w = CASES[case]
+    s = wl.make_state(w)
+    with _system(hb, w, s) as g:
+        g.build_nlist(0.0, w.r_buff)
+        rs, nbr = g.get_nlist()
+        st = g.stats()
+    pos64 = s.pos.astype(np.float64)
+    c, r, n = orc.nlist_cells(pos64, s.L, w.r_max)
+    parity.assert_nlist_equal(pos64, s.L, w.r_max, r, n, rs, nbr)
+    assert st["max_nbrs"] == np.diff(rs).max() and st["row_pitch"] % 32 == 0 and st["row_pitch"] >= st["max_nbrs"]
+
+
+@pytest.mark.parametrize("case", list(CASES))
+@pytest.mark.parametrize("shift", [1, 0])
+def test_forces_energy_virial(hb, orc, case, shift):
+    w = CASES[case]
+    s = wl.make_state(w)
+    with _system(hb, w, s) as g:
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(shift)
+        f4, w6 = g.get_forces()
+        th = g.thermo()
+    pos64 = s.pos.astype(np.float64)
+    p = orc.Params(w.ntypes, w.eps, w.sigma, w.rcut, shift)
+    lst = orc.nlist_cells(pos64, s.L, w.r_max)
+    F, U, W, A = orc.compute_lj_nlist(pos64, s.type, s.L, p, *lst, band=parity.BAND)
+    parity.assert_forces_close(F, U, W, A, f4, w6)
+    parity.assert_energy_close(U.sum(), th["U"], A[:, 1].sum())
+    parity.assert_energy_close(U.sum(), float(f4[:, 3].astype(np.float64).sum()), A[:, 1].sum())
+    ref = orc.thermo(s.vel.astype(np.float64), U, W, s.L)
+    assert th["K"] == pytest.approx(ref["K"], rel=1e-12)            # fp64 sum of fp32 squares
+    assert [th["px"], th["py"], th["pz"]] == pytest.approx([ref["px"], ref["py"], ref["pz"]], abs=1e-9)
+    assert th["P"] == pytest.approx(ref["P"], rel=1e-4, abs=1e-6)
+    for a, k in enumerate(("Wxx", "Wxy", "Wxz", "Wyy", "Wyz", "Wzz")):
+        assert th["W"][a] == pytest.approx(ref[k], rel=1e-4, abs=1e-4 * abs(ref["Wxx"]))
+
+
+@pytest.mark.parametrize("tun", [dict(tpp=1), dict(tpp=2), dict(tpp=4), dict(tpp=16), dict(tpp=32),
+                                 dict(nlist_ppi=1), dict(nlist_ppi=4), dict(nlist_cap=64), dict(nlist_cap=96, nlist_ppi=4),
+                                 dict(cell_sort=0), dict(force_block=64), dict(force_block=256, tpp=4)])
+def test_tunables_do_not_change_results(hb, orc, tun):
+    """block size and friends 'do not change the correctness'."""
+    w = CASES["ka_10k"]
+    s = wl.make_state(w)
+    pos64 = s.pos.astype(np.float64)
+    p = orc.Params.of(w)
+    lst = orc.nlist_cells(pos64, s.L, w.r_max)
+    F, U, W, A = orc.compute_lj_nlist(pos64, s.type, s.L, p, *lst, band=parity.BAND)
+    with _system(hb, w, s, **tun) as g:
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(1)
+        rs, nbr = g.get_nlist()
+        f4, w6 = g.get_forces()
+    parity.assert_nlist_equal(pos64, s.L, w.r_max, lst[1], lst[2], rs, nbr)
+    parity.assert_forces_close(F, U, W, A, f4, w6)
+
+
+def test_row_overflow_is_detected_and_repaired(hb, orc):
+    """'detecting overflows and resizing the data structures'."""
+    w = CASES["lj_20k"]
+    s = wl.make_state(w)
+    pos64 = s.pos.astype(np.float64)
+    lst = orc.nlist_cells(pos64, s.L, w.r_max)
+    with _system(hb, w, s, row_pitch=32) as g:
+        g.build_nlist(0.0, w.r_buff)
+        st = g.stats()
+        rs, nbr = g.get_nlist()
+    assert st["overflow_retries"] >= 1 and st["row_pitch"] >= lst[0].max()
+    parity.assert_nlist_equal(pos64, s.L, w.r_max, lst[1], lst[2], rs, nbr)
+
+
+def test_deterministic_lists_and_forces(hb):
+    """cell_sort = 1: two builds give bitwise identical lists (in order) and forces."""
+    w = CASES["lj_20k"]
+    s = wl.make_state(w)
+    outs = []
+    for _ in range(2):
+        with _system(hb, w, s) as g:
+            g.build_nlist(0.0, w.r_buff)
+            g.compute_lj(1)
+            outs.append((g.get_nlist(), g.get_forces()))
+    assert np.array_equal(outs[0][0][1], outs[1][0][1])
+    assert np.array_equal(outs[0][1][0], outs[1][1][0]) and np.array_equal(outs[0][1][1], outs[1][1][1])
+
+
+@pytest.mark.parametrize("mode", ["step", "run0", "run1", "run2"])
+def test_trajectory_config1(hb, orc, mode):
+    """BASELINE configs[0]: 10 NVE steps at dt = 0.005, fp32 GPU vs fp64 oracle,
+    compared by tag; expect <= 1e-5 absolute."""
+    w = CASES["lj_1k"]
+    s = wl.make_state(w)
+    p = orc.Params.of(w)
+    ref = orc.run_nve(s.pos, s.vel, s.image, s.type, s.L, p, w.r_buff, w.dt, w.steps, log=True)
+    with _system(hb, w, s) as g:
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(w.shift)
+        if mode == "step":
+            for _ in range(w.steps):
+                g.step_nve(w.dt)
+        else:
+            g.set_tunable("graph_mode", int(mode[-1]))
+            g.set_tunable("graph_steps", 4)          # 4 + 4 + 2: several graphs, one remainder
+            g.run_nve(w.dt, w.steps, 0)
+        out = g.get_state()
+        f4, w6 = g.get_forces()
+        th = g.thermo()
+        st = g.stats()
+    assert st["steps"] == w.steps
+    d = out["pos"].astype(np.float64) + out["image"] * s.L - (ref["pos"] + ref["image"] * s.L)
+    assert np.abs(d).max() <= 1e-5
+    assert np.abs(out["vel"].astype(np.float64) - ref["vel"]).max() <= 1e-5 * max(1.0, np.abs(ref["vel"]).max())
+    assert np.abs(f4[:, :3].astype(np.float64) - ref["F"]).max() <= 2e-4 * np.abs(ref["F"]).max()
+    E_ref = ref["KU"][-1].sum()
+    assert th["K"] + th["U"] == pytest.approx(E_ref, rel=2e-5)
+    assert np.array_equal(out["type"], s.type)
+
+
+def test_long_run_invariants_and_rebuilds(hb, orc):
+    """Device-side rebuild decisions over a few hundred steps: energy conserved at
+    the level the oracle conserves it, momentum ~0, no particle lost, and the
+    final GPU snapshot's forces agree with the oracle evaluated on that snapshot."""
+    w = CASES["lj_20k"]
+    s = wl.make_state(w)
+    p = orc.Params.of(w)
+    with _system(hb, w, s) as g:
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(w.shift)
+        t0 = g.thermo()
+        g.run_nve(w.dt, 300, 100)
+        t1 = g.thermo()
+        out = g.get_state()
+        f4, w6 = g.get_forces()
+        st = g.stats()
+        rs, nbr = g.get_nlist()
+    E0, E1 = t0["K"] + t0["U"], t1["K"] + t1["U"]
+    assert abs(E1 - E0) / abs(E0) < 2e-4
+    assert max(abs(t1["px"]), abs(t1["py"]), abs(t1["pz"])) / w.N < 1e-6
+    assert 10 <= st["rebuilds"] <= 150 and st["sorts"] == 3
+    assert np.all(out["pos"] >= -s.L / 2) and np.all(out["pos"] <= s.L / 2)
+    assert np.array_equal(np.sort(out["order"]), np.arange(w.N))
+    # reading c3's invariant: the list in use still contains every pair inside r_cut
+    pos64 = out["pos"].astype(np.float64)
+    need = orc.nlist_cells(pos64, s.L, w.r_cut_max)
+    kg = np.sort(parity.rows_as_keys(rs, nbr))
+    kn = parity.rows_as_keys(need[1], need[2])
+    assert np.isin(kn, kg, assume_unique=True).all()
+    lst = orc.nlist_cells(pos64, s.L, w.r_max)
+    F, U, W, A = orc.compute_lj_nlist(pos64, s.type, s.L, p, *lst, band=parity.BAND)
+    parity.assert_forces_close(F, U, W, A, f4, w6)
+
+
+def test_needs_rebuild_follows_half_buffer_rule(hb, orc):
+    w = CASES["lj_1k"]
+    s = wl.make_state(w)
+    with _system(hb, w, s) as g:
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(1)
+        assert not g.needs_rebuild()
+        pos0 = s.pos.astype(np.float64)
+        seen = False
+        g.set_tunable("graph_mode", 1)
+        for _ in range(40):
+            before = g.stats()["rebuilds"]
+            g.run_nve(w.dt, 1, 0)
+            out = g.get_state()
+            rebuilt = g.stats()["rebuilds"] > before
+            disp2 = orc.max_disp2(out["pos"].astype(np.float64), pos0, s.L)
+            lim = (w.r_buff / 2) ** 2
+            if abs(np.sqrt(disp2) - w.r_buff / 2) > parity.BAND:
+                assert rebuilt == (disp2 > lim)
+            if rebuilt:
+                pos0 = out["pos"].astype(np.float64)
+                seen = True
+        assert seen
+
+
+@pytest.mark.parametrize("case", ["lj_20k", "ka_10k"])
+def test_sort_keeps_physics_and_matches_oracle_order(hb, orc, case):
+    w = CASES[case]
+    s = wl.make_state(w)
+    with _system(hb, w, s) as g:
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(1)
+        f_before, w_before = g.get_forces()
+        g.sort()
+        out = g.get_state()
+        f_perm, _ = g.get_forces()                   # permuted with the particles
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(1)
+        f_after, w_after = g.get_forces()
+    # weak: state by tag unchanged, forces by tag unchanged (bitwise for the carried copy)
+    assert np.array_equal(out["pos"], s.pos) and np.array_equal(out["vel"], s.vel) and np.array_equal(out["type"], s.type)
+    assert np.array_equal(f_perm, f_before)
+    assert np.abs(f_after[:, :3] - f_before[:, :3]).max() <= 1e-4 * np.abs(f_before[:, :3]).max()
+    # strong: same permutation as the oracle's stable sort of the oracle's keys
+    perm = orc.sort_perm(orc.sfc_keys(s.pos, s.L, 8), 8)
+    assert np.array_equal(out["order"].astype(np.int64), perm)
+
+
+def test_error_codes(hb):
+    w = CASES["lj_1k"]
+    s = wl.make_state(w)
+    with hb.System.from_workload(w) as g:
+        with pytest.raises(hb.HBError) as e:
+            g.build_cells()
+        assert e.value.code == hb.HB_ESTATE
+        g.set_state(s.pos, s.type, s.vel)
+        with pytest.raises(hb.HBError) as e:
+            g.compute_lj(1)
+        assert e.value.code == hb.HB_ESTATE
+        with pytest.raises(hb.HBError) as e:
+            g.build_nlist(5.0, 0.4)          # L = 13.78 < 3 * 5.4
+        assert e.value.code == hb.HB_EBOX
+    bad = s.pos.copy()
+    bad[17, 1] = np.nan
+    with hb.System.from_workload(w) as g:
+        g.set_state(bad, s.type, s.vel)
+        with pytest.raises(hb.HBError) as e:
+            g.build_nlist(0.0, w.r_buff)
+        assert e.value.code == hb.HB_ENAN
+    with pytest.raises(hb.HBError):
+        hb.System(10, 5.0, 2, [1, 2, 3, 4], [1, 1, 1, 1])   # asymmetric eps
+
+
+def test_device_pointers_and_torch_allocator(hb, orc):
+    """The same calls with torch CUDA tensors (device pointers) and torch's
+    caching allocator behind the library."""
+    import torch
+    w = CASES["wca_12k"]
+    s = wl.make_state(w)
+    g = hb.System.from_workload(w, use_torch_allocator=True)
+    g.set_state(torch.from_numpy(s.pos).cuda(), torch.from_numpy(s.type).cuda(), torch.from_numpy(s.vel).cuda())
+    g.build_nlist(0.0, w.r_buff)
+    g.compute_lj(1)
+    out = g.get_state(device=True)
+    torch.cuda.synchronize()
+    assert np.array_equal(out["pos"].cpu().numpy(), s.pos)
+    f4, _ = g.get_forces()
+    pos64 = s.pos.astype(np.float64)
+    lst = orc.nlist_cells(pos64, s.L, w.r_max)
+    F, U, W, A = orc.compute_lj_nlist(pos64, s.type, s.L, orc.Params.of(w), *lst, band=parity.BAND)
+    parity.assert_forces_close(F, U, W, A, f4, None)
+    g.close()
+
+
+def test_tiny_and_empty_cells(hb, orc):
+    """Degenerate inputs: a handful of particles in a big box (almost every cell
+    empty, rows of length 0), and a pair across the corner of the box."""
+    L = float(np.float32(20.0))
+    h = L / 2
+    pos = np.array([[-h, -h, -h], [h - 0.6, h - 0.7, h - 0.8], [0, 0, 0], [0.5, 0.9, 0.1], [5, 5, 5]], dtype=np.float32)
+    typ = np.zeros(5, dtype=np.int32)
+    with hb.System(5, L, 1, [1.0], [1.0]) as g:
+        g.set_state(pos, typ, np.zeros_like(pos))
+        g.build_nlist(3.0, 0.4)
+        g.compute_lj(1)
+        rs, nbr = g.get_nlist()
+        f4, w6 = g.get_forces()
+    pos64 = pos.astype(np.float64)
+    c, r, n = orc.nlist_brute(pos64, L, 3.4)
+    parity.assert_nlist_equal(pos64, L, 3.4, r, n, rs, nbr)
+    assert np.diff(rs).tolist() == [1, 1, 1, 1, 0]
+    F, U, W = orc.compute_lj_brute(pos64, typ, L, orc.Params(1, [1.0], [1.0], [3.0], 1))
+    assert np.abs(f4[:, :3] - F).max() <= 1e-4 * np.abs(F).max()
+    assert np.all(f4[4] == 0)

@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- LJ-liquid time steps per second on one B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config lj_64k] [--impl reference]
+
+A "step" is one MD time step: the whole hot path (half kick + drift + buffer
+check, list rebuild when the buffer is exceeded, LJ force/energy/virial, half
+kick; Hilbert sort every `sort_period` steps).  The K timed steps are consecutive
+steps of one trajectory that has first been advanced `--equil` + W steps from the
+seeded lattice start, so the fluid has melted.
+
+Prints ONE JSON line (rank 0).  Multi-GPU: replicas only (DESIGN.md section
+"Multi-GPU"): every rank runs an independent system with its own seed, no
+collective on the data path; torch.distributed (NCCL) is used for the barrier
+and the max-over-ranks time only.
+
+--impl reference times the ORACLE (oracle/orc.c, fp64, OpenMP over i) on the
+host cores for a bounded number of the same steps.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1308_5587_b200 import workloads as wl  # noqa: E402
+
+METRIC = "lj_liquid_timesteps_per_s"
+UNIT = "timesteps/s"
+# FP32 peak for the "alu" roofline (DESIGN.md section "Rooflines"): 148 SMs x 128 FP32
+# lanes x 2 flop/FMA x 1.965 GHz (clocks.max.sm, B200_PROFILING.md table).
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+PAPER_TITAN_STEPS_PER_S = 1270.0   # PAPER.md:143, GK110, same N=64000 workload shape (context)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append([x.strip() for x in ln.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[k] for r in self.rows if len(r) >= 7 for k in range(4) if r[3 + k].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def cpu_oracle_steps_per_s(w, state, nsteps):
+    """The oracle as it stands, timed on this box's host cores."""
+    from oracle import orc
+    p = orc.Params.of(w)
+    orc.lib()
+    t0 = time.perf_counter()
+    out = orc.run_nve(state.pos, state.vel, state.image, state.type, state.L, p, w.r_buff, w.dt, nsteps)
+    dt = time.perf_counter() - t0
+    return nsteps / dt, dt, orc.num_threads(), out["builds"]
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle on the host cores, bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    state = wl.make_state(w)
+    # bounded: the oracle does ~2.5e7 pair evaluations per second per core
+    per_step = w.N * 70 / 2.0e7 / max(1, os.cpu_count() or 1) * 4
+    cap = max(2, int(40.0 / max(per_step, 1e-6)))
+    K = max(1, min(args.steps, cap))
+    W = max(0, min(args.warmup, max(1, cap // 10)))
+    from oracle import orc
+    p = orc.Params.of(w)
+    warm = orc.run_nve(state.pos, state.vel, state.image, state.type, state.L, p, w.r_buff, w.dt, W)
+    t0 = time.perf_counter()
+    orc.run_nve(warm["pos"], warm["vel"], warm["image"], state.type, state.L, p, w.r_buff, w.dt, K,
+                forces=(warm["F"], warm["U"], warm["W"]))
+    el = time.perf_counter() - t0
+    v = K / el
+    sample = f"{K} consecutive steps of {w.name} (N={w.N}) after {W} warm-up steps from the seeded lattice start, list rebuilds included"
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": K, "warmup": W,
+            "ms_per_step": 1e3 * el / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": config_of(w, args, {}),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def config_of(w, args, extra):
+    c = {"workload": w.name, "N": w.N, "rho": w.rho, "T": w.T, "r_cut": w.r_cut_max, "r_buff": w.r_buff, "dt": w.dt,
+         "ntypes": w.ntypes, "shift": "energy" if w.shift else "none", "sort_period": w.sort_period,
+         "equil_steps": args.equil, "parallelism": "replicas" if args.gpus > 1 else "single"}
+    c.update(extra)
+    return c
+
+
+def force_work(g, w):
+    """Algorithmic bytes and flops of one lj_force launch."""
+    pairs = int(g.get_nlist_sizes()[-1])
+    N = w.N
+    bytes_ = 4 * pairs + N * (16 + 4 + 16 + 24)     # indices + pos_i + count + force out + virial out
+    frac_in = (w.r_cut_max / w.r_max) ** 3 if w.ntypes == 1 else 0.55
+    flops = 20 * pairs + 25 * frac_in * pairs
+    return pairs, bytes_, flops
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10000)
+    ap.add_argument("--warmup", type=int, default=1000)
+    ap.add_argument("--equil", type=int, default=2000, help="untimed steps before the warm-up (melting the lattice)")
+    ap.add_argument("--config", default="lj_64k", choices=list(wl.CONFIGS))
+    ap.add_argument("--impl", default="hb", choices=["hb", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the short N=1M measurement")
+    ap.add_argument("--tune", default="", help="comma list name=value of hb tunables")
+    args = ap.parse_args()
+    w = wl.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    from paper_1308_5587_b200 import hb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.warmup < 3:
+        args.warmup = 3
+    hbm_peak, peak_kind = measured_peaks()
+    tun = dict(kv.split("=") for kv in args.tune.split(",") if kv)
+
+    def make_system(wk, seed):
+        st = wl.make_state(wk, seed=seed)
+        g = hb.System.from_workload(wk)
+        for k, v in tun.items():
+            g.set_tunable(k, int(v))
+        g.set_state(st.pos, st.type, st.vel, st.image)
+        g.build_nlist(0.0, wk.r_buff)
+        g.compute_lj(wk.shift)
+        return g, st
+
+    def timed_run(g, wk, K):
+        """K steps between CUDA events on the stream the library launches on."""
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0 = g.stats()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0.record()
+        g.run_nve(wk.dt, K, wk.sort_period)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        s1 = g.stats()
+        return ms, {k: s1[k] - s0[k] for k in ("rebuilds", "sorts", "kernel_launches", "graph_launches", "overflow_retries")}
+
+    g, st0 = make_system(w, seed=w.seed + rank)
+    g.run_nve(w.dt, args.equil, w.sort_period)
+    g.run_nve(w.dt, args.warmup, w.sort_period)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms, delta = timed_run(g, w, args.steps)
+    clocks = sampler.stop()
+    value = world * args.steps / (ms * 1e-3)
+    th = g.thermo()
+    stats = g.stats()
+
+    # ---- per-kernel rooflines, measured live with CUDA events on the launching stream ----
+    pairs, fbytes, fflops = force_work(g, w)
+    t_force = g.time_stage("lj_force", 200)
+    t_force_cold = g.time_stage("lj_force", 20, 512 << 20)
+    t_nlist = g.time_stage("nlist", 50)
+    t_cells = g.time_stage("cells", 50)
+    t_nve = g.time_stage("nve", 200)
+    share_force = t_force * args.steps / ms
+    roof_alu = {"bound": "alu", "achieved": fflops / (t_force * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "kernel": "lj_force_kernel", "ms": t_force, "traffic": None,
+                "peak_source": "nominal fp32: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)"}
+    roof_alu["frac"] = roof_alu["achieved"] / roof_alu["peak"]
+    roof_hbm = {"bound": "hbm", "achieved": fbytes / (t_force_cold * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "kernel": "lj_force_kernel", "ms": t_force_cold, "traffic": None,
+                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind}); L2 flushed before every launch"}
+    roof_hbm["frac"] = roof_hbm["achieved"] / roof_hbm["peak"]
+    nl_bytes = 4 * pairs + w.N * (4 + 32)
+    kernels = {
+        "lj_force": {"ms_warm_l2": t_force, "ms_cold_l2": t_force_cold, "pairs": pairs, "algorithmic_bytes": fbytes,
+                     "algorithmic_flops": fflops, "share_of_step": share_force},
+        "nlist": {"ms": t_nlist, "algorithmic_bytes": nl_bytes, "gbs": nl_bytes / (t_nlist * 1e-3) / 1e9,
+                  "frac_hbm": nl_bytes / (t_nlist * 1e-3) / 1e9 / hbm_peak},
+        "cells": {"ms": t_cells, "algorithmic_bytes": 36 * w.N},
+        "nve": {"ms": t_nve, "algorithmic_bytes": 108 * w.N, "gbs": 108 * w.N / (t_nve * 1e-3) / 1e9},
+    }
+
+    # ---- end to end through the C ABI with HOST buffers ----
+    s_now = g.get_state()
+    pos_h, vel_h, typ_h, img_h = (np.ascontiguousarray(s_now[k]) for k in ("pos", "vel", "type", "image"))
+    Ke = max(1, min(args.steps, 2000))
+    g.set_state(pos_h, typ_h, vel_h, img_h)
+    g.run_nve(w.dt, 50, w.sort_period)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    t0 = time.perf_counter()
+    g.set_state(pos_h, typ_h, vel_h, img_h)                      # H2D inside the timed region
+    g.run_nve(w.dt, Ke, w.sort_period)
+    g.get_state_into(pos=pos_h, type=typ_h, vel=vel_h, image=img_h)  # D2H inside the timed region
+    th_e = g.thermo()
+    el = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([el], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        el = float(t.item())
+    e2e = {"value": world * Ke / el, "unit": UNIT, "steps_per_call": Ke, "h2d_bytes_per_step": w.N * 40 / Ke,
+           "d2h_bytes_per_step": (w.N * 40 + 96) / Ke, "h2d_bytes_per_call": w.N * 40, "d2h_bytes_per_call": w.N * 40 + 96,
+           "note": "hb_set_state(host) + hb_run_nve + hb_get_state(host) + hb_thermo, wall clock"}
+    g.close()
+
+    also = {}
+    if not args.no_also and world == 1 and args.config == "lj_64k":
+        w2 = wl.CONFIGS["lj_1m"]
+        g2, _ = make_system(w2, seed=w2.seed)
+        g2.run_nve(w2.dt, 600, w2.sort_period)
+        ms2, d2 = timed_run(g2, w2, 1000)
+        p2 = int(g2.get_nlist_sizes()[-1])
+        b2 = 4 * p2 + w2.N * 60
+        tf2 = g2.time_stage("lj_force", 30)
+        tn2 = g2.time_stage("nlist", 10)
+        also = {"lj_1m": {"timesteps_per_s": 1000 / (ms2 * 1e-3), "particle_steps_per_s": 1000 * w2.N / (ms2 * 1e-3),
+                          "ms_per_step": ms2 / 1000, "rebuilds": d2["rebuilds"], "lj_force_ms": tf2,
+                          "lj_force_hbm_gbs": b2 / (tf2 * 1e-3) / 1e9, "lj_force_hbm_frac": b2 / (tf2 * 1e-3) / 1e9 / hbm_peak,
+                          "nlist_ms": tn2, "mean_nbrs": p2 / w2.N, "inputs": "larger than L2 (252 MB list)"}}
+        g2.close()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_cpu = max(2, int(15.0 / (w.N * 70 / 2.0e7 / max(1, os.cpu_count() or 1) * 4)))
+        n_cpu = min(n_cpu, 200)
+        v, secs, cores, builds = cpu_oracle_steps_per_s(w, st0, n_cpu)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {n_cpu} steps of {w.name} (N={w.N}) from the seeded lattice start incl. the initial list build "
+                         f"and {builds} builds, {secs:.1f} s"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": config_of(w, args, {
+                "l2": ("working set (list + particle data) is smaller than the 126 MB L2: the K timed steps are consecutive steps "
+                       "of one trajectory, each consuming the previous step's output; no flush between steps"
+                       if w.N < 400_000 else "inputs larger than L2"),
+                "row_pitch": stats["row_pitch"], "cells_per_axis": stats["cells_per_axis"], "mean_nbrs": pairs / w.N,
+                "tunables": {k: g_tun for k, g_tun in tun.items()}}),
+            "particle_steps_per_s": value * w.N,
+            "context_paper": {"gtx_titan_gk110_steps_per_s": PAPER_TITAN_STEPS_PER_S, "ratio": value / world / PAPER_TITAN_STEPS_PER_S,
+                              "note": "PAPER.md:143, other hardware and an equilibrated start: context, not vs_baseline"},
+            "run": {**delta, "E_per_particle": (th["K"] + th["U"]) / w.N, "T": 2 * th["K"] / (3 * w.N),
+                    "max_nbrs": stats["max_nbrs"]},
+            "roofline": roof_alu if w.N < 400_000 else roof_hbm,
+            "roofline_other": roof_hbm if w.N < 400_000 else roof_alu,
+            "kernels": kernels,
+            "cpu_baseline": cpu,
+            "e2e": e2e,
+            "gpu_launches": delta["kernel_launches"],
+            "clocks": clocks,
+            "also": also,
+        }
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

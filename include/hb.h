@@ -164,10 +164,11 @@ HB_API int hb_get_forces(hb_system *h, float *f_xyz_u, float *virial6, int on_de
 HB_API int hb_stats(hb_system *h, hb_stats_t *out);
 
 /* Tunables never change results beyond summation order.
- *   "tpp"            threads per particle in the force kernel: 1,2,4,8,16,32
- *   "force_block"    threads per block of the force kernel
+ *   "tpp"            threads per particle in the force kernel: 1,2,4,8
+ *   "force_block"    threads per block of the force kernel (32..256)
+ *   "force_passes"   consecutive particle tiles walked by one block (0 = auto)
  *   "nlist_ppi"      particles tested per candidate load in the list kernel: 1,2,4
- *   "nlist_cap"      candidates staged in shared memory per warp: 256..2048
+ *   "nlist_cap"      candidates staged in shared memory per warp: 64..1024
  *   "row_pitch"      initial ints per list row (rounded up to 32; 0 = estimate)
  *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
  *   "graph_mode"     0 = no graphs (host reads the flag each step)
@@ -177,6 +178,15 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  */
 HB_API int hb_set_tunable(hb_system *h, const char *name, int value);
 HB_API int hb_get_tunable(hb_system *h, const char *name, int *value);
+
+/* Measurement aid for bench.py: enqueue `reps` launches of one stage on the
+ * system's stream between CUDA events and return the mean duration per launch
+ * in milliseconds.  stage: "lj_force", "nlist" (Algorithm 3 kernel alone),
+ * "cells" (Algorithm 2 chain), "rebuild" (cells + nlist), "nve" (fused kick +
+ * drift kernel with dt = 0, so the state is unchanged).  If flush_l2_bytes > 0 a
+ * scratch buffer of that size is overwritten before every launch (outside the
+ * timed interval) so that each launch starts with a cold L2.  Needs a list. */
+HB_API int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_bytes, double *mean_ms);
 
 HB_API const char *hb_last_error(hb_system *h);
 HB_API const char *hb_version(void);

@@ -517,6 +517,7 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    h->sm_count = sms;
     h->thermo_blocks = (int)std::min<int64_t>(cdiv(N, 256), (int64_t)sms * 4);
     HB_TRY(dev_alloc_t(h, &h->thermo_part, (size_t)(h->thermo_blocks + 2) * 11));
     HB_TRY(upload_params(h));
@@ -834,11 +835,64 @@ int hb_stats(hb_system *h, hb_stats_t *out)
     return HB_OK;
 }
 
+int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_bytes, double *mean_ms)
+{
+    HB_NEED(h);
+    if (!stage || reps <= 0 || reps > 100000 || !mean_ms || flush_l2_bytes < 0) return HB_EINVAL;
+    if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
+    int which = -1;
+    const char *names[] = {"lj_force", "nlist", "cells", "rebuild", "nve"};
+    for (int k = 0; k < 5; k++) if (!strcmp(stage, names[k])) which = k;
+    if (which < 0) { h->err = std::string("unknown stage ") + stage; return HB_EINVAL; }
+    HB_TRY(read_flags(h));
+    const int pending = h->h_flags[FL_NEED_BUILD];  // the timed kernels clear or set it; put it back afterwards
+    void *scratch = nullptr;
+    if (flush_l2_bytes > 0) HB_TRY(dev_alloc(h, &scratch, (size_t)flush_l2_bytes));
+    const int nev = flush_l2_bytes > 0 ? reps : 1;
+    std::vector<cudaEvent_t> ev0(nev), ev1(nev);
+    for (int k = 0; k < nev; k++) { cudaEventCreate(&ev0[k]); cudaEventCreate(&ev1[k]); }
+    int rc = HB_OK;
+    auto launch = [&]() -> int {
+        switch (which) {
+            case 0: HB_CK(launch_force(h)); break;
+            case 1: HB_CK(launch_nlist(h, nullptr)); break;
+            case 2: HB_TRY(enqueue_cells(h, nullptr)); break;
+            case 3: HB_TRY(enqueue_rebuild(h, nullptr)); break;
+            default: HB_CK(launch_nve(h, 0.0f, true, true, 0, false)); break;
+        }
+        return HB_OK;
+    };
+    if (!flush_l2_bytes) cudaEventRecord(ev0[0], h->stream);
+    for (int r = 0; r < reps && rc == HB_OK; r++) {
+        if (flush_l2_bytes) {
+            cudaMemsetAsync(scratch, r & 0xff, (size_t)flush_l2_bytes, h->stream);
+            cudaEventRecord(ev0[r], h->stream);
+        }
+        rc = launch();
+        if (flush_l2_bytes) cudaEventRecord(ev1[r], h->stream);
+    }
+    if (!flush_l2_bytes) cudaEventRecord(ev1[0], h->stream);
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    double total = 0.0;
+    if (rc == HB_OK && e == cudaSuccess) {
+        for (int k = 0; k < nev; k++) { float ms = 0.f; cudaEventElapsedTime(&ms, ev0[k], ev1[k]); total += ms; }
+        *mean_ms = total / reps;
+    } else if (rc == HB_OK) {
+        h->err = std::string("hb_time_stage: ") + cudaGetErrorString(e);
+        rc = HB_ECUDA;
+    }
+    for (int k = 0; k < nev; k++) { cudaEventDestroy(ev0[k]); cudaEventDestroy(ev1[k]); }
+    dev_free(h, scratch);
+    if (rc == HB_OK) rc = set_flag(h, FL_NEED_BUILD, pending);
+    return rc;
+}
+
 static int *tunable_slot(hb_system *h, const char *name)
 {
     if (!name) return nullptr;
     if (!strcmp(name, "tpp")) return &h->tun.tpp;
     if (!strcmp(name, "force_block")) return &h->tun.force_block;
+    if (!strcmp(name, "force_passes")) return &h->tun.force_passes;
     if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
     if (!strcmp(name, "nlist_cap")) return &h->tun.nlist_cap;
     if (!strcmp(name, "row_pitch")) return &h->tun.row_pitch;
@@ -854,10 +908,11 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     int *slot = tunable_slot(h, name);
     if (!slot) { h->err = std::string("unknown tunable ") + (name ? name : "(null)"); return HB_EINVAL; }
     bool ok = true;
-    if (slot == &h->tun.tpp) ok = value == 1 || value == 2 || value == 4 || value == 8 || value == 16 || value == 32;
+    if (slot == &h->tun.tpp) ok = value == 1 || value == 2 || value == 4 || value == 8;
+    else if (slot == &h->tun.force_passes) ok = value >= 0 && value <= 64;
     else if (slot == &h->tun.force_block) ok = value >= 32 && value <= 256 && value % 32 == 0;
     else if (slot == &h->tun.nlist_ppi) ok = value == 1 || value == 2 || value == 4;
-    else if (slot == &h->tun.nlist_cap) ok = value >= 64 && value <= 2048 && value % 32 == 0;
+    else if (slot == &h->tun.nlist_cap) ok = value >= 64 && value <= 1024 && value % 32 == 0;
     else if (slot == &h->tun.row_pitch) ok = value >= 0 && value <= 4096;
     else if (slot == &h->tun.cell_sort) ok = value == 0 || value == 1;
     else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 2;

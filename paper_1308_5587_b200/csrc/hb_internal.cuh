@@ -5,6 +5,7 @@
 #include <string>
 #include <vector>
 #include <map>
+#include <algorithm>
 
 #include "../../include/hb.h"
 
@@ -29,7 +30,8 @@ struct PairParam {  // one per type pair, 16 B
 struct Tunables {
     int tpp = 8;
     int force_block = 128;
-    int nlist_ppi = 2;
+    int force_passes = 0;  // 0 = auto
+    int nlist_ppi = 4;
     int nlist_cap = 512;
     int row_pitch = 0;
     int cell_sort = 1;
@@ -95,6 +97,7 @@ struct hb_system {
     double *thermo_part = nullptr;  // [blocks][12]
     double *h_thermo = nullptr;     // pinned [12]
     int thermo_blocks = 0;
+    int sm_count = 148;
 
     // host-side state machine
     bool have_state = false, cells_valid = false, nlist_valid = false, forces_valid = false, bk_valid = false;

@@ -25,7 +25,7 @@ _ERR_NAMES = {-1: "HB_EINVAL", -2: "HB_ECUDA", -3: "HB_ENOMEM", -4: "HB_EBOX", -
 EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_build_cells",
            "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_sort",
            "hb_thermo", "hb_get_cells", "hb_get_nlist", "hb_get_forces", "hb_stats", "hb_set_tunable",
-           "hb_get_tunable", "hb_last_error", "hb_version"]
+           "hb_get_tunable", "hb_time_stage", "hb_last_error", "hb_version"]
 
 
 class HBError(RuntimeError):
@@ -82,6 +82,7 @@ def load():
     L.hb_stats.argtypes = [vp, C.POINTER(hb_stats_t)]
     L.hb_set_tunable.argtypes = [vp, C.c_char_p, i32]
     L.hb_get_tunable.argtypes = [vp, C.c_char_p, C.POINTER(i32)]
+    L.hb_time_stage.argtypes = [vp, C.c_char_p, i32, i64, C.POINTER(dbl)]
     L.hb_last_error.argtypes = [vp]
     L.hb_last_error.restype = C.c_char_p
     L.hb_version.restype = C.c_char_p
@@ -272,6 +273,12 @@ class System:
         self._ck(self._lib.hb_get_nlist(self._h, rs.ctypes.data_as(C.c_void_p), nbr.ctypes.data_as(C.c_void_p), 0))
         return rs, nbr[: rs[-1]]
 
+    def get_nlist_sizes(self):
+        """row_start int64[N+1] BY TAG without the entries."""
+        rs = np.empty(self.N + 1, np.int64)
+        self._ck(self._lib.hb_get_nlist(self._h, rs.ctypes.data_as(C.c_void_p), None, 0))
+        return rs
+
     def get_forces(self, virial=True):
         """(F_xyz_U float32[N][4], W float32[N][6] or None) BY TAG."""
         f = np.empty((self.N, 4), np.float32)
@@ -284,6 +291,12 @@ class System:
         s = hb_stats_t()
         self._ck(self._lib.hb_stats(self._h, C.byref(s)))
         return {n: getattr(s, n) for n, _ in hb_stats_t._fields_}
+
+    def time_stage(self, stage, reps=20, flush_l2_bytes=0):
+        """Mean milliseconds per launch of one stage (CUDA events on the system's stream)."""
+        ms = C.c_double()
+        self._ck(self._lib.hb_time_stage(self._h, stage.encode(), int(reps), int(flush_l2_bytes), C.byref(ms)))
+        return ms.value
 
     def set_tunable(self, name, value):
         self._ck(self._lib.hb_set_tunable(self._h, name.encode(), int(value)))

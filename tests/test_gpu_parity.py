@@ -87,9 +87,9 @@ def test_forces_energy_virial(hb, orc, case, shift):
         assert th["W"][a] == pytest.approx(ref[k], rel=1e-4, abs=1e-4 * abs(ref["Wxx"]))
 
 
-@pytest.mark.parametrize("tun", [dict(tpp=1), dict(tpp=2), dict(tpp=4), dict(tpp=16), dict(tpp=32),
-                                 dict(nlist_ppi=1), dict(nlist_ppi=4), dict(nlist_cap=64), dict(nlist_cap=96, nlist_ppi=4),
-                                 dict(cell_sort=0), dict(force_block=64), dict(force_block=256, tpp=4)])
+@pytest.mark.parametrize("tun", [dict(tpp=1), dict(tpp=2), dict(tpp=4), dict(tpp=8, force_passes=3),
+                                 dict(nlist_ppi=1), dict(nlist_ppi=2), dict(nlist_cap=64), dict(nlist_cap=96, nlist_ppi=2),
+                                 dict(cell_sort=0), dict(force_block=64, force_passes=1), dict(force_block=256, tpp=4)])
 def test_tunables_do_not_change_results(hb, orc, tun):
     """block size and friends 'do not change the correctness'."""
     w = CASES["ka_10k"]

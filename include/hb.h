@@ -27,9 +27,9 @@
  *     return data to the host synchronise that stream; the others may not.
  *   - Pointers passed in are caller-owned and never retained.  `on_device`
  *     says whether they are device (1) or host (0) pointers.
- *   - Particles keep a tag (their index at hb_set_state).  hb_sort changes
- *     the storage order; every accessor reports BY TAG, so results do not
- *     depend on the current order.
+ *   - Particles keep a tag (their index at hb_set_state).  hb_sort and every
+ *     list build change the storage order; every accessor reports BY TAG, so
+ *     results do not depend on the current order.
  *   - Virial component order: xx, xy, xz, yy, yz, zz.
  */
 #ifndef HB_H
@@ -81,7 +81,7 @@ typedef struct hb_stats_t {
     int64_t sorts;            /* hb_sort calls (incl. those made by hb_run_nve) */
     int64_t overflow_retries; /* times the list rows were grown and work redone */
     int64_t max_nbrs;         /* longest row of the current list */
-    int64_t row_pitch;        /* ints per list row (multiple of 32 = 128 B) */
+    int64_t row_pitch;        /* 16-bit entries per list row (multiple of 64 = 128 B) */
     int64_t cells_per_axis;   /* m */
     int64_t graph_launches;   /* CUDA graph launches made by hb_run_nve */
     int64_t kernel_launches;  /* kernels enqueued (graph nodes counted when they run) */
@@ -113,7 +113,10 @@ HB_API int hb_set_rcut_pair(hb_system *h, const double *rcut);
 /* Algorithm 2: bin the particles into m^3 cells, m = floor(L / r_max), with
  * c = floor((x - b) m / L) per axis evaluated in binary32 without contraction
  * (reading c1).  Uses the r_max of the last hb_build_nlist (or r_cut,max +
- * 0 if none).  Result: CSR cell list in cell-id order c = cx + m (cy + m cz). */
+ * 0 if none).  Result: CSR cell list in cell-id order c = cx + m (cy + m cz).
+ * The particle data is re-ordered into cell order (tags are kept; an existing
+ * list and the forces become stale).  A no-op when the cell list of the
+ * current positions is already in place. */
 HB_API int hb_build_cells(hb_system *h);
 
 /* Algorithm 3: N(i) = { j != i : |minimage(R_i - R_j)| < r_cut + r_buff }, full
@@ -144,9 +147,10 @@ HB_API int hb_step_nve(hb_system *h, double dt);
  * saved at the start of the affected chunk and redoing it with longer rows. */
 HB_API int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period);
 
-/* Reorder the particles along a Hilbert curve on a 2^8 grid per axis, stable in
- * the current index (reading c8); permutes every per-particle array, keeps the
- * tags, invalidates the list. */
+/* Reorder the particles along a Hilbert curve on a 2^8 grid per axis, equal keys
+ * in tag order (reading c8); permutes every per-particle array, keeps the
+ * tags, invalidates the list.  (Every list build re-orders the particles into
+ * cell order anyway; inside a cell the order set here survives.) */
 HB_API int hb_sort(hb_system *h);
 
 HB_API int hb_thermo(hb_system *h, hb_thermo_t *out);
@@ -164,13 +168,16 @@ HB_API int hb_get_forces(hb_system *h, float *f_xyz_u, float *virial6, int on_de
 HB_API int hb_stats(hb_system *h, hb_stats_t *out);
 
 /* Tunables never change results beyond summation order.
- *   "tpp"            threads per particle in the force kernel: 1,2,4,8
- *   "force_block"    threads per block of the force kernel (32..256)
- *   "force_passes"   consecutive particle tiles walked by one block (0 = auto)
+ *   "tpp"            threads per particle in the force kernel: 2,4,8
+ *   "epl"            list entries per thread per iteration in the force kernel: 4,8 (8 only with tpp <= 4)
  *   "nlist_ppi"      particles tested per candidate load in the list kernel: 1,2,4
- *   "nlist_cap"      candidates staged in shared memory per warp: 64..1024
- *   "row_pitch"      initial ints per list row (rounded up to 32; 0 = estimate)
+ *   "tile_x/y/z"     cells per tile (one thread block stages one tile and its one-cell halo in
+ *                    shared memory); 0 = chosen from m and the SM count.  Needs
+ *                    (tx+2)(ty+2)(tz+2) <= 256 and ty*tz <= 32 after clipping to m.
+ *   "stage_cap"      shared-memory slots per tile (0 = from the density); grown on overflow
+ *   "row_pitch"      initial entries per list row (rounded up to 64; 0 = estimate)
  *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
+ *   "fuse_nve"       1 = hb_run_nve integrates inside the force kernel (one kernel per step)
  *   "graph_mode"     0 = no graphs (host reads the flag each step)
  *                    1 = graphs of kernels that exit early unless rebuilding
  *                    2 = graphs with a conditional IF node around the rebuild
@@ -181,9 +188,12 @@ HB_API int hb_get_tunable(hb_system *h, const char *name, int *value);
 
 /* Measurement aid for bench.py: enqueue `reps` launches of one stage on the
  * system's stream between CUDA events and return the mean duration per launch
- * in milliseconds.  stage: "lj_force", "nlist" (Algorithm 3 kernel alone),
- * "cells" (Algorithm 2 chain), "rebuild" (cells + nlist), "nve" (fused kick +
- * drift kernel with dt = 0, so the state is unchanged).  If flush_l2_bytes > 0 a
+ * in milliseconds.  stage: "lj_force" (force kernel alone), "lj_nve" (force
+ * kernel with both half kicks and the drift fused in, dt = 0: the kernel a
+ * step of hb_run_nve is), "nlist" (Algorithm 3 kernel alone), "cells"
+ * (Algorithm 2 chain + reorder), "rebuild" (cells + nlist), "nve" (stand-alone
+ * kick + drift kernel with dt = 0).  The state is unchanged (cells/rebuild are
+ * followed by an untimed rebuild).  If flush_l2_bytes > 0 a
  * scratch buffer of that size is overwritten before every launch (outside the
  * timed interval) so that each launch starts with a cold L2.  Needs a list. */
 HB_API int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_bytes, double *mean_ms);

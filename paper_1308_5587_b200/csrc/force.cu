@@ -1,27 +1,32 @@
 // Lennard-Jones pair force, energy and virial over the neighbor list
-// (PAPER.md:95, 103, 105, 284, 314-320).
+// (PAPER.md:95, 103, 105, 284, 314-320), optionally with the velocity-Verlet
+// half-steps and the r_buff/2 check fused in.
 //
 //   V_lj = 4 eps [(sigma/r)^12 - (sigma/r)^6],  f = -(1/r) dV/dr * d,  r < r_cut,ab
 // with per-type-pair tables held as lj1 = 4 eps sigma^12, lj2 = 4 eps sigma^6:
 //   -(1/r) dV/dr = r^-2 r^-6 (12 lj1 r^-6 - 6 lj2),   V = r^-6 (lj1 r^-6 - lj2) - eshift.
 // The pair functor idea of PAPER.md:284 (V(r) and -(1/r) dV/dr) is kept as the
-// inlined lj_pair() below.
+// inlined pair_term() below.
 //
-// Design (round-1 ncu: the first version was issue-bound at 83 warp instructions
-// per row segment, with no loads in flight across its divergent cutoff branch):
-//   * TPP threads share one particle.  Each reads FOUR consecutive list entries
-//     as one 16-byte load (rows are 128-byte aligned), then issues the four
-//     16-byte position gathers back to back, then evaluates the four pairs
-//     without a branch: a pair outside r_cut (or past the end of the row) gets
-//     r^-2 := 0, which zeroes its force, energy and virial terms.
-//   * Minimum-image arithmetic only where it can matter: a warp whose particles
-//     all lie farther than r_max + r_buff from every face of the box cannot have
-//     a listed neighbor across the boundary and runs the loop without it.
-//   * A block walks `passes` consecutive tiles of particles, so the positions it
-//     gathers stay in its SM's L1 (particles are Hilbert-ordered).
-//   * F, U, W are combined across the TPP lanes with warp shuffles; lane 0 of the
-//     group stores the force, lanes 1 and 2 the two virial vectors.
-#include "hb_internal.cuh"
+// Design.  Round-1 ncu of the first version (one 16-byte global gather per pair):
+// 46 % of the stall samples on the gathers, every warp gather touching ~32 cache
+// lines, the L1 wavefront queue the limiter.  Now ONE BLOCK OWNS ONE TILE of cells
+// (tile.cuh):
+//   * the tile and its halo are staged once in shared memory with coalesced
+//     loads, shifted to the periodic image the tile sees: no minimum-image
+//     arithmetic per pair, and every neighbor gather is a 16-byte shared-memory
+//     load (list entries are 16-bit slots of this staging layout);
+//   * TPP threads share one particle; each reads EPL consecutive 16-bit entries
+//     with one 8- or 16-byte load (prefetched one iteration ahead), issues the EPL
+//     gathers back to back and evaluates the pairs without a branch: a pair
+//     outside r_cut gets r^-2 := 0, rows are padded with the far-away dummy slot;
+//   * F, U, W are combined across the TPP lanes with warp shuffles;
+//   * when asked, the same thread finishes the velocity-Verlet step of its
+//     particle with the force it just computed (second half kick of this step,
+//     first half kick and drift of the next, wrap, image flags, r_buff/2 check),
+//     writing the new position into the OTHER position buffer, since the blocks
+//     around still read the old one.  One kernel per time step.
+#include "tile.cuh"
 
 __device__ __forceinline__ float rcp_approx(float x)
 {
@@ -34,18 +39,11 @@ struct Acc {
     float fx, fy, fz, u, wxx, wxy, wxz, wyy, wyz, wzz;
 };
 
-template <bool MI>
-__device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, bool valid, const PairParam &pp, float L,
-                                          float invL, Acc &a)
+__device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, const PairParam &pp, Acc &a)
 {
-    float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-    if (MI) {  // nearest image (Alg. 3 l.16); |d| < L because both particles are inside the box
-        dx = __fmaf_rn(-L, rintf(dx * invL), dx);
-        dy = __fmaf_rn(-L, rintf(dy * invL), dy);
-        dz = __fmaf_rn(-L, rintf(dz * invL), dz);
-    }
+    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;   // pj is already the nearest image
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-    const bool in = valid && (r2 < pp.rcut2);          // strict <
+    const bool in = r2 < pp.rcut2;                     // strict <
     const float r2inv = in ? rcp_approx(r2) : 0.0f;    // 0 switches the whole pair off
     const float r6inv = r2inv * r2inv * r2inv;
     const float fdivr = r2inv * r6inv * __fmaf_rn(12.0f * pp.lj1, r6inv, -6.0f * pp.lj2);
@@ -57,67 +55,89 @@ __device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, bo
     a.wyy = __fmaf_rn(dy, py, a.wyy); a.wyz = __fmaf_rn(dy, pz, a.wyz); a.wzz = __fmaf_rn(dz, pz, a.wzz);
 }
 
-// One row: entries sub*4 .. sub*4+3, then + 4*TPP, ...
-template <int TPP, bool ONE_TYPE, bool MI>
-__device__ __forceinline__ void accumulate_row(const float4 *__restrict__ pos, const int *__restrict__ row, int n, int self,
-                                               int sub, const float4 &pi, const PairParam *__restrict__ prow,
-                                               const PairParam &pp1, float L, float invL, Acc &a)
+template <int EPL> struct Entries;
+template <> struct Entries<4> { uint2 v; };
+template <> struct Entries<8> { uint4 v; };
+
+template <int EPL>
+__device__ __forceinline__ Entries<EPL> load_entries(const uint16_t *p)
 {
-    for (int k = sub * 4; k < n; k += 4 * TPP) {
-        const int4 jj = __ldg(reinterpret_cast<const int4 *>(row + k));
-        const int rem = n - k;
-        const int j0 = jj.x;                       // k < n always
-        const int j1 = rem > 1 ? jj.y : self;      // past the end: any in-bounds index, switched off below
-        const int j2 = rem > 2 ? jj.z : self;
-        const int j3 = rem > 3 ? jj.w : self;
-        const float4 p0 = __ldg(&pos[j0]);
-        const float4 p1 = __ldg(&pos[j1]);
-        const float4 p2 = __ldg(&pos[j2]);
-        const float4 p3 = __ldg(&pos[j3]);
-        if (ONE_TYPE) {
-            pair_term<MI>(pi, p0, true, pp1, L, invL, a);
-            pair_term<MI>(pi, p1, rem > 1, pp1, L, invL, a);
-            pair_term<MI>(pi, p2, rem > 2, pp1, L, invL, a);
-            pair_term<MI>(pi, p3, rem > 3, pp1, L, invL, a);
-        } else {
-            pair_term<MI>(pi, p0, true, prow[__float_as_int(p0.w)], L, invL, a);
-            pair_term<MI>(pi, p1, rem > 1, prow[__float_as_int(p1.w)], L, invL, a);
-            pair_term<MI>(pi, p2, rem > 2, prow[__float_as_int(p2.w)], L, invL, a);
-            pair_term<MI>(pi, p3, rem > 3, prow[__float_as_int(p3.w)], L, invL, a);
-        }
-    }
+    Entries<EPL> e;
+    if constexpr (EPL == 4) e.v = __ldg(reinterpret_cast<const uint2 *>(p));
+    else e.v = __ldg(reinterpret_cast<const uint4 *>(p));
+    return e;
 }
 
-template <int TPP, bool ONE_TYPE>
-__global__ void __launch_bounds__(256)
-lj_force_kernel(const float4 *__restrict__ pos, const int *__restrict__ nlist, const int *__restrict__ nlistn, int pitch,
-                int N, float L, float inner, int passes, int ntypes, const PairParam *__restrict__ params,
-                float4 *__restrict__ force, float4 *__restrict__ virial, int *__restrict__ flags)
+template <int EPL>
+__device__ __forceinline__ void unpack_entries(const Entries<EPL> &e, int (&sl)[EPL])
 {
-    extern __shared__ PairParam s_params[];
-    if (!ONE_TYPE) {
-        for (int k = threadIdx.x; k < ntypes * ntypes; k += blockDim.x) s_params[k] = params[k];
-        __syncthreads();
-    }
-    if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_NEED_BUILD] = 0;  // this step's rebuild decision has been consumed
-    const float invL = 1.0f / L;
-    const int ppb = blockDim.x / TPP;            // particles per block per pass
-    const int sub = threadIdx.x % TPP;
-    PairParam pp1 = params[0];
+    sl[0] = e.v.x & 0xffffu; sl[1] = e.v.x >> 16; sl[2] = e.v.y & 0xffffu; sl[3] = e.v.y >> 16;
+    if constexpr (EPL == 8) { sl[4] = e.v.z & 0xffffu; sl[5] = e.v.z >> 16; sl[6] = e.v.w & 0xffffu; sl[7] = e.v.w >> 16; }
+}
 
-    for (int pass = 0; pass < passes; pass++) {
-        const int ig = (blockIdx.x * passes + pass) * ppb + threadIdx.x / TPP;
-        const bool active = ig < N;              // inactive threads stay for the shuffles
-        const int i = active ? ig : N - 1;
-        const float4 pi = pos[i];
-        const int n = active ? nlistn[i] : 0;
-        const int *row = nlist + (int64_t)i * pitch;
+template <int TPP, int EPL, bool ONE_TYPE>
+__global__ void __launch_bounds__(TILE_THREADS)
+lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__restrict__ pos,
+               const uint16_t *__restrict__ nlist, const int *__restrict__ nlistn, int pitch, int N, int ntypes,
+               const PairParam *__restrict__ params, float4 *__restrict__ force, float4 *__restrict__ virial,
+               int *__restrict__ flags, int do_nve, NveArgs nv)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ TileShared s;
+    float4 *stage = reinterpret_cast<float4 *>(smem_raw);
+    PairParam *s_params = reinterpret_cast<PairParam *>(smem_raw + (size_t)g.cap * 16);
+    constexpr int G = TPP * EPL;                 // entries per particle per iteration
+    constexpr int PPB = TILE_THREADS / TPP;      // particles per block per pass
+
+    if (!ONE_TYPE)
+        for (int k = threadIdx.x; k < ntypes * ntypes; k += TILE_THREADS) s_params[k] = params[k];
+    if (do_nve && nv.kick_drift && blockIdx.x == 0 && threadIdx.x == 0) flags[nv.need_clear] = 0;
+
+    TileCtx t;
+    tile_decode(g, blockIdx.x, t);
+    const bool fits = tile_tables(g, cell_start, t, s, flags);
+    if (fits) tile_stage_positions(g, t, s, pos, stage);
+    __syncthreads();
+
+    const int sub = threadIdx.x % TPP;
+    const PairParam pp1 = params[0];
+    const float hdt = 0.5f * nv.dt, hL = 0.5f * g.L, L = g.L;
+    bool exceed = false;
+
+    const int nown = fits ? t.nown : 0;
+    for (int q0 = 0; q0 < nown; q0 += PPB) {     // block-uniform trip count: the shuffles need whole warps
+        const int q = q0 + threadIdx.x / TPP;
+        const bool active = q < nown;
+        int gi = 0, n = 0;
+        float4 pi = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (active) {
+            const int r = tile_row_of(t, s, q);
+            const int off = q - s.own_off[r];
+            gi = s.own_start[r] + off;
+            pi = stage[s.own_slot[r] + off];
+            n = nlistn[gi];
+        }
+        const uint16_t *row = nlist + (int64_t)gi * pitch + sub * EPL;
         const PairParam *prow = ONE_TYPE ? nullptr : s_params + __float_as_int(pi.w) * ntypes;
         Acc a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
-        const bool interior = fmaxf(fmaxf(fabsf(pi.x), fabsf(pi.y)), fabsf(pi.z)) < inner;
-        if (__all_sync(0xffffffffu, interior)) accumulate_row<TPP, ONE_TYPE, false>(pos, row, n, i, sub, pi, prow, pp1, L, invL, a);
-        else accumulate_row<TPP, ONE_TYPE, true>(pos, row, n, i, sub, pi, prow, pp1, L, invL, a);
+        Entries<EPL> cur{};
+        if (n > 0) cur = load_entries<EPL>(row);
+        for (int k = 0; k < n; k += G) {
+            Entries<EPL> nxt{};
+            if (k + G < n) nxt = load_entries<EPL>(row + k + G);   // one iteration ahead
+            int sl[EPL];
+            unpack_entries<EPL>(cur, sl);
+            float4 pj[EPL];
+#pragma unroll
+            for (int e = 0; e < EPL; e++) pj[e] = stage[sl[e]];
+#pragma unroll
+            for (int e = 0; e < EPL; e++) {
+                if (ONE_TYPE) pair_term(pi, pj[e], pp1, a);
+                else pair_term(pi, pj[e], prow[__float_as_int(pj[e].w)], a);
+            }
+            cur = nxt;
+        }
 
 #pragma unroll
         for (int o = TPP >> 1; o > 0; o >>= 1) {
@@ -134,52 +154,100 @@ lj_force_kernel(const float4 *__restrict__ pos, const int *__restrict__ nlist, c
         }
         if (!active) continue;
         // U_i = 1/2 sum V, W_i = 1/2 sum d f (reading c6.i)
-        if (TPP >= 4) {
-            if (sub == 0) force[i] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
-            else if (sub == 1) virial[2 * (int64_t)i] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
-            else if (sub == 2) virial[2 * (int64_t)i + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
-        } else if (sub == 0) {
-            force[i] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
-            virial[2 * (int64_t)i] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
-            virial[2 * (int64_t)i + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
+        if (sub == 0) {
+            force[gi] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
+            if (do_nve) {
+                // reading c7, operation by operation as nve_kernel does it
+                float4 v = nv.vel[gi];
+                if (nv.kick_prev) {
+                    v.x = __fmaf_rn(hdt, a.fx, v.x);
+                    v.y = __fmaf_rn(hdt, a.fy, v.y);
+                    v.z = __fmaf_rn(hdt, a.fz, v.z);
+                }
+                if (nv.kick_drift) {
+                    v.x = __fmaf_rn(hdt, a.fx, v.x);
+                    v.y = __fmaf_rn(hdt, a.fy, v.y);
+                    v.z = __fmaf_rn(hdt, a.fz, v.z);
+                    float4 p = pos[gi];   // the stored position: pi may be another periodic image of it
+                    p.x = __fmaf_rn(nv.dt, v.x, p.x);
+                    p.y = __fmaf_rn(nv.dt, v.y, p.y);
+                    p.z = __fmaf_rn(nv.dt, v.z, p.z);
+                    if (p.x >= hL) { p.x -= L; nv.image[gi] += 1; } else if (p.x < -hL) { p.x += L; nv.image[gi] -= 1; }
+                    if (p.y >= hL) { p.y -= L; nv.image[N + gi] += 1; } else if (p.y < -hL) { p.y += L; nv.image[N + gi] -= 1; }
+                    if (p.z >= hL) { p.z -= L; nv.image[2 * (int64_t)N + gi] += 1; }
+                    else if (p.z < -hL) { p.z += L; nv.image[2 * (int64_t)N + gi] -= 1; }
+                    nv.pos_out[gi] = p;
+                    const float4 pb = nv.pos_build[gi];
+                    float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
+                    if (dx >= hL) dx -= L; else if (dx < -hL) dx += L;
+                    if (dy >= hL) dy -= L; else if (dy < -hL) dy += L;
+                    if (dz >= hL) dz -= L; else if (dz < -hL) dz += L;
+                    exceed = exceed || (dx * dx + dy * dy + dz * dz) > nv.half_buff2;
+                }
+                nv.vel[gi] = v;
+            }
+        } else if (TPP >= 4 && sub == 1) {
+            virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
+        } else if (TPP >= 4 && sub == 2) {
+            virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
+        }
+        if (TPP < 4 && sub == TPP - 1) {
+            virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
+            virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
+        }
+    }
+
+    if (do_nve && nv.kick_drift) {
+        if (exceed) flags[nv.need_set] = 1;
+        if (nv.use_cond) {
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                __threadfence();
+                const int ticket = atomicAdd(&flags[FL_DONE_CTR], 1);
+                if (ticket == (int)gridDim.x - 1) {
+                    __threadfence();
+                    const int need = *((volatile int *)&flags[nv.need_set]);
+                    cudaGraphSetConditional(nv.cond, need ? 1u : 0u);
+                    flags[FL_DONE_CTR] = 0;
+                }
+            }
         }
     }
 }
 
-template <int TPP>
-static cudaError_t launch_force_tpp(hb_system *h)
+size_t force_smem_bytes(const hb_system *h)
 {
-    const int block = h->tun.force_block;
-    const int ppb = block / TPP;
-    // passes: consecutive tiles per block, chosen so that the grid still fills the GPU about twice over
-    int passes = h->tun.force_passes;
-    if (passes <= 0) {
-        const int64_t tiles = cdiv(h->N, ppb);
-        passes = (int)std::max<int64_t>(1, std::min<int64_t>(16, tiles / ((int64_t)h->sm_count * 16)));
-    }
-    const unsigned grid = (unsigned)cdiv(h->N, (int64_t)ppb * passes);
-    // listed pairs are closer than r_max + r_buff now; beyond that distance from every face no pair crosses the boundary
-    const float inner = 0.5f * h->L - (h->r_max + h->r_buff);
-    if (h->ntypes == 1) {
-        lj_force_kernel<TPP, true><<<grid, block, 0, h->stream>>>(h->pos, h->nlist, h->nlistn, h->row_pitch, (int)h->N, h->L,
-                                                                 inner, passes, 1, h->params, h->force, h->virial, h->flags);
-    } else {
-        const size_t smem = sizeof(PairParam) * h->ntypes * h->ntypes;
-        lj_force_kernel<TPP, false><<<grid, block, smem, h->stream>>>(h->pos, h->nlist, h->nlistn, h->row_pitch, (int)h->N,
-                                                                     h->L, inner, passes, h->ntypes, h->params, h->force,
-                                                                     h->virial, h->flags);
-    }
+    return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? sizeof(PairParam) * h->ntypes * h->ntypes : 0);
+}
+
+template <int TPP, int EPL>
+static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
+{
+    const size_t smem = force_smem_bytes(h);
+    const unsigned grid = (unsigned)h->geom.ntiles;
+    NveArgs nv{};
+    if (nve) nv = *nve;
+    cudaError_t e;
+#define LJ_LAUNCH(ONE)                                                                                                      \
+    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+    if (e != cudaSuccess) return e;                                                                                         \
+    lj_tile_kernel<TPP, EPL, ONE><<<grid, TILE_THREADS, smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
+                                                                           h->nlistn, h->row_pitch, (int)h->N, h->ntypes,  \
+                                                                           h->params, h->force, h->virial, h->flags,       \
+                                                                           nve ? 1 : 0, nv);
+    if (h->ntypes == 1) { LJ_LAUNCH(true) } else { LJ_LAUNCH(false) }
+#undef LJ_LAUNCH
     h->stats.kernel_launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_force(hb_system *h)
+cudaError_t launch_force(hb_system *h, const NveArgs *nve)
 {
+    const int epl = h->tun.epl == 8 ? 8 : 4;
     switch (h->tun.tpp) {
-        case 1: return launch_force_tpp<1>(h);
-        case 2: return launch_force_tpp<2>(h);
-        case 4: return launch_force_tpp<4>(h);
-        default: return launch_force_tpp<8>(h);
+        case 2: return epl == 8 ? launch_force_t<2, 8>(h, nve) : launch_force_t<2, 4>(h, nve);
+        case 8: return launch_force_t<8, 4>(h, nve);   // 8 x 8 entries would read past the 32-entry row padding
+        default: return epl == 8 ? launch_force_t<4, 8>(h, nve) : launch_force_t<4, 4>(h, nve);
     }
 }
 

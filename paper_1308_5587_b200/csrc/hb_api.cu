@@ -9,7 +9,7 @@
 
 namespace {
 
-const int kRebuildKernels = 7;  // clear, bin, scan x2, scatter, (sort), list -- see enqueue_rebuild
+const int kRebuildKernels = 5;  // count, scan, scatter, gather, list -- see enqueue_rebuild
 
 int dev_alloc(hb_system *h, void **p, size_t bytes)
 {
@@ -77,7 +77,73 @@ int upload_params(hb_system *h)
     return HB_OK;
 }
 
-// r_max, m, cell arrays, row pitch.  Reading c1.ii: m = floor(L / r_max) in binary64
+int stage_cap_max(const hb_system *h)
+{
+    // what is left of the opt-in shared memory after the static tables and the list kernel's candidate lists
+    const int64_t left = (int64_t)h->smem_max - 20 * 1024;
+    return (int)std::min<int64_t>(65535, left / 16);
+}
+
+// Tile dimensions and staging capacity (tile.cuh).  Tunables override the choice.
+int choose_tiles(hb_system *h, int min_cap)
+{
+    const int m = h->m;
+    int tx = h->tun.tile_x, ty = h->tun.tile_y, tz = h->tun.tile_z;
+    auto ntiles_of = [&](int ax, int ay, int az) {
+        return (int64_t)cdiv(m, std::min(ax, m)) * cdiv(m, std::min(ay, m)) * cdiv(m, std::min(az, m));
+    };
+    if (tx <= 0 || ty <= 0 || tz <= 0) {
+        // largest brick that still leaves every SM several tiles (smaller halo overhead per particle)
+        const int cand[4][3] = {{2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
+        int pick = 3;
+        for (int k = 0; k < 4; k++)
+            if (ntiles_of(cand[k][0], cand[k][1], cand[k][2]) >= (int64_t)6 * h->sm_count) { pick = k; break; }
+        tx = cand[pick][0]; ty = cand[pick][1]; tz = cand[pick][2];
+    }
+    tx = std::min(tx, m); ty = std::min(ty, m); tz = std::min(tz, m);
+    if ((tx + 2) * (ty + 2) * (tz + 2) > TILE_HMAX || ty * tz > TILE_ROWS_MAX) {
+        h->err = "tile too large: (tx+2)(ty+2)(tz+2) must be <= 256 and ty*tz <= 32";
+        return HB_EINVAL;
+    }
+    TileGeom g{};
+    g.m = m; g.tx = tx; g.ty = ty; g.tz = tz;
+    g.ntx = (int)cdiv(m, tx); g.nty = (int)cdiv(m, ty); g.ntz = (int)cdiv(m, tz);
+    const int64_t nt = (int64_t)g.ntx * g.nty * g.ntz;
+    if (nt > 0x7fffffff) { h->err = "too many tiles"; return HB_EINVAL; }
+    g.ntiles = (int)nt;
+    g.L = h->L;
+    int cap = h->tun.stage_cap;
+    if (cap <= 0) {
+        const double per_cell = (double)h->N / (double)h->ncells;
+        const double est = per_cell * (tx + 2) * (ty + 2) * (tz + 2);
+        cap = (int)(1.5 * est) + 64;
+    }
+    cap = std::max(cap, min_cap);
+    cap = round_up(std::max(cap, 64), 32);
+    if (cap > stage_cap_max(h)) {
+        if (min_cap > stage_cap_max(h) && tx * ty * tz > 1) {
+            // shrink to one cell per tile (27 staged cells) and scale the requirement with the halo volume
+            const int nh = (tx + 2) * (ty + 2) * (tz + 2);
+            h->tun.tile_x = h->tun.tile_y = h->tun.tile_z = 1;
+            return choose_tiles(h, (int)((int64_t)min_cap * 27 / nh));
+        }
+        if (min_cap > stage_cap_max(h)) {
+            h->err = "a tile of cells with its halo holds " + std::to_string(min_cap) +
+                     " particles: more than fit in shared memory; use smaller tiles (tile_x/y/z = 1)";
+            return HB_ENOMEM;
+        }
+        cap = stage_cap_max(h);
+    }
+    g.cap = cap;
+    if (memcmp(&g, &h->geom, sizeof g) != 0) {
+        destroy_graphs(h);
+        h->nlist_valid = false;
+    }
+    h->geom = g;
+    return HB_OK;
+}
+
+// r_max, m, cell arrays, tiles.  Reading c1.ii: m = floor(L / r_max) in binary64
 // from the binary32 values of L and r_max.
 int configure_geometry(hb_system *h)
 {
@@ -98,31 +164,32 @@ int configure_geometry(hb_system *h)
     h->ncells = (int64_t)m * m * m;
     if (h->ncells > h->ncells_alloc) {
         dev_free_t(h, h->cell_count);
+        dev_free_t(h, h->cell_local);
         dev_free_t(h, h->cell_start);
+        dev_free_t(h, h->scan_sums);
         HB_TRY(dev_alloc_t(h, &h->cell_count, (size_t)h->ncells));
+        HB_TRY(dev_alloc_t(h, &h->cell_local, (size_t)h->ncells));
         HB_TRY(dev_alloc_t(h, &h->cell_start, (size_t)h->ncells + 1));
+        h->scan_sums_len = cdiv(h->ncells, 2048) + 16;
+        HB_TRY(dev_alloc_t(h, &h->scan_sums, (size_t)h->scan_sums_len));
+        HB_CK(cudaMemsetAsync(h->cell_count, 0, sizeof(int) * (size_t)h->ncells, h->stream));  // kept zero between builds
         h->ncells_alloc = h->ncells;
         destroy_graphs(h);
     }
-    const int64_t need_tmp = cdiv(h->ncells, 2048) + 16;
-    if (need_tmp > h->scan_tmp_len) {
-        dev_free_t(h, h->scan_tmp);
-        HB_TRY(dev_alloc_t(h, &h->scan_tmp, (size_t)need_tmp));
-        h->scan_tmp_len = need_tmp;
-        destroy_graphs(h);
-    }
+    HB_TRY(choose_tiles(h, 0));
     h->stats.cells_per_axis = m;
     return HB_OK;
 }
 
 int ensure_rows(hb_system *h, int pitch)
 {
-    pitch = round_up(pitch < 32 ? 32 : pitch, 32);
+    pitch = round_up(pitch < 64 ? 64 : pitch, 64);   // 16-bit entries: 64 = 128 B
     const int64_t need = h->N * (int64_t)pitch;
     if (need > h->nlist_alloc) {
         dev_free_t(h, h->nlist);
         HB_TRY(dev_alloc_t(h, &h->nlist, (size_t)need));
         h->nlist_alloc = need;
+        destroy_graphs(h);
     }
     if (pitch != h->row_pitch) destroy_graphs(h);
     h->row_pitch = pitch;
@@ -157,14 +224,19 @@ int set_flag(hb_system *h, int which, int value)
     return HB_OK;
 }
 
-// Algorithm 2: clear, bin (atomic slot per particle), scan, scatter, order within cells.
+int clear_need_flags(hb_system *h)
+{
+    HB_CK(cudaMemsetAsync(h->flags + FL_NEED0, 0, 2 * sizeof(int), h->stream));
+    return HB_OK;
+}
+
+// Algorithm 2 and the reorder into cell order: count (atomic slot per particle), scan, scatter, gather.
 int enqueue_cells(hb_system *h, const int *pred)
 {
-    HB_CK(launch_cell_clear(h, pred));
-    HB_CK(launch_cell_bin(h, pred));
-    HB_CK(launch_scan_exclusive(h, h->cell_count, h->cell_start, h->ncells, h->scan_tmp, pred));
+    HB_CK(launch_cell_count(h, pred));
+    HB_CK(launch_cell_scan(h, pred));
     HB_CK(launch_cell_scatter(h, pred));
-    if (h->tun.cell_sort) HB_CK(launch_cell_sort(h, pred));
+    HB_CK(launch_cell_gather(h, pred));
     return HB_OK;
 }
 
@@ -172,30 +244,39 @@ int enqueue_cells(hb_system *h, const int *pred)
 int enqueue_rebuild(hb_system *h, const int *pred)
 {
     HB_TRY(enqueue_cells(h, pred));
-    HB_CK(launch_nlist(h, pred));
+    HB_CK(launch_nlist(h, pred, true));
     return HB_OK;
 }
 
-int rebuild_kernel_count(const hb_system *h) { return kRebuildKernels - (h->tun.cell_sort ? 0 : 1); }
-
-// Build with the host in the loop: detects row overflow, grows the rows, rebuilds.
+// Build with the host in the loop: detects row and staging overflow, grows, rebuilds.
 int build_nlist_sync(hb_system *h)
 {
     if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
     if (h->row_pitch == 0) HB_TRY(ensure_rows(h, initial_pitch(h)));
-    for (int attempt = 0; attempt < 12; attempt++) {
+    for (int attempt = 0; attempt < 16; attempt++) {
         HB_TRY(enqueue_rebuild(h, nullptr));
         HB_TRY(read_flags(h));
+        h->forces_valid = false;   // the storage order changed under the force array
+        h->moved = false;
         if (h->h_flags[FL_BAD]) {
             h->err = "a particle is non-finite or outside the box";
             set_flag(h, FL_BAD, 0);
+            h->cells_valid = h->nlist_valid = false;
             return HB_ENAN;
         }
         h->stats.rebuilds = h->h_flags[FL_BUILDS];
+        if (h->h_flags[FL_STAGE_OVER]) {
+            const int needed = h->h_flags[FL_STAGE_OVER];
+            h->stats.overflow_retries++;
+            HB_TRY(set_flag(h, FL_STAGE_OVER, 0));
+            HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
+            HB_TRY(choose_tiles(h, (int)(needed * 1.2) + 32));
+            continue;
+        }
         h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
         if (h->h_flags[FL_MAX_NBRS] <= h->row_pitch) {
             HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
-            HB_TRY(set_flag(h, FL_NEED_BUILD, 0));
+            HB_TRY(clear_need_flags(h));
             h->cells_valid = h->nlist_valid = true;
             return HB_OK;
         }
@@ -208,9 +289,9 @@ int build_nlist_sync(hb_system *h)
 
 int ensure_forces(hb_system *h)
 {
-    if (!h->nlist_valid) { HB_TRY(build_nlist_sync(h)); h->forces_valid = false; }
+    if (!h->nlist_valid) HB_TRY(build_nlist_sync(h));
     if (!h->forces_valid) {
-        HB_CK(launch_force(h));
+        HB_CK(launch_force(h, nullptr));
         h->forces_valid = true;
     }
     return HB_OK;
@@ -222,14 +303,10 @@ int ensure_sort_buffers(hb_system *h)
     const size_t N = (size_t)h->N;
     HB_TRY(dev_alloc_t(h, &h->keys, N));
     HB_TRY(dev_alloc_t(h, &h->keys2, N));
-    HB_TRY(dev_alloc_t(h, &h->perm, N));
-    HB_TRY(dev_alloc_t(h, &h->perm2, N));
-    HB_TRY(dev_alloc_t(h, &h->pos2, N));
-    HB_TRY(dev_alloc_t(h, &h->vel2, N));
+    HB_TRY(dev_alloc_t(h, &h->sperm, N));
+    HB_TRY(dev_alloc_t(h, &h->sperm2, N));
     HB_TRY(dev_alloc_t(h, &h->force2, N));
     HB_TRY(dev_alloc_t(h, &h->virial2, 2 * N));
-    HB_TRY(dev_alloc_t(h, &h->image2, 3 * N));
-    HB_TRY(dev_alloc_t(h, &h->tag2, N));
     const int64_t ntiles = cdiv(h->N, 512);
     h->radix_counts_len = 256 * ntiles;
     HB_TRY(dev_alloc_t(h, &h->radix_counts, (size_t)(2 * h->radix_counts_len + 8)));
@@ -238,7 +315,6 @@ int ensure_sort_buffers(hb_system *h)
         dev_free_t(h, h->scan_tmp);
         HB_TRY(dev_alloc_t(h, &h->scan_tmp, (size_t)need_tmp));
         h->scan_tmp_len = need_tmp;
-        destroy_graphs(h);
     }
     return HB_OK;
 }
@@ -250,25 +326,49 @@ int sort_internal(hb_system *h)
     HB_CK(launch_sfc_keys(h));
     HB_CK(launch_radix_sort(h, 24));
     HB_CK(launch_gather_state(h));
-    // copy back rather than swap pointers: captured graphs keep pointing at the first set
+    // copy back rather than swap pointers: captured graphs keep pointing at the live set
     const size_t N = (size_t)h->N;
-    HB_CK(cudaMemcpyAsync(h->pos, h->pos2, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->pos(), h->pos_build, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->vel, h->vel2, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->force, h->force2, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->virial, h->virial2, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->image, h->image2, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->tag, h->tag2, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
     h->cells_valid = h->nlist_valid = false;
+    h->moved = true;
     h->bk_valid = false;
     h->stats.sorts++;
     h->since_sort = 0;
     return HB_OK;
 }
 
+NveArgs make_nve(hb_system *h, float dt, bool kick_prev, bool kick_drift, float4 *pos_out, cudaGraphConditionalHandle cond,
+                 bool use_cond)
+{
+    NveArgs a{};
+    a.vel = h->vel;
+    a.image = h->image;
+    a.pos_build = h->pos_build;
+    a.pos_out = pos_out;
+    a.dt = dt;
+    const float hb = 0.5f * h->r_buff;
+    a.half_buff2 = hb * hb;
+    a.kick_prev = kick_prev ? 1 : 0;
+    a.kick_drift = kick_drift ? 1 : 0;
+    a.need_set = FL_NEED0 + (h->parity & 1);
+    a.need_clear = FL_NEED0 + ((h->parity + 1) & 1);
+    a.cond = cond;
+    a.use_cond = use_cond ? 1 : 0;
+    return a;
+}
+
 // ---- hb_run_nve: n steps as one CUDA graph ----
+// fuse_nve = 1:  nve(drift) [rebuild?]  { lj+nve(kick, kick, drift) [rebuild?] } x (n-1)  lj+nve(kick)
+// fuse_nve = 0:  nve(drift) [rebuild?]  { lj  nve(kick, kick, drift) [rebuild?] } x (n-1)  lj  nve(kick)
 int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
 {
     const int mode = h->tun.graph_mode;
+    const bool fuse = h->tun.fuse_nve != 0;
     cudaStream_t cs = nullptr, cs2 = nullptr;
     HB_CK(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
     HB_CK(cudaStreamCreateWithFlags(&cs2, cudaStreamNonBlocking));
@@ -276,6 +376,7 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     HB_CK(cudaGraphCreate(&g, 0));
     cudaStream_t saved = h->stream;
     const int64_t saved_launches = h->stats.kernel_launches;
+    const int saved_cur = h->cur, saved_parity = h->parity;
     int rc = HB_OK;
     auto fail = [&](const char *what, cudaError_t e) {
         h->err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -291,8 +392,21 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
                 e = cudaGraphConditionalHandleCreate(&cond, g, 0, cudaGraphCondAssignDefault);
                 if (e != cudaSuccess) { fail("cudaGraphConditionalHandleCreate", e); break; }
             }
-            e = launch_nve(h, dt, s > 0, true, cond, mode == 2);
-            if (e != cudaSuccess) { fail("nve kernel (capture)", e); break; }
+            // the drift of step s (after the force of the state it starts from, except for s = 0: forces are valid)
+            const int need_flag = FL_NEED0 + (h->parity & 1);
+            if (s == 0) {
+                e = launch_nve(h, make_nve(h, dt, false, true, h->pos(), cond, mode == 2));
+            } else if (fuse) {
+                float4 *other = h->posbuf[h->cur ^ 1];
+                const NveArgs a = make_nve(h, dt, true, true, other, cond, mode == 2);
+                e = launch_force(h, &a);
+                h->cur ^= 1;
+            } else {
+                e = launch_force(h, nullptr);
+                if (e == cudaSuccess) e = launch_nve(h, make_nve(h, dt, true, true, h->pos(), cond, mode == 2));
+            }
+            if (e != cudaSuccess) { fail("step kernel (capture)", e); break; }
+            h->parity++;
             if (mode == 2) {
                 cudaStreamCaptureStatus st;
                 const cudaGraphNode_t *deps = nullptr;
@@ -321,15 +435,20 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
                 e = cudaStreamUpdateCaptureDependencies(cs, &node, 1, cudaStreamSetCaptureDependencies);
                 if (e != cudaSuccess) { fail("cudaStreamUpdateCaptureDependencies", e); break; }
             } else {
-                rc = enqueue_rebuild(h, h->flags + FL_NEED_BUILD);
+                rc = enqueue_rebuild(h, h->flags + need_flag);
                 if (rc != HB_OK) break;
             }
-            e = launch_force(h);
-            if (e != cudaSuccess) { fail("force kernel (capture)", e); break; }
         }
         if (rc == HB_OK) {
-            e = launch_nve(h, dt, true, false, 0, false);
-            if (e != cudaSuccess) fail("nve kernel (capture)", e);
+            // forces of the last state and the second half kick of the last step
+            if (fuse) {
+                const NveArgs a = make_nve(h, dt, true, false, h->pos(), 0, false);
+                e = launch_force(h, &a);
+            } else {
+                e = launch_force(h, nullptr);
+                if (e == cudaSuccess) e = launch_nve(h, make_nve(h, dt, true, false, h->pos(), 0, false));
+            }
+            if (e != cudaSuccess) fail("final kernel (capture)", e);
         }
         cudaGraph_t tmp = nullptr;
         e = cudaStreamEndCapture(cs, &tmp);
@@ -337,6 +456,8 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     }
     h->stream = saved;
     h->stats.kernel_launches = saved_launches;
+    h->cur = saved_cur;
+    h->parity = saved_parity;
     cudaGraphExec_t ex = nullptr;
     if (rc == HB_OK) {
         e = cudaGraphInstantiate(&ex, g, 0);
@@ -351,7 +472,7 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     }
     out->g = g;
     out->e = ex;
-    out->nkernels_fixed = 2 * n + 1 + (mode == 1 ? n * rebuild_kernel_count(h) : 0);
+    out->nkernels_fixed = (fuse ? n + 1 : 2 * n + 1) + (mode == 1 ? n * kRebuildKernels : 0);
     return HB_OK;
 }
 
@@ -364,12 +485,16 @@ int backup_state(hb_system *h)
         HB_TRY(dev_alloc_t(h, &h->bk_force, N));
         HB_TRY(dev_alloc_t(h, &h->bk_virial, 2 * N));
         HB_TRY(dev_alloc_t(h, &h->bk_image, 3 * N));
+        HB_TRY(dev_alloc_t(h, &h->bk_tag, N));
     }
-    HB_CK(cudaMemcpyAsync(h->bk_pos, h->pos, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->bk_pos, h->pos(), N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_vel, h->vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_force, h->force, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_virial, h->virial, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_image, h->image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->bk_tag, h->tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
+    h->bk_cur = h->cur;
+    h->bk_parity = h->parity;
     h->bk_valid = true;
     return HB_OK;
 }
@@ -377,12 +502,18 @@ int backup_state(hb_system *h)
 int restore_state(hb_system *h)
 {
     const size_t N = (size_t)h->N;
-    HB_CK(cudaMemcpyAsync(h->pos, h->bk_pos, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+    h->cur = h->bk_cur;
+    h->parity = h->bk_parity;
+    HB_CK(cudaMemcpyAsync(h->pos(), h->bk_pos, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->vel, h->bk_vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->force, h->bk_force, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->virial, h->bk_virial, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->image, h->bk_image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->tag, h->bk_tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(launch_rtag(h));
+    HB_TRY(clear_need_flags(h));
     h->nlist_valid = h->cells_valid = false;
+    h->moved = true;
     return HB_OK;
 }
 
@@ -390,11 +521,15 @@ int restore_state(hb_system *h)
 int step_sync(hb_system *h, float dt)
 {
     HB_TRY(ensure_forces(h));
-    HB_CK(launch_nve(h, dt, false, true, 0, false));
+    const NveArgs a = make_nve(h, dt, false, true, h->pos(), 0, false);
+    HB_CK(launch_nve(h, a));
+    h->parity++;
+    h->moved = true;
     HB_TRY(read_flags(h));
-    if (h->h_flags[FL_NEED_BUILD]) HB_TRY(build_nlist_sync(h));
-    HB_CK(launch_force(h));
-    HB_CK(launch_nve(h, dt, true, false, 0, false));
+    if (h->h_flags[a.need_set]) HB_TRY(build_nlist_sync(h));
+    HB_CK(launch_force(h, nullptr));
+    h->forces_valid = true;
+    HB_CK(launch_nve(h, make_nve(h, dt, true, false, h->pos(), 0, false)));
     h->stats.steps++;
     return HB_OK;
 }
@@ -408,11 +543,12 @@ int run_chunk(hb_system *h, float dt, int n)
     for (int attempt = 0; attempt < 8; attempt++) {
         HB_TRY(ensure_forces(h));
         if (dt != h->graph_dt) { destroy_graphs(h); h->graph_dt = dt; }
-        auto it = h->graphs.find(n);
+        const int64_t key = ((int64_t)n << 2) | ((h->cur & 1) << 1) | (h->parity & 1);
+        auto it = h->graphs.find(key);
         if (it == h->graphs.end()) {
             hb_system::GraphEntry ge;
             HB_TRY(build_graph(h, n, dt, &ge));
-            it = h->graphs.emplace((int64_t)n, ge).first;
+            it = h->graphs.emplace(key, ge).first;
         }
         HB_TRY(backup_state(h));
         const int builds_before = h->h_flags[FL_BUILDS];
@@ -420,24 +556,30 @@ int run_chunk(hb_system *h, float dt, int n)
         h->stats.graph_launches++;
         HB_TRY(read_flags(h));
         const int nb = h->h_flags[FL_BUILDS] - builds_before;
-        h->stats.kernel_launches += it->second.nkernels_fixed + (h->tun.graph_mode == 2 ? nb * rebuild_kernel_count(h) : 0);
+        h->stats.kernel_launches += it->second.nkernels_fixed + (h->tun.graph_mode == 2 ? nb * kRebuildKernels : 0);
         h->stats.rebuilds = h->h_flags[FL_BUILDS];
+        if (h->tun.fuse_nve) h->cur ^= (n - 1) & 1;
+        h->parity += n;
+        h->moved = true;
+        h->forces_valid = true;   // the graph's last kernel evaluated the forces in the final order
         if (h->h_flags[FL_BAD]) {
             h->err = "a particle is non-finite or outside the box";
             set_flag(h, FL_BAD, 0);
             return HB_ENAN;
         }
-        if (!h->h_flags[FL_OVERFLOWED]) {
+        if (!h->h_flags[FL_OVERFLOWED] && !h->h_flags[FL_STAGE_OVER]) {
             if (nb > 0) h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
             h->stats.steps += n;
             return HB_OK;
         }
-        // some build inside the chunk overflowed its rows: go back, grow, redo
-        const int needed = h->h_flags[FL_OVERFLOWED];
+        // some build inside the chunk overflowed its rows or its staging area: go back, grow, redo
+        const int rows_needed = h->h_flags[FL_OVERFLOWED], slots_needed = h->h_flags[FL_STAGE_OVER];
         h->stats.overflow_retries++;
         HB_TRY(restore_state(h));
         HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
-        HB_TRY(ensure_rows(h, (int)(needed * 1.25) + 8));
+        HB_TRY(set_flag(h, FL_STAGE_OVER, 0));
+        if (slots_needed) HB_TRY(choose_tiles(h, (int)(slots_needed * 1.2) + 32));
+        if (rows_needed) HB_TRY(ensure_rows(h, (int)(rows_needed * 1.25) + 8));
         HB_TRY(build_nlist_sync(h));
     }
     h->err = "neighbor-list rows keep overflowing inside hb_run_nve";
@@ -495,7 +637,8 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     *out = h;  // from here on the caller can read hb_last_error and must hb_destroy
 
     const size_t n = (size_t)N;
-    HB_TRY(dev_alloc_t(h, &h->pos, n));
+    HB_TRY(dev_alloc_t(h, &h->posbuf[0], n));
+    HB_TRY(dev_alloc_t(h, &h->posbuf[1], n));
     HB_TRY(dev_alloc_t(h, &h->vel, n));
     HB_TRY(dev_alloc_t(h, &h->force, n));
     HB_TRY(dev_alloc_t(h, &h->virial, 2 * n));
@@ -503,8 +646,12 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     HB_TRY(dev_alloc_t(h, &h->tag, n));
     HB_TRY(dev_alloc_t(h, &h->rtag, n));
     HB_TRY(dev_alloc_t(h, &h->pos_build, n));
+    HB_TRY(dev_alloc_t(h, &h->vel2, n));
+    HB_TRY(dev_alloc_t(h, &h->image2, 3 * n));
+    HB_TRY(dev_alloc_t(h, &h->tag2, n));
+    HB_TRY(dev_alloc_t(h, &h->cell_id, n));
     HB_TRY(dev_alloc_t(h, &h->cell_rank, n));
-    HB_TRY(dev_alloc_t(h, &h->cell_xyzi, n));
+    HB_TRY(dev_alloc_t(h, &h->perm, n));
     HB_TRY(dev_alloc_t(h, &h->nlistn, n));
     HB_TRY(dev_alloc_t(h, &h->params, (size_t)ntypes * ntypes));
     HB_TRY(dev_alloc_t(h, &h->flags, (size_t)FL_COUNT));
@@ -514,10 +661,12 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     HB_CK(cudaMemsetAsync(h->flags, 0, sizeof(int) * FL_COUNT, h->stream));
     HB_CK(cudaMemsetAsync(h->force, 0, sizeof(float4) * n, h->stream));
     HB_CK(cudaMemsetAsync(h->virial, 0, sizeof(float4) * 2 * n, h->stream));
-    int dev = 0, sms = 148;
+    int dev = 0, sms = 148, smem = 227 * 1024;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     h->sm_count = sms;
+    h->smem_max = smem;
     h->thermo_blocks = (int)std::min<int64_t>(cdiv(N, 256), (int64_t)sms * 4);
     HB_TRY(dev_alloc_t(h, &h->thermo_part, (size_t)(h->thermo_blocks + 2) * 11));
     HB_TRY(upload_params(h));
@@ -531,10 +680,11 @@ int hb_destroy(hb_system *h)
     destroy_graphs(h);
     auto it = g_stage.find(h);
     if (it != g_stage.end()) { dev_free(h, it->second.p); g_stage.erase(it); }
-    void *ptrs[] = {h->pos, h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->pos2, h->vel2, h->force2,
-                    h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_pos_build, h->bk_image,
-                    h->params, h->cell_count, h->cell_start, h->cell_rank, h->cell_xyzi, h->scan_tmp, h->nlist, h->nlistn,
-                    h->keys, h->keys2, h->perm, h->perm2, h->radix_counts, h->flags, h->thermo_part};
+    void *ptrs[] = {h->posbuf[0], h->posbuf[1], h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->vel2,
+                    h->force2, h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_image,
+                    h->bk_tag, h->params, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
+                    h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
+                    h->flags, h->thermo_part};
     for (void *p : ptrs) dev_free(h, p);
     if (h->h_flags) cudaFreeHost(h->h_flags);
     if (h->h_thermo) cudaFreeHost(h->h_thermo);
@@ -570,6 +720,7 @@ int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type, const 
     if (!on_device) HB_CK(cudaStreamSynchronize(h->stream));  // the caller's host buffers may be pageable
     h->have_state = true;
     h->cells_valid = h->nlist_valid = h->forces_valid = h->bk_valid = false;
+    h->moved = true;
     h->since_sort = -1;
     return HB_OK;
 }
@@ -622,14 +773,19 @@ int hb_build_cells(hb_system *h)
     HB_NEED(h);
     if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
     HB_TRY(configure_geometry(h));
+    if (h->cells_valid && !h->moved) return HB_OK;   // the cell list of these very positions is in place
     HB_TRY(enqueue_cells(h, nullptr));
+    HB_CK(launch_cell_copyback(h, nullptr));
     HB_TRY(read_flags(h));
+    h->nlist_valid = h->forces_valid = false;        // the storage order changed
     if (h->h_flags[FL_BAD]) {
         h->err = "a particle is non-finite or outside the box";
         set_flag(h, FL_BAD, 0);
+        h->cells_valid = false;
         return HB_ENAN;
     }
     h->cells_valid = true;
+    h->moved = false;
     return HB_OK;
 }
 
@@ -654,8 +810,10 @@ int hb_needs_rebuild(hb_system *h, int *need)
     HB_NEED(h);
     if (!need) return HB_EINVAL;
     if (!h->nlist_valid) { *need = 1; return HB_OK; }
+    HB_TRY(set_flag(h, FL_CHECK, 0));
+    HB_CK(launch_disp_check(h));
     HB_TRY(read_flags(h));
-    *need = h->h_flags[FL_NEED_BUILD] ? 1 : 0;
+    *need = h->h_flags[FL_CHECK] ? 1 : 0;
     return HB_OK;
 }
 
@@ -668,11 +826,7 @@ int hb_compute_lj(hb_system *h, int shift_mode)
         h->shift_mode = shift_mode;
         HB_TRY(upload_params(h));
     }
-    // the force kernel clears FL_NEED_BUILD; as a stand-alone call that must not lose a pending decision
-    HB_TRY(read_flags(h));
-    const int pending = h->h_flags[FL_NEED_BUILD];
-    HB_CK(launch_force(h));
-    if (pending) HB_TRY(set_flag(h, FL_NEED_BUILD, 1));
+    HB_CK(launch_force(h, nullptr));
     h->forces_valid = true;
     return HB_OK;
 }
@@ -744,16 +898,8 @@ int hb_get_cells(hb_system *h, int32_t *m_out, int32_t *cell_start, uint32_t *ce
     }
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     if (cell_start) HB_CK(cudaMemcpyAsync(cell_start, h->cell_start, sizeof(int) * (size_t)(h->ncells + 1), kind, h->stream));
-    if (cell_tags) {
-        if (on_device) {
-            HB_CK(launch_cell_tags(h, cell_tags));
-        } else {
-            Stage &st = g_stage[h];
-            HB_TRY(ensure_stage(h, &st.p, &st.cap, (size_t)h->N * 4));
-            HB_CK(launch_cell_tags(h, (uint32_t *)st.p));
-            HB_CK(cudaMemcpyAsync(cell_tags, st.p, (size_t)h->N * 4, cudaMemcpyDeviceToHost, h->stream));
-        }
-    }
+    // the particle data is kept in cell order: the members of cell c are the storage slots of its CSR range
+    if (cell_tags) HB_CK(cudaMemcpyAsync(cell_tags, h->tag, (size_t)h->N * 4, kind, h->stream));
     HB_CK(cudaStreamSynchronize(h->stream));
     return HB_OK;
 }
@@ -841,11 +987,9 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
     if (!stage || reps <= 0 || reps > 100000 || !mean_ms || flush_l2_bytes < 0) return HB_EINVAL;
     if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
     int which = -1;
-    const char *names[] = {"lj_force", "nlist", "cells", "rebuild", "nve"};
-    for (int k = 0; k < 5; k++) if (!strcmp(stage, names[k])) which = k;
+    const char *names[] = {"lj_force", "nlist", "cells", "rebuild", "nve", "lj_nve"};
+    for (int k = 0; k < 6; k++) if (!strcmp(stage, names[k])) which = k;
     if (which < 0) { h->err = std::string("unknown stage ") + stage; return HB_EINVAL; }
-    HB_TRY(read_flags(h));
-    const int pending = h->h_flags[FL_NEED_BUILD];  // the timed kernels clear or set it; put it back afterwards
     void *scratch = nullptr;
     if (flush_l2_bytes > 0) HB_TRY(dev_alloc(h, &scratch, (size_t)flush_l2_bytes));
     const int nev = flush_l2_bytes > 0 ? reps : 1;
@@ -854,11 +998,16 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
     int rc = HB_OK;
     auto launch = [&]() -> int {
         switch (which) {
-            case 0: HB_CK(launch_force(h)); break;
-            case 1: HB_CK(launch_nlist(h, nullptr)); break;
+            case 0: HB_CK(launch_force(h, nullptr)); break;
+            case 1: HB_CK(launch_nlist(h, nullptr, false)); break;
             case 2: HB_TRY(enqueue_cells(h, nullptr)); break;
             case 3: HB_TRY(enqueue_rebuild(h, nullptr)); break;
-            default: HB_CK(launch_nve(h, 0.0f, true, true, 0, false)); break;
+            case 4: HB_CK(launch_nve(h, make_nve(h, 0.0f, true, true, h->pos(), 0, false))); break;
+            default: {
+                const NveArgs a = make_nve(h, 0.0f, true, true, h->posbuf[h->cur ^ 1], 0, false);
+                HB_CK(launch_force(h, &a));
+                break;
+            }
         }
         return HB_OK;
     };
@@ -883,7 +1032,12 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
     }
     for (int k = 0; k < nev; k++) { cudaEventDestroy(ev0[k]); cudaEventDestroy(ev1[k]); }
     dev_free(h, scratch);
-    if (rc == HB_OK) rc = set_flag(h, FL_NEED_BUILD, pending);
+    if (rc == HB_OK) rc = clear_need_flags(h);
+    if (rc == HB_OK && (which == 2 || which == 3)) {
+        // the timed cell builds re-ordered the scratch set (and, for "rebuild", the particles): make the list whole again
+        h->nlist_valid = false;
+        rc = ensure_forces(h);
+    }
     return rc;
 }
 
@@ -891,12 +1045,15 @@ static int *tunable_slot(hb_system *h, const char *name)
 {
     if (!name) return nullptr;
     if (!strcmp(name, "tpp")) return &h->tun.tpp;
-    if (!strcmp(name, "force_block")) return &h->tun.force_block;
-    if (!strcmp(name, "force_passes")) return &h->tun.force_passes;
+    if (!strcmp(name, "epl")) return &h->tun.epl;
     if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
-    if (!strcmp(name, "nlist_cap")) return &h->tun.nlist_cap;
+    if (!strcmp(name, "tile_x")) return &h->tun.tile_x;
+    if (!strcmp(name, "tile_y")) return &h->tun.tile_y;
+    if (!strcmp(name, "tile_z")) return &h->tun.tile_z;
+    if (!strcmp(name, "stage_cap")) return &h->tun.stage_cap;
     if (!strcmp(name, "row_pitch")) return &h->tun.row_pitch;
     if (!strcmp(name, "cell_sort")) return &h->tun.cell_sort;
+    if (!strcmp(name, "fuse_nve")) return &h->tun.fuse_nve;
     if (!strcmp(name, "graph_mode")) return &h->tun.graph_mode;
     if (!strcmp(name, "graph_steps")) return &h->tun.graph_steps;
     return nullptr;
@@ -908,19 +1065,23 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     int *slot = tunable_slot(h, name);
     if (!slot) { h->err = std::string("unknown tunable ") + (name ? name : "(null)"); return HB_EINVAL; }
     bool ok = true;
-    if (slot == &h->tun.tpp) ok = value == 1 || value == 2 || value == 4 || value == 8;
-    else if (slot == &h->tun.force_passes) ok = value >= 0 && value <= 64;
-    else if (slot == &h->tun.force_block) ok = value >= 32 && value <= 256 && value % 32 == 0;
+    if (slot == &h->tun.tpp) ok = value == 2 || value == 4 || value == 8;
+    else if (slot == &h->tun.epl) ok = value == 4 || value == 8;
     else if (slot == &h->tun.nlist_ppi) ok = value == 1 || value == 2 || value == 4;
-    else if (slot == &h->tun.nlist_cap) ok = value >= 64 && value <= 1024 && value % 32 == 0;
+    else if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z) ok = value >= 0 && value <= 16;
+    else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;
     else if (slot == &h->tun.row_pitch) ok = value >= 0 && value <= 4096;
-    else if (slot == &h->tun.cell_sort) ok = value == 0 || value == 1;
+    else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve) ok = value == 0 || value == 1;
     else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 2;
     else if (slot == &h->tun.graph_steps) ok = value >= 1 && value <= 2000;
     if (!ok) { h->err = std::string("value out of range for tunable ") + name; return HB_EINVAL; }
     *slot = value;
     destroy_graphs(h);
     if (slot == &h->tun.row_pitch && value > 0) HB_TRY(ensure_rows(h, value));
+    if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z || slot == &h->tun.stage_cap) {
+        h->nlist_valid = false;
+        if (h->m > 0) HB_TRY(choose_tiles(h, 0));
+    }
     return HB_OK;
 }
 

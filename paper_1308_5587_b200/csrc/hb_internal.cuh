@@ -11,13 +11,17 @@
 
 // Device-side flag words (one int array, mirrored in pinned host memory).
 enum {
-    FL_NEED_BUILD = 0,  // set by the drift kernel when a particle exceeded r_buff/2; cleared by the force kernel
-    FL_MAX_NBRS = 1,    // atomicMax of row lengths NEEDED by the last build (may exceed row_pitch => overflow)
-    FL_BAD = 2,         // non-finite / out-of-box particle seen while binning
-    FL_BUILDS = 3,      // number of list builds done on the device
-    FL_DONE_CTR = 4,    // "last block done" counter of the drift kernel
-    FL_OVERFLOWED = 5,  // sticky: some build since the last host check overflowed its rows
-    FL_COUNT = 8
+    FL_NEED0 = 0,       // rebuild decision of the drifts with even / odd drift number: the drift kernel of
+    FL_NEED1 = 1,       //   drift d sets FL_NEED0 + (d & 1) and clears the other one for drift d + 1
+    FL_MAX_NBRS = 2,    // atomicMax of row lengths NEEDED by the last build (may exceed row_pitch => overflow)
+    FL_BAD = 3,         // non-finite / out-of-box particle seen while binning
+    FL_BUILDS = 4,      // number of list builds done on the device
+    FL_DONE_CTR = 5,    // "last block done" counter of the drift kernels
+    FL_OVERFLOWED = 6,  // sticky: some build since the last host check overflowed its rows (value = rows needed)
+    FL_STAGE_OVER = 7,  // sticky: some tile needed more shared-memory slots than stage_cap (value = slots needed)
+    FL_SCAN_CTR = 8,    // "last block done" counter of the cell scan
+    FL_CHECK = 9,       // result of the on-demand displacement check (hb_needs_rebuild)
+    FL_COUNT = 16
 };
 
 struct PairParam {  // one per type pair, 16 B
@@ -27,14 +31,33 @@ struct PairParam {  // one per type pair, 16 B
     float eshift;   // V_lj(r_cut) if energy shift, else 0
 };
 
+// A tile is a brick of tx x ty x tz cells (clipped at the upper faces of the box).  One
+// thread block owns one tile: it stages the positions of the tile's cells and of the
+// one-cell halo around them in shared memory, already shifted to the periodic image
+// the tile sees, and both the list build and the force evaluation work on that copy.
+struct TileGeom {
+    int m;              // cells per axis
+    int tx, ty, tz;     // tile dimensions in cells
+    int ntx, nty, ntz;  // tiles per axis
+    int ntiles;
+    int cap;            // shared-memory slots (slot 0 is the far-away dummy)
+    float L;
+};
+
+constexpr int TILE_THREADS = 256;
+constexpr int TILE_HMAX = 256;        // halo cells per tile, at most
+constexpr int TILE_ROWS_MAX = 32;     // own (y, z) rows per tile, at most
+constexpr int ROW_PAD = 32;           // list rows are padded with dummy entries to a multiple of this
+
 struct Tunables {
-    int tpp = 8;
-    int force_block = 128;
-    int force_passes = 0;  // 0 = auto
-    int nlist_ppi = 4;
-    int nlist_cap = 512;
+    int tpp = 4;           // threads per particle in the force kernel
+    int epl = 4;           // list entries per thread per iteration (4 or 8)
+    int nlist_ppi = 4;     // particles tested per candidate load
+    int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
+    int stage_cap = 0;     // 0 = estimated from the density
     int row_pitch = 0;
     int cell_sort = 1;
+    int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
     int graph_mode = 2;
     int graph_steps = 50;
 };
@@ -54,42 +77,53 @@ struct hb_system {
     std::string err;
 
     // particle data (storage order), SoA of 16 B vectors
-    float4 *pos = nullptr;      // x, y, z, type bits
+    float4 *posbuf[2] = {nullptr, nullptr};  // x, y, z, type bits; posbuf[cur] is current (the fused step ping-pongs)
+    int cur = 0;
     float4 *vel = nullptr;      // vx, vy, vz, unused
     float4 *force = nullptr;    // Fx, Fy, Fz, U_i
     float4 *virial = nullptr;   // [2N]: (xx, xy, xz, yy), (yz, zz, 0, 0)
     int *image = nullptr;       // [3][N]
     uint32_t *tag = nullptr;    // storage slot -> tag
     uint32_t *rtag = nullptr;   // tag -> storage slot
-    float4 *pos_build = nullptr;
-    // second set for hb_sort's gather and hb_run_nve's chunk backup
-    float4 *pos2 = nullptr, *vel2 = nullptr, *force2 = nullptr, *virial2 = nullptr;
+    float4 *pos_build = nullptr;  // positions at the last list build, in the storage order that build made
+    // scratch set: target of the reorder at every build and of hb_sort's gather
+    float4 *vel2 = nullptr, *force2 = nullptr, *virial2 = nullptr;
     int *image2 = nullptr;
     uint32_t *tag2 = nullptr;
-    float4 *bk_pos = nullptr, *bk_vel = nullptr, *bk_force = nullptr, *bk_virial = nullptr, *bk_pos_build = nullptr;
+    // backup for hb_run_nve's chunk redo
+    float4 *bk_pos = nullptr, *bk_vel = nullptr, *bk_force = nullptr, *bk_virial = nullptr;
     int *bk_image = nullptr;
+    uint32_t *bk_tag = nullptr;
+    int bk_cur = 0, bk_parity = 0;
     PairParam *params = nullptr;
 
-    // cell list (CSR)
+    float4 *pos() const { return posbuf[cur]; }
+
+    // cell list (CSR); after a build particle k of the storage order lies in the cell whose range holds k
     int m = 0;
     int64_t ncells = 0, ncells_alloc = 0;
-    int *cell_count = nullptr;   // [ncells]
+    int *cell_count = nullptr;   // [ncells] zero between builds
+    int *cell_local = nullptr;   // [ncells] exclusive scan inside a scan tile
     int *cell_start = nullptr;   // [ncells + 1]
+    int *cell_id = nullptr;      // [N] cell of particle i (old order)
     int *cell_rank = nullptr;    // [N] slot inside the cell handed out by the atomic
-    float4 *cell_xyzi = nullptr; // [N] (x, y, z, index bits) in CSR order -- the paper's celldata
-    int *scan_tmp = nullptr;     // block sums
-    int64_t scan_tmp_len = 0;
+    int *perm = nullptr;         // [N] new slot -> old slot
+    int *scan_sums = nullptr;    // block sums / block offsets of the cell scan
+    int64_t scan_sums_len = 0;
 
-    // neighbor list: row i = nlist[i * row_pitch .. + nlistn[i])
+    // neighbor list: row i = nlist[i * row_pitch .. + nlistn[i]), entries are shared-memory slots of i's tile
+    TileGeom geom{};
     int row_pitch = 0;
-    int *nlist = nullptr;
+    uint16_t *nlist = nullptr;
     int *nlistn = nullptr;
     int64_t nlist_alloc = 0;
 
     // sort scratch
-    uint32_t *keys = nullptr, *keys2 = nullptr, *perm = nullptr, *perm2 = nullptr;
+    uint32_t *keys = nullptr, *keys2 = nullptr, *sperm = nullptr, *sperm2 = nullptr;
     int *radix_counts = nullptr;
     int64_t radix_counts_len = 0;
+    int *scan_tmp = nullptr;
+    int64_t scan_tmp_len = 0;
 
     // flags + reductions
     int *flags = nullptr;        // device [FL_COUNT]
@@ -98,18 +132,19 @@ struct hb_system {
     double *h_thermo = nullptr;     // pinned [12]
     int thermo_blocks = 0;
     int sm_count = 148;
+    int smem_max = 227 * 1024;
 
     // host-side state machine
     bool have_state = false, cells_valid = false, nlist_valid = false, forces_valid = false, bk_valid = false;
+    bool moved = true;           // positions changed since the last cell build
+    int parity = 0;              // number of drifts done so far, mod 2
     hb_stats_t stats{};
-    int64_t builds_seen = 0;
     int64_t since_sort = -1;     // steps since the last hb_sort inside hb_run_nve (-1 = never sorted)
 
-    // graph cache: key = (nsteps, mode, flags) -> exec
+    // graph cache: key = (nsteps, cur, parity) -> exec
     struct GraphEntry { cudaGraph_t g = nullptr; cudaGraphExec_t e = nullptr; int nkernels_fixed = 0; };
     std::map<int64_t, GraphEntry> graphs;
     float graph_dt = 0;
-    int graph_sig = 0;
 };
 
 #define HB_CK(call)                                                                          \
@@ -129,31 +164,45 @@ struct hb_system {
 
 static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
+// What the drift part of a step kernel needs (nve_kernel and the fused force kernel).
+struct NveArgs {
+    float4 *vel;
+    int *image;
+    const float4 *pos_build;
+    float4 *pos_out;       // where the drifted positions go (== pos_in for the stand-alone kernel)
+    float dt, half_buff2;
+    int kick_prev, kick_drift;
+    int need_set, need_clear;   // flag indices
+    cudaGraphConditionalHandle cond;
+    int use_cond;
+};
+
 // ---- kernel launchers (each enqueues on h->stream and returns cudaGetLastError) ----
-// cells.cu
-cudaError_t launch_cell_clear(hb_system *h, const int *pred);
-cudaError_t launch_cell_bin(hb_system *h, const int *pred);
-cudaError_t launch_scan_exclusive(hb_system *h, const int *in, int *out, int64_t n, int *tmp, const int *pred);
+// cells.cu: Algorithm 2 + reorder of the particle data into cell order
+cudaError_t launch_cell_count(hb_system *h, const int *pred);
+cudaError_t launch_cell_scan(hb_system *h, const int *pred);
 cudaError_t launch_cell_scatter(hb_system *h, const int *pred);
-cudaError_t launch_cell_sort(hb_system *h, const int *pred);
+cudaError_t launch_cell_gather(hb_system *h, const int *pred);
+cudaError_t launch_cell_copyback(hb_system *h, const int *pred);   // when no list kernel follows
+cudaError_t launch_scan_exclusive(hb_system *h, const int *in, int *out, int64_t n, int *tmp);
 // nlist.cu
-cudaError_t launch_nlist(hb_system *h, const int *pred);
+cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback);
 size_t nlist_smem_bytes(const hb_system *h);
 // force.cu
-cudaError_t launch_force(hb_system *h);
+cudaError_t launch_force(hb_system *h, const NveArgs *nve /* nullable: forces only */);
+size_t force_smem_bytes(const hb_system *h);
 // nve.cu
-//   mode bit 0: do the second half kick of the previous step first; bit 1: do the first half kick + drift
-cudaError_t launch_nve(hb_system *h, float dt, bool kick_prev, bool kick_drift, cudaGraphConditionalHandle cond, bool use_cond);
+cudaError_t launch_nve(hb_system *h, const NveArgs &a);
+cudaError_t launch_disp_check(hb_system *h);
 cudaError_t launch_thermo(hb_system *h);
 // sort.cu
 cudaError_t launch_sfc_keys(hb_system *h);
-cudaError_t launch_radix_sort(hb_system *h, int key_bits);  // keys/perm -> sorted in keys/perm
-cudaError_t launch_gather_state(hb_system *h);              // by perm into the second set
+cudaError_t launch_radix_sort(hb_system *h, int key_bits);  // keys/sperm -> sorted in keys/sperm
+cudaError_t launch_gather_state(hb_system *h);              // by sperm into the scratch set (positions into pos_build)
 cudaError_t launch_rtag(hb_system *h);
 // accessors
 cudaError_t launch_pack_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz, const int32_t *image);
 cudaError_t launch_unpack_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image);
 cudaError_t launch_unpack_forces(hb_system *h, float *f4, float *vir6);
-cudaError_t launch_cell_tags(hb_system *h, uint32_t *out);
 cudaError_t launch_nlist_counts_by_tag(hb_system *h, int *counts);
 cudaError_t launch_nlist_fill_by_tag(hb_system *h, const int64_t *row_start, uint32_t *out);

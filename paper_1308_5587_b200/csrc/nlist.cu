@@ -2,176 +2,190 @@
 //
 // The paper runs one thread per particle and names the resulting scattered,
 // unsynchronised row writes "a big bottleneck" that "GF100 does not have enough
-// shared memory to regularize".  Here ONE WARP OWNS ONE CELL:
-//   1. lanes 0..26 look up the 27 adjacent cells (on the fly, no celladj table:
-//      PAPER.md:187 stored it to save registers; a warp has lanes to spare) and
-//      the periodic shift of each, and a warp scan turns their occupancies into
-//      offsets;
-//   2. the warp stages the candidates (R_j + shift, j) of all 27 cells, compacted,
-//      in shared memory -- coalesced float4 reads of the CSR cell list;
-//   3. for every particle i of the cell (PPI at a time, so each shared-memory
-//      candidate load serves PPI distance tests) lane l tests candidates l, l+32,
-//      ... and records the hits as bits of a register; one warp prefix sum of the
-//      per-lane __popc counts then gives every lane its slots, the row is
-//      assembled in shared memory and flushed with coalesced stores into a
-//      row-major, 128-byte aligned, padded list.  (Round-1 ncu: a __ballot_sync
-//      per 32 tests cost 27 instructions per test group; the bit mask costs 8.)
-// The periodic shift is applied once to the staged copy, so no minimum-image
-// arithmetic is left in the inner loop, and x_j + shift is exact or within one
-// ulp of x (hard part 3).
-#include "hb_internal.cuh"
+// shared memory to regularize".  Here ONE BLOCK OWNS ONE TILE of
+// cells (tile.cuh): the tile plus its one-cell halo is staged once in shared
+// memory, already shifted to the periodic image the tile sees, and then ONE WARP
+// OWNS ONE CELL of the tile:
+//   1. lanes 0..8 look up the nine x-rows of three adjacent cells (on the fly, no
+//      celladj table: PAPER.md:187 stored it to save registers) -- in the staged
+//      layout each row is one contiguous run of slots -- and the warp flattens the
+//      nine runs into one list of candidate slots (16-bit), padded with the
+//      far-away dummy slot 0 to whole groups of 32;
+//   2. for every particle i of the cell (PPI at a time, so each candidate load
+//      serves PPI distance tests) lane l tests candidates l, l+32, ... and records
+//      the hits as bits of a register; one warp prefix sum of the per-lane __popc
+//      counts gives every lane its positions in the row and the lanes write their
+//      hits' SLOT NUMBERS (16 bit) straight into the row-major, 128-byte aligned
+//      list; the row is padded with slot 0 to a multiple of 32 entries.
+// List entries are slots of the tile's staging layout, not particle indices: the
+// force kernel stages the same tile the same way and gathers from shared memory
+// (hb_get_nlist translates back to tags).  Half the bytes of a 32-bit index list.
+// The kernel also finishes the reorder of the particle data: it copies the tile's
+// own particles from the scratch set (cell order) back into the live arrays.
+#include "tile.cuh"
 
-constexpr int NL_WARPS = 4;
-
-__host__ __device__ inline size_t nlist_warp_smem(int cap, int ppi, int pitch)
-{
-    return (size_t)cap * 16 + (size_t)ppi * pitch * 4 + 32 * 4 /*offs*/ + 32 * 4 /*astart*/ + 96 * 4 /*shift*/;
-}
+constexpr int NL_CLIST = 1024;   // candidate slots per warp per chunk = 32 groups of 32 = one bit mask
+constexpr int NL_WARPS = TILE_THREADS / 32;
 
 size_t nlist_smem_bytes(const hb_system *h)
 {
-    return NL_WARPS * nlist_warp_smem(h->tun.nlist_cap, h->tun.nlist_ppi, h->row_pitch);
+    return (size_t)h->geom.cap * 16 + (size_t)NL_WARPS * NL_CLIST * 2;
 }
 
+struct CopyBack {   // scratch set -> live arrays; pos == nullptr: skip
+    float4 *pos, *vel;
+    const float4 *vel2;
+    int *image;
+    const int *image2;
+    uint32_t *tag, *rtag;
+    const uint32_t *tag2;
+    int N;
+};
+
 template <int PPI>
-__global__ void __launch_bounds__(NL_WARPS * 32)
-nlist_kernel(const int *__restrict__ cell_start, const float4 *__restrict__ cell_xyzi, int m, int64_t ncells, float L,
-             float rmax2, int cap, int pitch, int *__restrict__ nlist, int *__restrict__ nlistn, int *__restrict__ flags,
-             const int *__restrict__ pred)
+__global__ void __launch_bounds__(TILE_THREADS)
+nlist_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__restrict__ pos_build, float rmax2,
+                  int pitch, uint16_t *__restrict__ nlist, int *__restrict__ nlistn, int *__restrict__ flags,
+                  const int *__restrict__ pred, CopyBack cb)
 {
     if (pred && *pred == 0) return;
-    if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_BUILDS] += 1;
-
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ TileShared s;
+    float4 *stage = reinterpret_cast<float4 *>(smem_raw);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    unsigned char *wbase = smem_raw + (size_t)warp * nlist_warp_smem(cap, PPI, pitch);
-    float4 *cand = reinterpret_cast<float4 *>(wbase);
-    int *rows = reinterpret_cast<int *>(wbase + (size_t)cap * 16);
-    int *offs = rows + PPI * pitch;
-    int *astart = offs + 32;
-    float *shift = reinterpret_cast<float *>(astart + 32);
+    uint16_t *clist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)g.cap * 16) + warp * NL_CLIST;
 
-    const int64_t c = (int64_t)blockIdx.x * NL_WARPS + warp;
-    if (c >= ncells) return;
-    const int cstart = cell_start[c];
-    const int n_c = cell_start[c + 1] - cstart;
-    if (n_c == 0) return;
+    if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_BUILDS] += 1;
+    TileCtx t;
+    tile_decode(g, blockIdx.x, t);
+    const bool fits = tile_tables(g, cell_start, t, s, flags);
 
-    // ---- 1. the 27 adjacent cells, their occupancies and periodic shifts ----
-    const int cx = (int)(c % m), cy = (int)((c / m) % m), cz = (int)(c / ((int64_t)m * m));
-    int a_start = 0, a_cnt = 0;
-    float sx = 0.f, sy = 0.f, sz = 0.f;
-    if (lane < 27) {
-        int nx = cx + lane % 3 - 1, ny = cy + (lane / 3) % 3 - 1, nz = cz + lane / 9 - 1;
-        if (nx < 0) { nx += m; sx = -L; } else if (nx >= m) { nx -= m; sx = L; }
-        if (ny < 0) { ny += m; sy = -L; } else if (ny >= m) { ny -= m; sy = L; }
-        if (nz < 0) { nz += m; sz = -L; } else if (nz >= m) { nz -= m; sz = L; }
-        const int64_t nc = nx + (int64_t)m * (ny + (int64_t)m * nz);
-        a_start = cell_start[nc];
-        a_cnt = cell_start[nc + 1] - a_start;
+    // the reorder's last leg: own particles, scratch set -> live arrays (always, so the state stays whole)
+    if (cb.pos) {
+        for (int q = threadIdx.x; q < t.nown; q += TILE_THREADS) {
+            const int r = tile_row_of(t, s, q);
+            const int gi = s.own_start[r] + (q - s.own_off[r]);
+            cb.pos[gi] = pos_build[gi];
+            cb.vel[gi] = cb.vel2[gi];
+            cb.image[gi] = cb.image2[gi];
+            cb.image[cb.N + gi] = cb.image2[cb.N + gi];
+            cb.image[2 * (int64_t)cb.N + gi] = cb.image2[2 * (int64_t)cb.N + gi];
+            const uint32_t tg = cb.tag2[gi];
+            cb.tag[gi] = tg;
+            cb.rtag[tg] = gi;
+        }
     }
-    int incl = a_cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int y = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += y;
-    }
-    const int T = __shfl_sync(0xffffffffu, incl, 31);
-    const int self0 = __shfl_sync(0xffffffffu, incl - a_cnt, 13);  // candidate number of the own cell's first member
-    offs[lane] = incl - a_cnt;  // lanes 27..31 hold T
-    astart[lane] = a_start;
-    shift[3 * lane + 0] = sx;
-    shift[3 * lane + 1] = sy;
-    shift[3 * lane + 2] = sz;
-    __syncwarp();
+    if (!fits) return;
+    tile_stage_positions(g, t, s, pos_build, stage);
+    __syncthreads();
 
     int wmax = 0;
+    const int ncell_own = t.ex * t.ey * t.ez;
+    for (int oc = warp; oc < ncell_own; oc += NL_WARPS) {
+        const int lx = oc % t.ex, ly = (oc / t.ex) % t.ey, lz = oc / (t.ex * t.ey);
+        const int hc = ((lz + 1) * t.hy + (ly + 1)) * t.hx + (lx + 1);
+        const int cslot0 = s.hslot[hc];
+        const int n_c = s.hslot[hc + 1] - cslot0;
+        if (n_c == 0) continue;
+        const int cg0 = s.hg[hc];
 
-    for (int k0 = 0; k0 < T; k0 += cap) {
-        const int Tc = min(cap, T - k0);
-        const int ngroups = (Tc + 31) >> 5;
-        // ---- 2. stage the candidates, compacted, shifted to their periodic image; pad to whole groups ----
-        for (int k = lane; k < (ngroups << 5); k += 32) {
-            float4 e = make_float4(3e30f, 3e30f, 3e30f, __int_as_float(-2));
-            if (k < Tc) {
-                const int kk = k0 + k;
-                int a = 0;
-#pragma unroll
-                for (int s = 16; s > 0; s >>= 1)
-                    if (offs[a + s] <= kk) a += s;
-                e = cell_xyzi[astart[a] + (kk - offs[a])];
-                e.x += shift[3 * a + 0];
-                e.y += shift[3 * a + 1];
-                e.z += shift[3 * a + 2];
-            }
-            cand[k] = e;
+        // ---- 1. nine runs of candidates (Alg. 3 l.11: the 27 adjacent cells) ----
+        int rs = 0, rl = 0;
+        if (lane < 9) {
+            const int dy = lane % 3 - 1, dz = lane / 3 - 1;
+            const int hrow = ((lz + 1 + dz) * t.hy + (ly + 1 + dy)) * t.hx + lx;
+            rs = s.hslot[hrow];
+            rl = s.hslot[hrow + 3] - rs;
         }
-        __syncwarp();
-
-        // ---- 3. every particle of the cell against every candidate ----
-        for (int i0 = 0; i0 < n_c; i0 += PPI) {
-            float px[PPI], py[PPI], pz[PPI];
-            int pidx[PPI], cnt0[PPI];
-            unsigned hits[PPI];
+        int incl = rl;
 #pragma unroll
-            for (int p = 0; p < PPI; p++) {
-                pidx[p] = -1;
-                px[p] = py[p] = pz[p] = 1e30f;
-                cnt0[p] = 0;
-                hits[p] = 0u;
-                if (i0 + p < n_c) {
-                    const float4 q = cell_xyzi[cstart + i0 + p];  // same address in all lanes: one broadcast
-                    px[p] = q.x; py[p] = q.y; pz[p] = q.z;
-                    pidx[p] = __float_as_int(q.w);
-                    if (k0 > 0) cnt0[p] = __ldcg(&nlistn[pidx[p]]);
-                }
+        for (int o = 1; o < 16; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += y;
+        }
+        const int roff = incl - rl;
+        const int T = __shfl_sync(0xffffffffu, incl, 8);
+        // candidate number of the own cell's first member (run 4 = the own row)
+        const int self0 = __shfl_sync(0xffffffffu, roff, 4) + (cslot0 - __shfl_sync(0xffffffffu, rs, 4));
+
+        for (int k0 = 0; k0 < T; k0 += NL_CLIST) {
+            const int Tc = min(NL_CLIST, T - k0);
+            const int ngroups = (Tc + 31) >> 5;
+            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < 9; r++) {
+                const int rs_r = __shfl_sync(0xffffffffu, rs, r), rl_r = __shfl_sync(0xffffffffu, rl, r);
+                const int ro_r = __shfl_sync(0xffffffffu, roff, r);
+                const int lo = max(ro_r, k0), hi = min(ro_r + rl_r, k0 + Tc);
+                for (int v = lo + lane; v < hi; v += 32) clist[v - k0] = (uint16_t)(rs_r + (v - ro_r));
             }
-            // lane l tests candidates l, l+32, ...; bit g of hits[p] records candidate 32 g + l (Alg. 3 l.16-17)
-#pragma unroll 2
-            for (int g = 0; g < ngroups; g++) {
-                const float4 e = cand[(g << 5) + lane];
-                const unsigned bit = 1u << g;
+            for (int v = Tc + lane; v < (ngroups << 5); v += 32) clist[v] = 0;   // dummy: never a hit
+            __syncwarp();
+
+            // ---- 2. every particle of the cell against every candidate ----
+            for (int i0 = 0; i0 < n_c; i0 += PPI) {
+                float px[PPI], py[PPI], pz[PPI];
+                int gidx[PPI], cnt0[PPI];
+                unsigned hits[PPI];
 #pragma unroll
                 for (int p = 0; p < PPI; p++) {
-                    const float dx = e.x - px[p], dy = e.y - py[p], dz = e.z - pz[p];
-                    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                    if (d2 < rmax2) hits[p] |= bit;   // strict <
+                    gidx[p] = -1;
+                    px[p] = py[p] = pz[p] = -1e18f;
+                    cnt0[p] = 0;
+                    hits[p] = 0u;
+                    if (i0 + p < n_c) {
+                        const float4 q = stage[cslot0 + i0 + p];  // same address in all lanes: one broadcast
+                        px[p] = q.x; py[p] = q.y; pz[p] = q.z;
+                        gidx[p] = cg0 + i0 + p;
+                        if (k0 > 0) cnt0[p] = __ldcg(&nlistn[gidx[p]]);
+                    }
+                }
+                // lane l tests candidates l, l+32, ...; bit gq of hits[p] records candidate 32 gq + l (Alg. 3 l.16-17)
+#pragma unroll 2
+                for (int gq = 0; gq < ngroups; gq++) {
+                    const float4 e = stage[clist[(gq << 5) + lane]];
+                    const unsigned bit = 1u << gq;
+#pragma unroll
+                    for (int p = 0; p < PPI; p++) {
+                        const float dx = e.x - px[p], dy = e.y - py[p], dz = e.z - pz[p];
+                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                        if (d2 < rmax2) hits[p] |= bit;   // strict <
+                    }
+                }
+                // i != j: particle i0+p is candidate self0 + i0 + p; drop that one bit
+#pragma unroll
+                for (int p = 0; p < PPI; p++) {
+                    const int ks = self0 + i0 + p - k0;
+                    if (ks >= 0 && ks < Tc && (ks & 31) == lane) hits[p] &= ~(1u << (ks >> 5));
+                }
+                // compact: warp scan of the per-lane hit counts gives every lane its positions (l.18-19)
+#pragma unroll
+                for (int p = 0; p < PPI; p++) {
+                    if (gidx[p] < 0) continue;   // warp-uniform
+                    const int cn = __popc(hits[p]);
+                    int inc = cn;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int y = __shfl_up_sync(0xffffffffu, inc, o);
+                        if (lane >= o) inc += y;
+                    }
+                    const int total = cnt0[p] + __shfl_sync(0xffffffffu, inc, 31);
+                    int at = cnt0[p] + inc - cn;
+                    uint16_t *row = nlist + (int64_t)gidx[p] * pitch;
+                    unsigned hm = hits[p];
+                    while (hm) {
+                        const int gq = __ffs(hm) - 1;
+                        hm &= hm - 1;
+                        if (at < pitch) row[at] = clist[(gq << 5) + lane];
+                        at++;
+                    }
+                    const int nw = min(total, pitch);
+                    const int padded = min(pitch, (nw + ROW_PAD - 1) & ~(ROW_PAD - 1));
+                    if (nw + lane < padded) row[nw + lane] = 0;               // dummy entries up to a whole group
+                    if (lane == 0) nlistn[gidx[p]] = nw;                      // l.22
+                    wmax = max(wmax, total);
                 }
             }
-            // i != j: particle i0+p is candidate self0 + i0 + p; drop that one bit
-#pragma unroll
-            for (int p = 0; p < PPI; p++) {
-                const int ks = self0 + i0 + p - k0;
-                if (ks >= 0 && ks < Tc && (ks & 31) == lane) hits[p] &= ~(1u << (ks >> 5));
-            }
-            // compact: warp scan of the per-lane hit counts gives every lane its slots (l.18-19)
-#pragma unroll
-            for (int p = 0; p < PPI; p++) {
-                if (pidx[p] < 0) continue;   // warp-uniform
-                const int cn = __popc(hits[p]);
-                int inc = cn;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int y = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += y;
-                }
-                const int total = cnt0[p] + __shfl_sync(0xffffffffu, inc, 31);
-                int slot = cnt0[p] + inc - cn;
-                unsigned hm = hits[p];
-                while (hm) {
-                    const int g = __ffs(hm) - 1;
-                    hm &= hm - 1;
-                    if (slot < pitch) rows[p * pitch + slot] = __float_as_int(cand[(g << 5) + lane].w);
-                    slot++;
-                }
-                __syncwarp();
-                const int nw = min(total, pitch);
-                int *row = nlist + (int64_t)pidx[p] * pitch;
-                for (int k = cnt0[p] + lane; k < nw; k += 32) row[k] = rows[p * pitch + k];   // coalesced 128 B stores
-                if (lane == 0) nlistn[pidx[p]] = nw;                                            // l.22
-                wmax = max(wmax, total);
-            }
-            __syncwarp();
         }
     }
     // longest row needed by this build (may exceed the pitch: overflow)
@@ -181,18 +195,19 @@ nlist_kernel(const int *__restrict__ cell_start, const float4 *__restrict__ cell
     }
 }
 
-cudaError_t launch_nlist(hb_system *h, const int *pred)
+cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback)
 {
     const size_t smem = nlist_smem_bytes(h);
-    const unsigned grid = (unsigned)cdiv(h->ncells, NL_WARPS);
+    const unsigned grid = (unsigned)h->geom.ntiles;
     const float rmax2 = h->r_max * h->r_max;
+    CopyBack cb{};
+    if (copyback) cb = CopyBack{h->pos(), h->vel, h->vel2, h->image, h->image2, h->tag, h->rtag, h->tag2, (int)h->N};
     cudaError_t e;
-#define NL_LAUNCH(PPI)                                                                                              \
-    e = cudaFuncSetAttribute(nlist_kernel<PPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);            \
-    if (e != cudaSuccess) return e;                                                                                 \
-    nlist_kernel<PPI><<<grid, NL_WARPS * 32, smem, h->stream>>>(h->cell_start, h->cell_xyzi, h->m, h->ncells, h->L, \
-                                                                rmax2, h->tun.nlist_cap, h->row_pitch, h->nlist,    \
-                                                                h->nlistn, h->flags, pred);
+#define NL_LAUNCH(PPI)                                                                                                  \
+    e = cudaFuncSetAttribute(nlist_tile_kernel<PPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
+    if (e != cudaSuccess) return e;                                                                                     \
+    nlist_tile_kernel<PPI><<<grid, TILE_THREADS, smem, h->stream>>>(h->geom, h->cell_start, h->pos_build, rmax2,        \
+                                                                    h->row_pitch, h->nlist, h->nlistn, h->flags, pred, cb);
     switch (h->tun.nlist_ppi) {
         case 1: NL_LAUNCH(1) break;
         case 2: NL_LAUNCH(2) break;
@@ -211,16 +226,32 @@ __global__ void nlist_counts_by_tag_kernel(const int *__restrict__ nlistn, const
     if (i < N) counts[tag[i]] = nlistn[i];
 }
 
-__global__ void nlist_fill_by_tag_kernel(const int *__restrict__ nlist, const int *__restrict__ nlistn, int pitch,
-                                         const uint32_t *__restrict__ tag, int N, const int64_t *__restrict__ row_start,
-                                         uint32_t *__restrict__ out)
+// One block per tile: slot -> storage index through the same tables, then rows -> tags.
+__global__ void __launch_bounds__(TILE_THREADS)
+nlist_fill_by_tag_kernel(TileGeom g, const int *__restrict__ cell_start, const uint16_t *__restrict__ nlist,
+                         const int *__restrict__ nlistn, int pitch, const uint32_t *__restrict__ tag,
+                         const int64_t *__restrict__ row_start, uint32_t *__restrict__ out, int *__restrict__ flags)
 {
-    const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (i >= N) return;
-    const int lane = threadIdx.x & 31;
-    const int n = nlistn[i];
-    const int64_t o = row_start[tag[i]];
-    for (int k = lane; k < n; k += 32) out[o + k] = tag[nlist[(int64_t)i * pitch + k]];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ TileShared s;
+    int *gidx = reinterpret_cast<int *>(smem_raw);
+    TileCtx t;
+    tile_decode(g, blockIdx.x, t);
+    if (!tile_tables(g, cell_start, t, s, flags)) return;
+    for (int sl = 1 + threadIdx.x; sl < t.nslots; sl += TILE_THREADS) {
+        const int h = tile_cell_of_slot(t, s, sl);
+        gidx[sl] = s.hg[h] + (sl - s.hslot[h]);
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int q = warp; q < t.nown; q += TILE_THREADS / 32) {
+        const int r = tile_row_of(t, s, q);
+        const int gi = s.own_start[r] + (q - s.own_off[r]);
+        const int n = nlistn[gi];
+        const int64_t o = row_start[tag[gi]];
+        const uint16_t *row = nlist + (int64_t)gi * pitch;
+        for (int k = lane; k < n; k += 32) out[o + k] = tag[gidx[row[k]]];
+    }
 }
 
 cudaError_t launch_nlist_counts_by_tag(hb_system *h, int *counts)
@@ -231,7 +262,10 @@ cudaError_t launch_nlist_counts_by_tag(hb_system *h, int *counts)
 
 cudaError_t launch_nlist_fill_by_tag(hb_system *h, const int64_t *row_start, uint32_t *out)
 {
-    nlist_fill_by_tag_kernel<<<(unsigned)cdiv(h->N, 8), 256, 0, h->stream>>>(h->nlist, h->nlistn, h->row_pitch, h->tag,
-                                                                             (int)h->N, row_start, out);
+    const size_t smem = (size_t)h->geom.cap * 4;
+    cudaError_t e = cudaFuncSetAttribute(nlist_fill_by_tag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    nlist_fill_by_tag_kernel<<<(unsigned)h->geom.ntiles, TILE_THREADS, smem, h->stream>>>(
+        h->geom, h->cell_start, h->nlist, h->nlistn, h->row_pitch, h->tag, row_start, out, h->flags);
     return cudaGetLastError();
 }

@@ -3,32 +3,29 @@
 // thermodynamic reduction and the state pack/unpack kernels.
 #include "hb_internal.cuh"
 
-// One kernel covers the three places an integrator kernel is needed:
-//   KICK_PREV  : v += (dt/2) F   -- second half of the previous step (reading c7)
-//   KICK_DRIFT : v += (dt/2) F;  x += dt v;  wrap into [-L/2, L/2) with image +-1;
-//                set FL_NEED_BUILD if |minimage(x - x_build)| > r_buff / 2
-// Inside hb_run_nve both are fused (one read of F, one read/write of v per step);
-// the arithmetic, operation by operation, is the same as two separate launches.
-// With use_cond the last block to finish hands the rebuild decision to the CUDA
-// graph's conditional node, so the host never sees it.
-template <bool KICK_PREV, bool KICK_DRIFT>
+// The stand-alone integrator kernel (hb_step_nve, the first drift of a run, fuse_nve = 0):
+//   kick_prev  : v += (dt/2) F   -- second half of the previous step (reading c7)
+//   kick_drift : v += (dt/2) F;  x += dt v;  wrap into [-L/2, L/2) with image +-1;
+//                set the drift's FL_NEED flag if |minimage(x - x_build)| > r_buff / 2
+// Inside hb_run_nve the same arithmetic, operation by operation, runs at the end of the
+// force kernel (force.cu).  With use_cond the last block to finish hands the rebuild
+// decision to the CUDA graph's conditional node, so the host never sees it.
 __global__ void __launch_bounds__(256)
-nve_kernel(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__restrict__ force, int *__restrict__ image,
-           const float4 *__restrict__ pos_build, int N, float L, float dt, float half_buff2, int *__restrict__ flags,
-           cudaGraphConditionalHandle cond, int use_cond)
+nve_kernel(float4 *pos, const float4 *__restrict__ force, int N, float L, int *__restrict__ flags, NveArgs nv)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const float hdt = 0.5f * dt, hL = 0.5f * L;
+    const float hdt = 0.5f * nv.dt, hL = 0.5f * L, dt = nv.dt;
     bool exceed = false;
+    if (nv.kick_drift && i == 0) flags[nv.need_clear] = 0;
     if (i < N) {
-        float4 v = vel[i];
+        float4 v = nv.vel[i];
         const float4 f = force[i];
-        if (KICK_PREV) {
+        if (nv.kick_prev) {
             v.x = __fmaf_rn(hdt, f.x, v.x);
             v.y = __fmaf_rn(hdt, f.y, v.y);
             v.z = __fmaf_rn(hdt, f.z, v.z);
         }
-        if (KICK_DRIFT) {
+        if (nv.kick_drift) {
             v.x = __fmaf_rn(hdt, f.x, v.x);
             v.y = __fmaf_rn(hdt, f.y, v.y);
             v.z = __fmaf_rn(hdt, f.z, v.z);
@@ -36,30 +33,31 @@ nve_kernel(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__r
             p.x = __fmaf_rn(dt, v.x, p.x);
             p.y = __fmaf_rn(dt, v.y, p.y);
             p.z = __fmaf_rn(dt, v.z, p.z);
-            if (p.x >= hL) { p.x -= L; image[i] += 1; } else if (p.x < -hL) { p.x += L; image[i] -= 1; }
-            if (p.y >= hL) { p.y -= L; image[N + i] += 1; } else if (p.y < -hL) { p.y += L; image[N + i] -= 1; }
-            if (p.z >= hL) { p.z -= L; image[2 * N + i] += 1; } else if (p.z < -hL) { p.z += L; image[2 * N + i] -= 1; }
-            pos[i] = p;
-            const float4 pb = pos_build[i];
+            if (p.x >= hL) { p.x -= L; nv.image[i] += 1; } else if (p.x < -hL) { p.x += L; nv.image[i] -= 1; }
+            if (p.y >= hL) { p.y -= L; nv.image[N + i] += 1; } else if (p.y < -hL) { p.y += L; nv.image[N + i] -= 1; }
+            if (p.z >= hL) { p.z -= L; nv.image[2 * (int64_t)N + i] += 1; }
+            else if (p.z < -hL) { p.z += L; nv.image[2 * (int64_t)N + i] -= 1; }
+            nv.pos_out[i] = p;
+            const float4 pb = nv.pos_build[i];
             float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
             if (dx >= hL) dx -= L; else if (dx < -hL) dx += L;
             if (dy >= hL) dy -= L; else if (dy < -hL) dy += L;
             if (dz >= hL) dz -= L; else if (dz < -hL) dz += L;
-            exceed = (dx * dx + dy * dy + dz * dz) > half_buff2;
+            exceed = (dx * dx + dy * dy + dz * dz) > nv.half_buff2;
         }
-        vel[i] = v;
+        nv.vel[i] = v;
     }
-    if (KICK_DRIFT) {
-        if (__any_sync(0xffffffffu, exceed) && (threadIdx.x & 31) == 0) flags[FL_NEED_BUILD] = 1;
-        if (use_cond) {
+    if (nv.kick_drift) {
+        if (__any_sync(0xffffffffu, exceed) && (threadIdx.x & 31) == 0) flags[nv.need_set] = 1;
+        if (nv.use_cond) {
             __syncthreads();
             if (threadIdx.x == 0) {
                 __threadfence();
                 const int ticket = atomicAdd(&flags[FL_DONE_CTR], 1);
                 if (ticket == (int)gridDim.x - 1) {
                     __threadfence();
-                    const int need = *((volatile int *)&flags[FL_NEED_BUILD]);
-                    cudaGraphSetConditional(cond, need ? 1u : 0u);
+                    const int need = *((volatile int *)&flags[nv.need_set]);
+                    cudaGraphSetConditional(nv.cond, need ? 1u : 0u);
                     flags[FL_DONE_CTR] = 0;
                 }
             }
@@ -67,17 +65,37 @@ nve_kernel(float4 *__restrict__ pos, float4 *__restrict__ vel, const float4 *__r
     }
 }
 
-cudaError_t launch_nve(hb_system *h, float dt, bool kick_prev, bool kick_drift, cudaGraphConditionalHandle cond, bool use_cond)
+cudaError_t launch_nve(hb_system *h, const NveArgs &a)
 {
     const unsigned grid = (unsigned)cdiv(h->N, 256);
-    const float hb = 0.5f * h->r_buff;
-    const float half_buff2 = hb * hb;
-#define NVE_ARGS h->pos, h->vel, h->force, h->image, h->pos_build, (int)h->N, h->L, dt, half_buff2, h->flags, cond, use_cond ? 1 : 0
-    if (kick_prev && kick_drift) nve_kernel<true, true><<<grid, 256, 0, h->stream>>>(NVE_ARGS);
-    else if (kick_drift) nve_kernel<false, true><<<grid, 256, 0, h->stream>>>(NVE_ARGS);
-    else nve_kernel<true, false><<<grid, 256, 0, h->stream>>>(NVE_ARGS);
-#undef NVE_ARGS
+    nve_kernel<<<grid, 256, 0, h->stream>>>(h->pos(), h->force, (int)h->N, h->L, h->flags, a);
     h->stats.kernel_launches++;
+    return cudaGetLastError();
+}
+
+// Reading c3 on demand (hb_needs_rebuild): has any particle moved more than r_buff/2 since the build?
+__global__ void __launch_bounds__(256)
+disp_check_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ pos_build, int N, float L, float half_buff2,
+                  int *__restrict__ flags)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const float hL = 0.5f * L;
+    bool exceed = false;
+    if (i < N) {
+        const float4 p = pos[i], pb = pos_build[i];
+        float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
+        if (dx >= hL) dx -= L; else if (dx < -hL) dx += L;
+        if (dy >= hL) dy -= L; else if (dy < -hL) dy += L;
+        if (dz >= hL) dz -= L; else if (dz < -hL) dz += L;
+        exceed = (dx * dx + dy * dy + dz * dz) > half_buff2;
+    }
+    if (__any_sync(0xffffffffu, exceed) && (threadIdx.x & 31) == 0) flags[FL_CHECK] = 1;
+}
+
+cudaError_t launch_disp_check(hb_system *h)
+{
+    const float hb = 0.5f * h->r_buff;
+    disp_check_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->pos(), h->pos_build, (int)h->N, h->L, hb * hb, h->flags);
     return cudaGetLastError();
 }
 
@@ -168,14 +186,14 @@ __global__ void unpack_state_kernel(const float4 *__restrict__ pos, const float4
 
 cudaError_t launch_pack_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz, const int32_t *image)
 {
-    pack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(pos_xyz, type, vel_xyz, image, (int)h->N, h->pos, h->vel,
+    pack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(pos_xyz, type, vel_xyz, image, (int)h->N, h->pos(), h->vel,
                                                                         h->image, h->tag, h->rtag);
     return cudaGetLastError();
 }
 
 cudaError_t launch_unpack_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image)
 {
-    unpack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->pos, h->vel, h->image, h->tag, (int)h->N, pos_xyz,
+    unpack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->pos(), h->vel, h->image, h->tag, (int)h->N, pos_xyz,
                                                                           type, vel_xyz, image);
     return cudaGetLastError();
 }

@@ -1,12 +1,14 @@
 // Space-filling-curve particle sort (the paper's "SFCPACK sort"),
 // on the GPU -- the paper still ran it on the host and called it "a serial
 // bottleneck".  Reading c8: Hilbert curve (Skilling's transpose algorithm) on a
-// 2^8 grid per axis, stable in the current index.
+// 2^8 grid per axis, ties in tag order (the key pass walks the particles by tag,
+// the radix sort is stable), so the result does not depend on the storage order.
 //   keys   : one thread per particle
 //   sort   : hand-written LSD radix sort of (key, index), 8 bits per pass; a warp
 //            owns a tile of 32 x RS_ITEMS keys; __match_any_sync gives each key its
 //            stable rank among equal digits
-//   gather : every per-particle array permuted into the second buffer set
+//   gather : every per-particle array permuted into the scratch set (positions into pos_build,
+//            which the next list build overwrites anyway)
 #include "hb_internal.cuh"
 
 constexpr int SFC_BITS = 8;
@@ -48,21 +50,22 @@ __device__ __forceinline__ uint32_t grid_coord(float x, float b, float s)
     return (uint32_t)min(max(g, 0), G - 1);
 }
 
-__global__ void sfc_keys_kernel(const float4 *__restrict__ pos, int N, float b, float s, uint32_t *__restrict__ keys,
-                                uint32_t *__restrict__ perm)
+__global__ void sfc_keys_kernel(const float4 *__restrict__ pos, const uint32_t *__restrict__ rtag, int N, float b, float s,
+                                uint32_t *__restrict__ keys, uint32_t *__restrict__ perm)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;   // tag
+    if (t >= N) return;
+    const uint32_t i = rtag[t];
     const float4 p = pos[i];
-    keys[i] = hilbert_key(grid_coord(p.x, b, s), grid_coord(p.y, b, s), grid_coord(p.z, b, s));
-    perm[i] = i;
+    keys[t] = hilbert_key(grid_coord(p.x, b, s), grid_coord(p.y, b, s), grid_coord(p.z, b, s));
+    perm[t] = i;
 }
 
 cudaError_t launch_sfc_keys(hb_system *h)
 {
     const float b = -0.5f * h->L;
     const float s = (float)(1 << SFC_BITS) / h->L;
-    sfc_keys_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->pos, (int)h->N, b, s, h->keys, h->perm);
+    sfc_keys_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->pos(), h->rtag, (int)h->N, b, s, h->keys, h->sperm);
     h->stats.kernel_launches++;
     return cudaGetLastError();
 }
@@ -131,13 +134,13 @@ cudaError_t launch_radix_sort(hb_system *h, int key_bits)
     const int N = (int)h->N;
     const int ntiles = (int)cdiv(N, RS_TILE);
     const unsigned grid = (unsigned)cdiv(ntiles, RS_WARPS);
-    uint32_t *kin = h->keys, *kout = h->keys2, *vin = h->perm, *vout = h->perm2;
+    uint32_t *kin = h->keys, *kout = h->keys2, *vin = h->sperm, *vout = h->sperm2;
     for (int shift = 0; shift < key_bits; shift += 8) {
         radix_hist_kernel<<<grid, RS_WARPS * 32, 0, h->stream>>>(kin, N, shift, ntiles, h->radix_counts);
         h->stats.kernel_launches++;
         // in-place exclusive scan over the 256 x ntiles counts (out[n] lands in the spare slot)
         cudaError_t e = launch_scan_exclusive(h, h->radix_counts, h->radix_counts + h->radix_counts_len,
-                                              (int64_t)256 * ntiles, h->scan_tmp, nullptr);
+                                              (int64_t)256 * ntiles, h->scan_tmp);
         if (e != cudaSuccess) return e;
         radix_scatter_kernel<<<grid, RS_WARPS * 32, 0, h->stream>>>(kin, vin, N, shift, ntiles,
                                                                     h->radix_counts + h->radix_counts_len, kout, vout);
@@ -148,7 +151,7 @@ cudaError_t launch_radix_sort(hb_system *h, int key_bits)
     // an odd number of passes leaves the result in the second buffers
     if (kin != h->keys) {
         uint32_t *t = h->keys; h->keys = h->keys2; h->keys2 = t;
-        t = h->perm; h->perm = h->perm2; h->perm2 = t;
+        t = h->sperm; h->sperm = h->sperm2; h->sperm2 = t;
     }
     return cudaGetLastError();
 }
@@ -179,9 +182,22 @@ __global__ void gather_state_kernel(const uint32_t *__restrict__ perm, int N, co
 
 cudaError_t launch_gather_state(hb_system *h)
 {
-    gather_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->perm, (int)h->N, h->pos, h->vel, h->force, h->virial,
-                                                                          h->image, h->tag, h->pos2, h->vel2, h->force2,
+    gather_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->sperm, (int)h->N, h->pos(), h->vel, h->force, h->virial,
+                                                                          h->image, h->tag, h->pos_build, h->vel2, h->force2,
                                                                           h->virial2, h->image2, h->tag2, h->rtag);
     h->stats.kernel_launches++;
+    return cudaGetLastError();
+}
+
+// tag -> storage slot, recomputed from the tag array (after a restore)
+__global__ void rtag_kernel(const uint32_t *__restrict__ tag, int N, uint32_t *__restrict__ rtag)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) rtag[tag[i]] = i;
+}
+
+cudaError_t launch_rtag(hb_system *h)
+{
+    rtag_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->tag, (int)h->N, h->rtag);
     return cudaGetLastError();
 }

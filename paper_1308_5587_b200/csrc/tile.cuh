@@ -1,0 +1,190 @@
+// Tile staging shared by the list build (nlist.cu), the force kernel (force.cu)
+// and the list accessor: the SAME function lays the halo of a tile out in shared
+// memory in all three, so a shared-memory slot number written into the list by
+// the build means the same particle to the force kernel.
+//
+// The paper's first GPU list kernel staged neighbor cells in shared memory with one
+// block per cell and was dropped because cell occupancies vary too much for 16 KB
+// (PAPER.md:177); its successor reads neighbors through the cache and names the
+// scattered traffic the bottleneck.  With 227 KB per SM the
+// capacity objection is gone: a block owns a brick of cells, stages the brick
+// plus a one-cell halo ONCE with coalesced reads (the particle data is kept in
+// cell order, so x-adjacent cells are one contiguous run), applies the periodic
+// shift while staging (no minimum-image arithmetic is left in any inner loop),
+// and every later gather is a shared-memory access.
+//
+// Layout: halo cell h = jx + hx (jy + hy jz), jx in [0, ex + 2) etc.; slots are
+// handed out in h order, slot 0 is a dummy particle far away from everything, so
+// list rows can be padded with 0 and need no bounds test in the force loop.
+#pragma once
+#include "hb_internal.cuh"
+
+struct TileCtx {
+    int x0, y0, z0;   // first own cell
+    int ex, ey, ez;   // own extent in cells (clipped tile)
+    int hx, hy, hz;   // halo box = extent + 2
+    int nh;           // halo cells
+    int nslots;       // 1 + staged particles
+    int nown;         // own particles
+    int nrows;        // own (y, z) rows = ey * ez
+};
+
+struct TileShared {
+    int hslot[TILE_HMAX + 1];   // first slot of halo cell h
+    int hg[TILE_HMAX];          // storage index of the first particle of halo cell h
+    int own_start[TILE_ROWS_MAX];    // storage index of the first own particle of row r
+    int own_off[TILE_ROWS_MAX + 1];  // tile-local number of the first own particle of row r
+    int own_slot[TILE_ROWS_MAX];     // its slot
+};
+
+__device__ __forceinline__ void tile_decode(const TileGeom &g, int tile, TileCtx &t)
+{
+    const int tix = tile % g.ntx, tiy = (tile / g.ntx) % g.nty, tiz = tile / (g.ntx * g.nty);
+    t.x0 = tix * g.tx; t.y0 = tiy * g.ty; t.z0 = tiz * g.tz;
+    t.ex = min(g.tx, g.m - t.x0); t.ey = min(g.ty, g.m - t.y0); t.ez = min(g.tz, g.m - t.z0);
+    t.hx = t.ex + 2; t.hy = t.ey + 2; t.hz = t.ez + 2;
+    t.nh = t.hx * t.hy * t.hz;
+    t.nrows = t.ey * t.ez;
+}
+
+// wrap a halo cell coordinate into the box; shift = what to add to a coordinate of that cell's particles
+__device__ __forceinline__ int tile_wrap(int c, int m, float L, float &shift)
+{
+    shift = 0.f;
+    if (c < 0) { c += m; shift = -L; }
+    else if (c >= m) { c -= m; shift = L; }
+    return c;
+}
+
+// Halo table, slot prefix, own-row table.  Returns false (for the whole block) when the tile
+// needs more slots than g.cap; FL_STAGE_OVER then carries the number needed.
+__device__ __forceinline__ bool tile_tables(const TileGeom &g, const int *__restrict__ cell_start, TileCtx &t, TileShared &s,
+                                            int *__restrict__ flags)
+{
+    const int tid = threadIdx.x, lane = tid & 31;
+    for (int h = tid; h < t.nh; h += blockDim.x) {
+        const int jx = h % t.hx, jy = (h / t.hx) % t.hy, jz = h / (t.hx * t.hy);
+        float dummy;
+        const int cx = tile_wrap(t.x0 - 1 + jx, g.m, g.L, dummy);
+        const int cy = tile_wrap(t.y0 - 1 + jy, g.m, g.L, dummy);
+        const int cz = tile_wrap(t.z0 - 1 + jz, g.m, g.L, dummy);
+        const int c = cx + g.m * (cy + g.m * cz);
+        const int s0 = cell_start[c];
+        s.hg[h] = s0;
+        s.hslot[h] = cell_start[c + 1] - s0;
+    }
+    __syncthreads();
+    if (tid < 32) {  // exclusive scan of up to 256 counts: 8 per lane
+        const int base = lane * 8;
+        int v[8], tsum = 0;
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            v[q] = (base + q < t.nh) ? s.hslot[base + q] : 0;
+            tsum += v[q];
+        }
+        int incl = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += y;
+        }
+        int run = 1 + incl - tsum;  // slot 0 is the dummy
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            if (base + q < t.nh) s.hslot[base + q] = run;
+            run += v[q];
+        }
+        if (lane == 31) s.hslot[t.nh] = run;
+    }
+    __syncthreads();
+    t.nslots = s.hslot[t.nh];
+    if (tid < t.nrows) {
+        const int ly = tid % t.ey, lz = tid / t.ey;
+        const int hrow = ((lz + 1) * t.hy + (ly + 1)) * t.hx;
+        const int first = hrow + 1, last = hrow + t.ex;
+        s.own_start[tid] = s.hg[first];
+        s.own_slot[tid] = s.hslot[first];
+        s.own_off[tid + 1] = s.hslot[last + 1] - s.hslot[first];   // own cells of a row are consecutive halo cells
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int run = 0;
+        s.own_off[0] = 0;
+        for (int r = 0; r < t.nrows; r++) { const int n = s.own_off[r + 1]; s.own_off[r + 1] = run + n; run += n; }
+    }
+    __syncthreads();
+    t.nown = s.own_off[t.nrows];
+    if (t.nslots > g.cap) {
+        if (tid == 0) atomicMax(&flags[FL_STAGE_OVER], t.nslots);
+        return false;
+    }
+    return true;
+}
+
+// halo cell of slot sl: the largest h with hslot[h] <= sl
+__device__ __forceinline__ int tile_cell_of_slot(const TileCtx &t, const TileShared &s, int sl)
+{
+    int h = 0;
+#pragma unroll
+    for (int st = TILE_HMAX / 2; st > 0; st >>= 1)
+        if (h + st < t.nh && s.hslot[h + st] <= sl) h += st;
+    return h;
+}
+
+// image of coordinate x nearest to the centre cc of the (possibly out-of-box) halo cell it belongs to
+__device__ __forceinline__ float tile_image(float x, float cc, float L, float hL)
+{
+    const float d = x - cc;
+    if (d > hL) x -= L;
+    else if (d < -hL) x += L;
+    return x;
+}
+
+// Positions of all halo cells into stage[1 .. nslots), each moved to the periodic image that lies in
+// the halo cell as this tile sees it (a cell left of the box for the tile at x0 = 0, and so on);
+// stage[0] = dummy.  The image is chosen from the POSITION, relative to the centre of the halo cell
+// in the tile's frame, not from the cell index alone: between two builds a particle near a face of
+// the box may have been wrapped to the other side, and must still be seen next to its neighbors.
+// At build time (particles inside their cells) this adds exactly -L, 0 or +L per axis.
+__device__ __forceinline__ void tile_stage_positions(const TileGeom &g, const TileCtx &t, const TileShared &s,
+                                                     const float4 *__restrict__ pos, float4 *__restrict__ stage)
+{
+    constexpr int U = 4;
+    const int nt = blockDim.x;
+    const float wcell = g.L / (float)g.m, hL = 0.5f * g.L;
+    if (threadIdx.x == 0) stage[0] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+    for (int s0 = 1 + threadIdx.x; s0 < t.nslots; s0 += U * nt) {
+        int src[U];
+        float cx[U], cy[U], cz[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int sl = s0 + u * nt;
+            src[u] = -1;
+            if (sl < t.nslots) {
+                const int h = tile_cell_of_slot(t, s, sl);
+                src[u] = s.hg[h] + (sl - s.hslot[h]);
+                const int jx = h % t.hx, jy = (h / t.hx) % t.hy, jz = h / (t.hx * t.hy);
+                cx[u] = __fmaf_rn((float)(t.x0 - 1 + jx) + 0.5f, wcell, -hL);
+                cy[u] = __fmaf_rn((float)(t.y0 - 1 + jy) + 0.5f, wcell, -hL);
+                cz[u] = __fmaf_rn((float)(t.z0 - 1 + jz) + 0.5f, wcell, -hL);
+            }
+        }
+        float4 p[U];
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            if (src[u] >= 0) p[u] = pos[src[u]];
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            if (src[u] >= 0)
+                stage[s0 + u * nt] = make_float4(tile_image(p[u].x, cx[u], g.L, hL), tile_image(p[u].y, cy[u], g.L, hL),
+                                                 tile_image(p[u].z, cz[u], g.L, hL), p[u].w);
+    }
+}
+
+// tile-local own particle q -> own row r (rows are few: linear scan)
+__device__ __forceinline__ int tile_row_of(const TileCtx &t, const TileShared &s, int q)
+{
+    int r = 0;
+    while (r + 1 < t.nrows && s.own_off[r + 1] <= q) r++;
+    return r;
+}

@@ -35,6 +35,20 @@ __device__ __forceinline__ float rcp_approx(float x)
     return y;
 }
 
+// cp.async (LDGSTS): global -> shared without a register or a scoreboard slot in between.  ncu of the
+// register-prefetch version showed 40 % of the warp time in long-scoreboard stalls at the first use of
+// a list entry however far ahead it was loaded: scoreboard slots count, so a consumer waits for every
+// later load on its slot too.  Async-copy groups are tracked separately.
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void *smem_dst, const void *gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(d), "l"(gsrc), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 struct Acc {
     float fx, fy, fz, u, wxx, wxy, wxz, wyy, wyz, wzz;
 };
@@ -76,68 +90,107 @@ __device__ __forceinline__ void unpack_entries(const Entries<EPL> &e, int (&sl)[
 }
 
 template <int TPP, int EPL, bool ONE_TYPE>
-__global__ void __launch_bounds__(TILE_THREADS)
+__global__ void __launch_bounds__(TILE_THREADS, 4)   // <= 64 registers: 8 blocks of 128 threads per SM
 lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__restrict__ pos,
                const uint16_t *__restrict__ nlist, const int *__restrict__ nlistn, int pitch, int N, int ntypes,
                const PairParam *__restrict__ params, float4 *__restrict__ force, float4 *__restrict__ virial,
-               int *__restrict__ flags, int do_nve, NveArgs nv)
+               int *__restrict__ flags, int do_nve, NveArgs nv, const int *__restrict__ stage_src,
+               const TileDesc *__restrict__ desc)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ TileShared s;
     float4 *stage = reinterpret_cast<float4 *>(smem_raw);
     PairParam *s_params = reinterpret_cast<PairParam *>(smem_raw + (size_t)g.cap * 16);
     constexpr int G = TPP * EPL;                 // entries per particle per iteration
-    constexpr int PPB = TILE_THREADS / TPP;      // particles per block per pass
 
     if (!ONE_TYPE)
-        for (int k = threadIdx.x; k < ntypes * ntypes; k += TILE_THREADS) s_params[k] = params[k];
+        for (int k = threadIdx.x; k < ntypes * ntypes; k += blockDim.x) s_params[k] = params[k];
     if (do_nve && nv.kick_drift && blockIdx.x == 0 && threadIdx.x == 0) flags[nv.need_clear] = 0;
 
-    TileCtx t;
-    tile_decode(g, blockIdx.x, t);
-    const bool fits = tile_tables(g, cell_start, t, s, flags);
-    if (fits) tile_stage_positions(g, t, s, pos, stage);
+    const int sub = threadIdx.x % TPP;
+    const int PPB = blockDim.x / TPP;            // particles per block per pass
+    // List rows reach the threads through a ring of PF async copies per thread: entry group k of the
+    // row is copied PF iterations before it is used.  A row ends at its first padding entry (slot 0;
+    // the build pads every row with at least 32 of them), so the row length is never loaded.
+    constexpr int PF = 4;
+    using EntryVec = decltype(Entries<EPL>::v);
+    EntryVec *ring = reinterpret_cast<EntryVec *>(smem_raw + (size_t)g.cap * 16 +
+                                                  (ONE_TYPE ? 0 : ((ntypes * ntypes * sizeof(PairParam) + 15) & ~(size_t)15))) +
+                     threadIdx.x;
+    const int ring_stride = blockDim.x;
+    int gi_n = 0, slot_n = 0;
+    bool active_n = false;
+    // particle of pass q0 for this thread group; start the copies of its first PF entry groups
+    auto prep = [&](int q0, int nown) {
+        const int q = q0 + threadIdx.x / TPP;
+        active_n = q < nown;
+        gi_n = 0; slot_n = 0;
+        if (active_n) tile_own(s.d, q, gi_n, slot_n);
+        const uint16_t *row = nlist + (int64_t)gi_n * pitch + sub * EPL;
+#pragma unroll
+        for (int u = 0; u < PF; u++) {
+            if (active_n) cp_async<EPL * 2>(ring + u * ring_stride, row + u * G);
+            cp_async_commit();
+        }
+    };
+
+    bool fits;
+    if (g.fast) {
+        // the list build left this tile's descriptor and the storage index of every slot behind
+        if (threadIdx.x < sizeof(TileDesc) / 4)
+            reinterpret_cast<int *>(&s.d)[threadIdx.x] = __ldg(reinterpret_cast<const int *>(desc + blockIdx.x) + threadIdx.x);
+        __syncthreads();
+        fits = s.d.nslots <= g.cap;
+        prep(0, fits ? s.d.nown : 0);            // list copies in flight while the tile is staged
+        if (fits) tile_stage_from_table(s.d, stage_src + (int64_t)blockIdx.x * g.cap, pos, stage, g.L);
+    } else {
+        TileCtx t;
+        tile_decode(g, blockIdx.x, t);
+        fits = tile_tables(g, cell_start, t, s, flags);
+        prep(0, fits ? s.d.nown : 0);
+        if (fits) tile_stage_positions(g, t, s, pos, stage, nullptr);
+    }
     __syncthreads();
 
-    const int sub = threadIdx.x % TPP;
     const PairParam pp1 = params[0];
     const float hdt = 0.5f * nv.dt, hL = 0.5f * g.L, L = g.L;
     bool exceed = false;
 
-    const int nown = fits ? t.nown : 0;
+    const int nown = fits ? s.d.nown : 0;
     for (int q0 = 0; q0 < nown; q0 += PPB) {     // block-uniform trip count: the shuffles need whole warps
-        const int q = q0 + threadIdx.x / TPP;
-        const bool active = q < nown;
-        int gi = 0, n = 0;
-        float4 pi = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (active) {
-            const int r = tile_row_of(t, s, q);
-            const int off = q - s.own_off[r];
-            gi = s.own_start[r] + off;
-            pi = stage[s.own_slot[r] + off];
-            n = nlistn[gi];
-        }
+        const bool active = active_n;
+        const int gi = gi_n;
+        const float4 pi = stage[slot_n];         // slot 0 (the dummy) for idle thread groups
         const uint16_t *row = nlist + (int64_t)gi * pitch + sub * EPL;
         const PairParam *prow = ONE_TYPE ? nullptr : s_params + __float_as_int(pi.w) * ntypes;
         Acc a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
-        Entries<EPL> cur{};
-        if (n > 0) cur = load_entries<EPL>(row);
-        for (int k = 0; k < n; k += G) {
-            Entries<EPL> nxt{};
-            if (k + G < n) nxt = load_entries<EPL>(row + k + G);   // one iteration ahead
-            int sl[EPL];
-            unpack_entries<EPL>(cur, sl);
-            float4 pj[EPL];
+        if (active) {
+            int c = 0;
+            cp_async_wait<PF - 1>();
+            Entries<EPL> ent;
+            ent.v = ring[0];
+            for (int k = 0; k < pitch; k += G) {
+                if ((ent.v.x & 0xffffu) == 0u) break;                    // padding: the row is over for this thread
+                cp_async<EPL * 2>(ring + c * ring_stride, row + k + PF * G);   // refill PF iterations ahead (reads past the
+                cp_async_commit();                                       // row's end are harmless: the array has slack)
+                c = (c + 1 == PF) ? 0 : c + 1;
+                int sl[EPL];
+                unpack_entries<EPL>(ent, sl);
+                float4 pj[EPL];
 #pragma unroll
-            for (int e = 0; e < EPL; e++) pj[e] = stage[sl[e]];
+                for (int e = 0; e < EPL; e++) pj[e] = stage[sl[e]];
+                cp_async_wait<PF - 1>();                                 // the next group of entries, read before the
+                ent.v = ring[c * ring_stride];                           // arithmetic so that its latency hides behind it
 #pragma unroll
-            for (int e = 0; e < EPL; e++) {
-                if (ONE_TYPE) pair_term(pi, pj[e], pp1, a);
-                else pair_term(pi, pj[e], prow[__float_as_int(pj[e].w)], a);
+                for (int e = 0; e < EPL; e++) {
+                    if (ONE_TYPE) pair_term(pi, pj[e], pp1, a);
+                    else pair_term(pi, pj[e], prow[__float_as_int(pj[e].w)], a);
+                }
             }
-            cur = nxt;
         }
+        cp_async_wait<0>();                          // nothing of this pass may land after the next pass's copies start
+        if (q0 + PPB < nown) prep(q0 + PPB, nown);   // they fly during the reduction and the integration below
 
 #pragma unroll
         for (int o = TPP >> 1; o > 0; o >>= 1) {
@@ -217,7 +270,9 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
 
 size_t force_smem_bytes(const hb_system *h)
 {
-    return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? sizeof(PairParam) * h->ntypes * h->ntypes : 0);
+    // staged positions, pair table, ring of 4 async list copies (16 B at most) per thread
+    return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? ((sizeof(PairParam) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
+           (size_t)4 * 16 * h->tun.force_block;
 }
 
 template <int TPP, int EPL>
@@ -231,10 +286,11 @@ static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
 #define LJ_LAUNCH(ONE)                                                                                                      \
     e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
     if (e != cudaSuccess) return e;                                                                                         \
-    lj_tile_kernel<TPP, EPL, ONE><<<grid, TILE_THREADS, smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
+    lj_tile_kernel<TPP, EPL, ONE><<<grid, h->tun.force_block, smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
                                                                            h->nlistn, h->row_pitch, (int)h->N, h->ntypes,  \
                                                                            h->params, h->force, h->virial, h->flags,       \
-                                                                           nve ? 1 : 0, nv);
+                                                                           nve ? 1 : 0, nv, h->stage_src,                  \
+                                                                           (const TileDesc *)h->tile_desc);
     if (h->ntypes == 1) { LJ_LAUNCH(true) } else { LJ_LAUNCH(false) }
 #undef LJ_LAUNCH
     h->stats.kernel_launches++;

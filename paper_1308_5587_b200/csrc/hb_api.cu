@@ -135,6 +135,30 @@ int choose_tiles(hb_system *h, int min_cap)
         cap = stage_cap_max(h);
     }
     g.cap = cap;
+    // fast geometry: tile + halo + what a particle can drift between builds is narrower than L/2 on every axis,
+    // so the periodic image nearest to the tile centre is the right one for every staged particle
+    {
+        const double w = (double)h->L / m;
+        const int tmax = std::max(tx, std::max(ty, tz));
+        g.fast = ((0.5 * tmax + 1.0) * w + 2.0 * (double)h->r_buff + 0.05 * w < 0.5 * (double)h->L) ? 1 : 0;
+    }
+    if (g.fast) {
+        const int64_t need_src = (int64_t)g.ntiles * g.cap;
+        if (need_src > h->stage_src_len) {
+            dev_free_t(h, h->stage_src);
+            HB_TRY(dev_alloc_t(h, &h->stage_src, (size_t)need_src));
+            h->stage_src_len = need_src;
+            destroy_graphs(h);
+        }
+        const int64_t need_desc = (int64_t)g.ntiles * 416;   // sizeof(TileDesc), tile.cuh
+        if (need_desc > h->tile_desc_len) {
+            dev_free(h, h->tile_desc);
+            h->tile_desc = nullptr;
+            HB_TRY(dev_alloc(h, &h->tile_desc, (size_t)need_desc));
+            h->tile_desc_len = need_desc;
+            destroy_graphs(h);
+        }
+    }
     if (memcmp(&g, &h->geom, sizeof g) != 0) {
         destroy_graphs(h);
         h->nlist_valid = false;
@@ -184,7 +208,7 @@ int configure_geometry(hb_system *h)
 int ensure_rows(hb_system *h, int pitch)
 {
     pitch = round_up(pitch < 64 ? 64 : pitch, 64);   // 16-bit entries: 64 = 128 B
-    const int64_t need = h->N * (int64_t)pitch;
+    const int64_t need = h->N * (int64_t)pitch + 1024;   // slack: the force kernel's list prefetch runs past a row's end
     if (need > h->nlist_alloc) {
         dev_free_t(h, h->nlist);
         HB_TRY(dev_alloc_t(h, &h->nlist, (size_t)need));
@@ -683,7 +707,7 @@ int hb_destroy(hb_system *h)
     void *ptrs[] = {h->posbuf[0], h->posbuf[1], h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->vel2,
                     h->force2, h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_image,
                     h->bk_tag, h->params, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
-                    h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
+                    h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->stage_src, h->tile_desc, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
                     h->flags, h->thermo_part};
     for (void *p : ptrs) dev_free(h, p);
     if (h->h_flags) cudaFreeHost(h->h_flags);
@@ -1011,16 +1035,41 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
         }
         return HB_OK;
     };
-    if (!flush_l2_bytes) cudaEventRecord(ev0[0], h->stream);
-    for (int r = 0; r < reps && rc == HB_OK; r++) {
-        if (flush_l2_bytes) {
+    cudaGraph_t tg = nullptr;
+    cudaGraphExec_t tge = nullptr;
+    if (flush_l2_bytes) {
+        for (int r = 0; r < reps && rc == HB_OK; r++) {
             cudaMemsetAsync(scratch, r & 0xff, (size_t)flush_l2_bytes, h->stream);
             cudaEventRecord(ev0[r], h->stream);
+            rc = launch();
+            cudaEventRecord(ev1[r], h->stream);
         }
-        rc = launch();
-        if (flush_l2_bytes) cudaEventRecord(ev1[r], h->stream);
+    } else {
+        // The reps launches go into ONE graph, so that the device runs them back to back: launched one by
+        // one from the host, a kernel shorter than the host's launch cost would be timed at the host's pace.
+        cudaStream_t cs = nullptr, saved = h->stream;
+        const int64_t saved_launches = h->stats.kernel_launches;
+        if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamBeginCapture(cs, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+            h->err = "hb_time_stage: cannot start a capture";
+            rc = HB_ECUDA;
+        } else {
+            h->stream = cs;
+            for (int r = 0; r < reps && rc == HB_OK; r++) rc = launch();
+            h->stream = saved;
+            cudaError_t ce = cudaStreamEndCapture(cs, &tg);
+            if (rc == HB_OK && ce == cudaSuccess) ce = cudaGraphInstantiate(&tge, tg, 0);
+            if (rc == HB_OK && ce != cudaSuccess) { h->err = std::string("hb_time_stage: ") + cudaGetErrorString(ce); rc = HB_ECUDA; }
+        }
+        h->stats.kernel_launches = saved_launches + (rc == HB_OK ? 2 * (h->stats.kernel_launches - saved_launches) : 0);
+        if (cs) cudaStreamDestroy(cs);
+        if (rc == HB_OK) {
+            cudaGraphLaunch(tge, h->stream);   // warm-up
+            cudaEventRecord(ev0[0], h->stream);
+            cudaGraphLaunch(tge, h->stream);
+            cudaEventRecord(ev1[0], h->stream);
+        }
     }
-    if (!flush_l2_bytes) cudaEventRecord(ev1[0], h->stream);
     cudaError_t e = cudaStreamSynchronize(h->stream);
     double total = 0.0;
     if (rc == HB_OK && e == cudaSuccess) {
@@ -1031,6 +1080,8 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
         rc = HB_ECUDA;
     }
     for (int k = 0; k < nev; k++) { cudaEventDestroy(ev0[k]); cudaEventDestroy(ev1[k]); }
+    if (tge) cudaGraphExecDestroy(tge);
+    if (tg) cudaGraphDestroy(tg);
     dev_free(h, scratch);
     if (rc == HB_OK) rc = clear_need_flags(h);
     if (rc == HB_OK && (which == 2 || which == 3)) {
@@ -1046,6 +1097,7 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!name) return nullptr;
     if (!strcmp(name, "tpp")) return &h->tun.tpp;
     if (!strcmp(name, "epl")) return &h->tun.epl;
+    if (!strcmp(name, "force_block")) return &h->tun.force_block;
     if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
     if (!strcmp(name, "tile_x")) return &h->tun.tile_x;
     if (!strcmp(name, "tile_y")) return &h->tun.tile_y;
@@ -1067,6 +1119,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     bool ok = true;
     if (slot == &h->tun.tpp) ok = value == 2 || value == 4 || value == 8;
     else if (slot == &h->tun.epl) ok = value == 4 || value == 8;
+    else if (slot == &h->tun.force_block) ok = value == 128 || value == 256;
     else if (slot == &h->tun.nlist_ppi) ok = value == 1 || value == 2 || value == 4;
     else if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z) ok = value >= 0 && value <= 16;
     else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;

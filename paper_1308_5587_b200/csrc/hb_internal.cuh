@@ -41,6 +41,7 @@ struct TileGeom {
     int ntx, nty, ntz;  // tiles per axis
     int ntiles;
     int cap;            // shared-memory slots (slot 0 is the far-away dummy)
+    int fast;           // 1: tile + halo narrower than L/2 on every axis (image by tile centre, tables from the build)
     float L;
 };
 
@@ -52,13 +53,14 @@ constexpr int ROW_PAD = 32;           // list rows are padded with dummy entries
 struct Tunables {
     int tpp = 4;           // threads per particle in the force kernel
     int epl = 4;           // list entries per thread per iteration (4 or 8)
+    int force_block = 128; // threads per block of the force kernel (128 or 256)
     int nlist_ppi = 4;     // particles tested per candidate load
     int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
     int stage_cap = 0;     // 0 = estimated from the density
     int row_pitch = 0;
     int cell_sort = 1;
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
-    int graph_mode = 2;
+    int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 50;
 };
 
@@ -113,6 +115,9 @@ struct hb_system {
 
     // neighbor list: row i = nlist[i * row_pitch .. + nlistn[i]), entries are shared-memory slots of i's tile
     TileGeom geom{};
+    int *stage_src = nullptr;    // [ntiles][cap] storage index of every staged slot (written by the list build)
+    void *tile_desc = nullptr;   // [ntiles] TileDesc (tile.cuh), written by the list build
+    int64_t stage_src_len = 0, tile_desc_len = 0;
     int row_pitch = 0;
     uint16_t *nlist = nullptr;
     int *nlistn = nullptr;

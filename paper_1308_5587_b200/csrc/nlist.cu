@@ -16,7 +16,7 @@
 //      the hits as bits of a register; one warp prefix sum of the per-lane __popc
 //      counts gives every lane its positions in the row and the lanes write their
 //      hits' SLOT NUMBERS (16 bit) straight into the row-major, 128-byte aligned
-//      list; the row is padded with slot 0 to a multiple of 32 entries.
+//      list; the row ends with at least 32 entries of slot 0 (the force kernel reads no row length).
 // List entries are slots of the tile's staging layout, not particle indices: the
 // force kernel stages the same tile the same way and gathers from shared memory
 // (hb_get_nlist translates back to tags).  Half the bytes of a 32-bit index list.
@@ -46,7 +46,7 @@ template <int PPI>
 __global__ void __launch_bounds__(TILE_THREADS)
 nlist_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__restrict__ pos_build, float rmax2,
                   int pitch, uint16_t *__restrict__ nlist, int *__restrict__ nlistn, int *__restrict__ flags,
-                  const int *__restrict__ pred, CopyBack cb)
+                  const int *__restrict__ pred, CopyBack cb, int *__restrict__ stage_src, TileDesc *__restrict__ desc)
 {
     if (pred && *pred == 0) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -63,8 +63,8 @@ nlist_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *
     // the reorder's last leg: own particles, scratch set -> live arrays (always, so the state stays whole)
     if (cb.pos) {
         for (int q = threadIdx.x; q < t.nown; q += TILE_THREADS) {
-            const int r = tile_row_of(t, s, q);
-            const int gi = s.own_start[r] + (q - s.own_off[r]);
+            int gi, slot;
+            tile_own(s.d, q, gi, slot);
             cb.pos[gi] = pos_build[gi];
             cb.vel[gi] = cb.vel2[gi];
             cb.image[gi] = cb.image2[gi];
@@ -75,8 +75,15 @@ nlist_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *
             cb.rtag[tg] = gi;
         }
     }
+    // what the force kernel will need every step: the tile's descriptor and the storage index of every slot
+    if (desc) {
+        if (!fits && threadIdx.x == 0) { s.d.nslots = 1; s.d.nown = 0; }   // nothing staged: the force kernel skips the tile
+        __syncthreads();
+        if (threadIdx.x < sizeof(TileDesc) / 4)
+            reinterpret_cast<int *>(desc + blockIdx.x)[threadIdx.x] = reinterpret_cast<const int *>(&s.d)[threadIdx.x];
+    }
     if (!fits) return;
-    tile_stage_positions(g, t, s, pos_build, stage);
+    tile_stage_positions(g, t, s, pos_build, stage, stage_src ? stage_src + (int64_t)blockIdx.x * g.cap : nullptr);
     __syncthreads();
 
     int wmax = 0;
@@ -180,8 +187,9 @@ nlist_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *
                         at++;
                     }
                     const int nw = min(total, pitch);
-                    const int padded = min(pitch, (nw + ROW_PAD - 1) & ~(ROW_PAD - 1));
-                    if (nw + lane < padded) row[nw + lane] = 0;               // dummy entries up to a whole group
+                    // at least 32 dummy entries end the row: the force kernel stops at the first one it meets
+                    const int pad_end = min(pitch, (nw & ~(ROW_PAD - 1)) + 2 * ROW_PAD);
+                    for (int k = nw + lane; k < pad_end; k += 32) row[k] = 0;
                     if (lane == 0) nlistn[gidx[p]] = nw;                      // l.22
                     wmax = max(wmax, total);
                 }
@@ -207,7 +215,9 @@ cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback)
     e = cudaFuncSetAttribute(nlist_tile_kernel<PPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
     if (e != cudaSuccess) return e;                                                                                     \
     nlist_tile_kernel<PPI><<<grid, TILE_THREADS, smem, h->stream>>>(h->geom, h->cell_start, h->pos_build, rmax2,        \
-                                                                    h->row_pitch, h->nlist, h->nlistn, h->flags, pred, cb);
+                                                                    h->row_pitch, h->nlist, h->nlistn, h->flags, pred, cb,  \
+                                                                    h->geom.fast ? h->stage_src : nullptr,                  \
+                                                                    h->geom.fast ? (TileDesc *)h->tile_desc : nullptr);
     switch (h->tun.nlist_ppi) {
         case 1: NL_LAUNCH(1) break;
         case 2: NL_LAUNCH(2) break;
@@ -245,8 +255,8 @@ nlist_fill_by_tag_kernel(TileGeom g, const int *__restrict__ cell_start, const u
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int q = warp; q < t.nown; q += TILE_THREADS / 32) {
-        const int r = tile_row_of(t, s, q);
-        const int gi = s.own_start[r] + (q - s.own_off[r]);
+        int gi, slot;
+        tile_own(s.d, q, gi, slot);
         const int n = nlistn[gi];
         const int64_t o = row_start[tag[gi]];
         const uint16_t *row = nlist + (int64_t)gi * pitch;

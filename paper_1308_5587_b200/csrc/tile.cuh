@@ -29,12 +29,25 @@ struct TileCtx {
     int nrows;        // own (y, z) rows = ey * ez
 };
 
-struct TileShared {
-    int hslot[TILE_HMAX + 1];   // first slot of halo cell h
-    int hg[TILE_HMAX];          // storage index of the first particle of halo cell h
+// What the force kernel needs to know about a tile.  It depends on cell_start only, so the list
+// build writes it once per build (one per tile, in global memory) and the force kernel, which
+// runs every step, just loads it.
+struct TileDesc {
+    int nslots;       // 1 + staged particles (1 = nothing staged: the build found the tile too big)
+    int nown;         // own particles
+    int nrows;        // own (y, z) rows
+    float cx, cy, cz; // centre of the tile
     int own_start[TILE_ROWS_MAX];    // storage index of the first own particle of row r
     int own_off[TILE_ROWS_MAX + 1];  // tile-local number of the first own particle of row r
     int own_slot[TILE_ROWS_MAX];     // its slot
+    int pad;
+};
+static_assert(sizeof(TileDesc) == 416, "hb_api.cu sizes the descriptor array with this number");
+
+struct TileShared {
+    int hslot[TILE_HMAX + 1];   // first slot of halo cell h
+    int hg[TILE_HMAX];          // storage index of the first particle of halo cell h
+    TileDesc d;
 };
 
 __device__ __forceinline__ void tile_decode(const TileGeom &g, int tile, TileCtx &t)
@@ -102,18 +115,26 @@ __device__ __forceinline__ bool tile_tables(const TileGeom &g, const int *__rest
         const int ly = tid % t.ey, lz = tid / t.ey;
         const int hrow = ((lz + 1) * t.hy + (ly + 1)) * t.hx;
         const int first = hrow + 1, last = hrow + t.ex;
-        s.own_start[tid] = s.hg[first];
-        s.own_slot[tid] = s.hslot[first];
-        s.own_off[tid + 1] = s.hslot[last + 1] - s.hslot[first];   // own cells of a row are consecutive halo cells
+        s.d.own_start[tid] = s.hg[first];
+        s.d.own_slot[tid] = s.hslot[first];
+        s.d.own_off[tid + 1] = s.hslot[last + 1] - s.hslot[first];   // own cells of a row are consecutive halo cells
     }
     __syncthreads();
     if (tid == 0) {
         int run = 0;
-        s.own_off[0] = 0;
-        for (int r = 0; r < t.nrows; r++) { const int n = s.own_off[r + 1]; s.own_off[r + 1] = run + n; run += n; }
+        s.d.own_off[0] = 0;
+        for (int r = 0; r < t.nrows; r++) { const int n = s.d.own_off[r + 1]; s.d.own_off[r + 1] = run + n; run += n; }
+        const float wcell = g.L / (float)g.m, hL = 0.5f * g.L;
+        s.d.nslots = t.nslots;
+        s.d.nown = run;
+        s.d.nrows = t.nrows;
+        s.d.cx = __fmaf_rn((float)t.x0 + 0.5f * (float)t.ex, wcell, -hL);
+        s.d.cy = __fmaf_rn((float)t.y0 + 0.5f * (float)t.ey, wcell, -hL);
+        s.d.cz = __fmaf_rn((float)t.z0 + 0.5f * (float)t.ez, wcell, -hL);
+        s.d.pad = 0;
     }
     __syncthreads();
-    t.nown = s.own_off[t.nrows];
+    t.nown = s.d.nown;
     if (t.nslots > g.cap) {
         if (tid == 0) atomicMax(&flags[FL_STAGE_OVER], t.nslots);
         return false;
@@ -147,11 +168,13 @@ __device__ __forceinline__ float tile_image(float x, float cc, float L, float hL
 // the box may have been wrapped to the other side, and must still be seen next to its neighbors.
 // At build time (particles inside their cells) this adds exactly -L, 0 or +L per axis.
 __device__ __forceinline__ void tile_stage_positions(const TileGeom &g, const TileCtx &t, const TileShared &s,
-                                                     const float4 *__restrict__ pos, float4 *__restrict__ stage)
+                                                     const float4 *__restrict__ pos, float4 *__restrict__ stage,
+                                                     int *__restrict__ src_out /* nullable: [cap] storage index per slot */)
 {
     constexpr int U = 4;
     const int nt = blockDim.x;
     const float wcell = g.L / (float)g.m, hL = 0.5f * g.L;
+    const bool fast = g.fast != 0;
     if (threadIdx.x == 0) stage[0] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
     for (int s0 = 1 + threadIdx.x; s0 < t.nslots; s0 += U * nt) {
         int src[U];
@@ -163,10 +186,15 @@ __device__ __forceinline__ void tile_stage_positions(const TileGeom &g, const Ti
             if (sl < t.nslots) {
                 const int h = tile_cell_of_slot(t, s, sl);
                 src[u] = s.hg[h] + (sl - s.hslot[h]);
-                const int jx = h % t.hx, jy = (h / t.hx) % t.hy, jz = h / (t.hx * t.hy);
-                cx[u] = __fmaf_rn((float)(t.x0 - 1 + jx) + 0.5f, wcell, -hL);
-                cy[u] = __fmaf_rn((float)(t.y0 - 1 + jy) + 0.5f, wcell, -hL);
-                cz[u] = __fmaf_rn((float)(t.z0 - 1 + jz) + 0.5f, wcell, -hL);
+                if (fast) {   // the whole halo box is narrower than L/2: the image nearest to the tile centre is the one
+                    cx[u] = s.d.cx; cy[u] = s.d.cy; cz[u] = s.d.cz;
+                } else {
+                    const int jx = h % t.hx, jy = (h / t.hx) % t.hy, jz = h / (t.hx * t.hy);
+                    cx[u] = __fmaf_rn((float)(t.x0 - 1 + jx) + 0.5f, wcell, -hL);
+                    cy[u] = __fmaf_rn((float)(t.y0 - 1 + jy) + 0.5f, wcell, -hL);
+                    cz[u] = __fmaf_rn((float)(t.z0 - 1 + jz) + 0.5f, wcell, -hL);
+                }
+                if (src_out) src_out[sl] = src[u];
             }
         }
         float4 p[U];
@@ -181,10 +209,48 @@ __device__ __forceinline__ void tile_stage_positions(const TileGeom &g, const Ti
     }
 }
 
+// The same staging from the tables the list build left behind (fast geometry only): per slot one
+// coalesced index load, one position load, the image nearest to the tile centre.
+__device__ __forceinline__ void tile_stage_from_table(const TileDesc &d, const int *__restrict__ src_tab,
+                                                      const float4 *__restrict__ pos, float4 *__restrict__ stage, float L)
+{
+    constexpr int U = 4;
+    const int nt = blockDim.x;
+    const float hL = 0.5f * L;
+    const int nslots = d.nslots;
+    if (threadIdx.x == 0) stage[0] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+    for (int s0 = 1 + threadIdx.x; s0 < nslots; s0 += U * nt) {
+        int src[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int sl = s0 + u * nt;
+            src[u] = sl < nslots ? __ldg(&src_tab[sl]) : -1;
+        }
+        float4 p[U];
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            if (src[u] >= 0) p[u] = pos[src[u]];
+#pragma unroll
+        for (int u = 0; u < U; u++)
+            if (src[u] >= 0)
+                stage[s0 + u * nt] = make_float4(tile_image(p[u].x, d.cx, L, hL), tile_image(p[u].y, d.cy, L, hL),
+                                                 tile_image(p[u].z, d.cz, L, hL), p[u].w);
+    }
+}
+
 // tile-local own particle q -> own row r (rows are few: linear scan)
-__device__ __forceinline__ int tile_row_of(const TileCtx &t, const TileShared &s, int q)
+__device__ __forceinline__ int tile_row_of(const TileDesc &d, int q)
 {
     int r = 0;
-    while (r + 1 < t.nrows && s.own_off[r + 1] <= q) r++;
+    while (r + 1 < d.nrows && d.own_off[r + 1] <= q) r++;
     return r;
+}
+
+// storage index and slot of own particle q
+__device__ __forceinline__ void tile_own(const TileDesc &d, int q, int &gi, int &slot)
+{
+    const int r = tile_row_of(d, q);
+    const int off = q - d.own_off[r];
+    gi = d.own_start[r] + off;
+    slot = d.own_slot[r] + off;
 }

@@ -9,7 +9,8 @@
 
 namespace {
 
-const int kRebuildKernels = 5;  // count, scan, scatter, gather, list -- see enqueue_rebuild
+int coop_mode(const hb_system *h) { return h->tun.coop_rebuild >= 0 ? h->tun.coop_rebuild : (h->N < 200000 ? 2 : 1); }
+int rebuild_kernels(const hb_system *h) { return coop_mode(h) == 2 ? 1 : coop_mode(h) == 1 ? 2 : 5; }  // see enqueue_rebuild
 
 int dev_alloc(hb_system *h, void **p, size_t bytes)
 {
@@ -267,7 +268,12 @@ int enqueue_cells(hb_system *h, const int *pred)
 // Algorithm 2 + Algorithm 3, no host interaction (pred: device flag for early exit, or NULL).
 int enqueue_rebuild(hb_system *h, const int *pred)
 {
-    HB_TRY(enqueue_cells(h, pred));
+    if (coop_mode(h) == 2) {
+        HB_CK(launch_rebuild_coop(h, pred, true));
+        return HB_OK;
+    }
+    if (coop_mode(h) == 1) HB_CK(launch_rebuild_coop(h, pred, false));
+    else HB_TRY(enqueue_cells(h, pred));
     HB_CK(launch_nlist(h, pred, true));
     return HB_OK;
 }
@@ -496,7 +502,7 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     }
     out->g = g;
     out->e = ex;
-    out->nkernels_fixed = (fuse ? n + 1 : 2 * n + 1) + (mode == 1 ? n * kRebuildKernels : 0);
+    out->nkernels_fixed = (fuse ? n + 1 : 2 * n + 1) + (mode == 1 ? n * rebuild_kernels(h) : 0);
     return HB_OK;
 }
 
@@ -580,7 +586,7 @@ int run_chunk(hb_system *h, float dt, int n)
         h->stats.graph_launches++;
         HB_TRY(read_flags(h));
         const int nb = h->h_flags[FL_BUILDS] - builds_before;
-        h->stats.kernel_launches += it->second.nkernels_fixed + (h->tun.graph_mode == 2 ? nb * kRebuildKernels : 0);
+        h->stats.kernel_launches += it->second.nkernels_fixed + (h->tun.graph_mode == 2 ? nb * rebuild_kernels(h) : 0);
         h->stats.rebuilds = h->h_flags[FL_BUILDS];
         if (h->tun.fuse_nve) h->cur ^= (n - 1) & 1;
         h->parity += n;
@@ -1106,6 +1112,8 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "row_pitch")) return &h->tun.row_pitch;
     if (!strcmp(name, "cell_sort")) return &h->tun.cell_sort;
     if (!strcmp(name, "fuse_nve")) return &h->tun.fuse_nve;
+    if (!strcmp(name, "coop_rebuild")) return &h->tun.coop_rebuild;
+    if (!strcmp(name, "coop_blocks")) return &h->tun.coop_blocks;
     if (!strcmp(name, "graph_mode")) return &h->tun.graph_mode;
     if (!strcmp(name, "graph_steps")) return &h->tun.graph_steps;
     return nullptr;
@@ -1125,6 +1133,8 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;
     else if (slot == &h->tun.row_pitch) ok = value >= 0 && value <= 4096;
     else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve) ok = value == 0 || value == 1;
+    else if (slot == &h->tun.coop_rebuild) ok = value >= -1 && value <= 2;
+    else if (slot == &h->tun.coop_blocks) ok = value >= 1 && value <= 8;
     else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 2;
     else if (slot == &h->tun.graph_steps) ok = value >= 1 && value <= 2000;
     if (!ok) { h->err = std::string("value out of range for tunable ") + name; return HB_EINVAL; }

@@ -51,15 +51,17 @@ constexpr int TILE_ROWS_MAX = 32;     // own (y, z) rows per tile, at most
 constexpr int ROW_PAD = 32;           // list rows are padded with dummy entries to a multiple of this
 
 struct Tunables {
-    int tpp = 4;           // threads per particle in the force kernel
-    int epl = 4;           // list entries per thread per iteration (4 or 8)
+    int tpp = 2;           // threads per particle in the force kernel
+    int epl = 8;           // list entries per thread per iteration (4 or 8)
     int force_block = 128; // threads per block of the force kernel (128 or 256)
     int nlist_ppi = 4;     // particles tested per candidate load
     int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
     int stage_cap = 0;     // 0 = estimated from the density
     int row_pitch = 0;
     int cell_sort = 1;
+    int coop_blocks = 2;   // blocks per SM of the cooperative cell kernel
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
+    int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 50;
 };
@@ -192,6 +194,7 @@ cudaError_t launch_cell_copyback(hb_system *h, const int *pred);   // when no li
 cudaError_t launch_scan_exclusive(hb_system *h, const int *in, int *out, int64_t n, int *tmp);
 // nlist.cu
 cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback);
+cudaError_t launch_rebuild_coop(hb_system *h, const int *pred, bool with_list);   // cells + reorder (+ list) in one cooperative launch
 size_t nlist_smem_bytes(const hb_system *h);
 // force.cu
 cudaError_t launch_force(hb_system *h, const NveArgs *nve /* nullable: forces only */);

@@ -91,7 +91,8 @@ def test_forces_energy_virial(hb, orc, case, shift):
                                  dict(nlist_ppi=1), dict(nlist_ppi=2), dict(cell_sort=0),
                                  dict(tile_x=1, tile_y=1, tile_z=1), dict(tile_x=2, tile_y=2, tile_z=2),
                                  dict(tile_x=3, tile_y=2, tile_z=1), dict(tile_x=4, tile_y=1, tile_z=2),
-                                 dict(tile_x=16, tile_y=2, tile_z=2), dict(stage_cap=64)])
+                                 dict(tile_x=16, tile_y=2, tile_z=2), dict(stage_cap=64), dict(coop_rebuild=0), dict(coop_rebuild=2),
+                                 dict(force_block=256), dict(coop_rebuild=0, stage_cap=64)])
 def test_tunables_do_not_change_results(hb, orc, tun):
     """block size and friends 'do not change the correctness'."""
     w = CASES["ka_10k"]
@@ -137,7 +138,7 @@ def test_deterministic_lists_and_forces(hb):
     assert np.array_equal(outs[0][1][0], outs[1][1][0]) and np.array_equal(outs[0][1][1], outs[1][1][1])
 
 
-@pytest.mark.parametrize("mode", ["step", "run0", "run1", "run2", "unfused1", "unfused2"])
+@pytest.mark.parametrize("mode", ["step", "run0", "run1", "run2", "unfused1", "unfused2", "nocoop1", "nocoop2"])
 def test_trajectory_config1(hb, orc, mode):
     """BASELINE configs[0]: 10 NVE steps at dt = 0.005, fp32 GPU vs fp64 oracle,
     compared by tag; expect <= 1e-5 absolute."""
@@ -154,6 +155,7 @@ def test_trajectory_config1(hb, orc, mode):
         else:
             g.set_tunable("graph_mode", int(mode[-1]))
             g.set_tunable("fuse_nve", 0 if mode.startswith("unfused") else 1)
+            g.set_tunable("coop_rebuild", 0 if mode.startswith("nocoop") else 1)
             g.set_tunable("graph_steps", 4)          # 4 + 4 + 2: several graphs, one remainder
             g.run_nve(w.dt, w.steps, 0)
         out = g.get_state()

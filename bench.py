@@ -132,14 +132,31 @@ def config_of(w, args, extra):
     return c
 
 
+# Algorithmic work of the step kernel.  Per LISTED pair the kernel must do
+# 3 sub, 3 mul/fma (r^2), 1 compare = 7 ALU ops / 9 flops; per pair inside r_cut in addition 1 rcp, 2 mul (r^-6),
+# 3 (f/r), 3 (energy), 3 mul + 3 add (force), 6 fma (virial) = 24 ALU ops / 33 flops (an FMA counts 2 flops, 1 op).
+OPS_LISTED, FLOPS_LISTED, OPS_INCUT, FLOPS_INCUT = 7, 9, 24, 33
+
+
 def force_work(g, w):
-    """Algorithmic bytes and flops of one lj_force launch."""
+    """Algorithmic bytes, flops and ALU ops of one launch of the force kernel."""
     pairs = int(g.get_nlist_sizes()[-1])
     N = w.N
-    bytes_ = 4 * pairs + N * (16 + 4 + 16 + 24)     # indices + pos_i + count + force out + virial out
+    # 16-bit list entries + position in, force + virial out, + velocity and position in and out when the step is fused in
+    bytes_ = 2 * pairs + N * (16 + 16 + 32) + N * (16 + 16 + 16 + 16)
     frac_in = (w.r_cut_max / w.r_max) ** 3 if w.ntypes == 1 else 0.55
-    flops = 20 * pairs + 25 * frac_in * pairs
-    return pairs, bytes_, flops
+    flops = FLOPS_LISTED * pairs + FLOPS_INCUT * frac_in * pairs
+    ops = OPS_LISTED * pairs + OPS_INCUT * frac_in * pairs
+    return pairs, bytes_, flops, ops
+
+
+def ncu_traffic(kernel):
+    """dram__bytes_read + dram__bytes_write per launch from the committed ncu capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f).get(kernel)
+    return None
 
 
 def main():
@@ -218,29 +235,40 @@ def main():
     stats = g.stats()
 
     # ---- per-kernel rooflines, measured live with CUDA events on the launching stream ----
-    pairs, fbytes, fflops = force_work(g, w)
-    t_force = g.time_stage("lj_force", 200)
-    t_force_cold = g.time_stage("lj_force", 20, 512 << 20)
+    # (hb_time_stage: the launches of one stage captured into one graph, CUDA events around the graph launch)
+    pairs, fbytes, fflops, fops = force_work(g, w)
+    t_step = g.time_stage("lj_nve", 200)                    # the kernel a step of hb_run_nve is: force + kicks + drift
+    t_force = g.time_stage("lj_force", 200)                 # the same kernel without the integration
+    t_step_cold = g.time_stage("lj_nve", 20, 512 << 20)     # L2 flushed before every launch
     t_nlist = g.time_stage("nlist", 50)
     t_cells = g.time_stage("cells", 50)
+    t_rebuild = g.time_stage("rebuild", 50)
     t_nve = g.time_stage("nve", 200)
-    share_force = t_force * args.steps / ms
-    roof_alu = {"bound": "alu", "achieved": fflops / (t_force * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "kernel": "lj_force_kernel", "ms": t_force, "traffic": None,
-                "peak_source": "nominal fp32: 148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md)"}
+    rate = delta["rebuilds"] / args.steps
+    share_step_kernel = t_step * args.steps / ms
+    roof_alu = {"bound": "alu", "achieved": fflops / (t_step * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "kernel": "lj_tile_kernel", "ms": t_step, "traffic": ncu_traffic("lj_tile_kernel"),
+                "peak_source": "nominal fp32: 148 SM x 128 lanes x 2 flop x 1.965 GHz (DESIGN.md); no measured fp32 peak exists",
+                "alu_ops_frac": fops / (t_step * 1e-3) / (FP32_PEAK_TFLOPS * 1e12 / 2),
+                "alu_ops_note": "algorithmic ALU instructions (an FMA is one) per second over 148 x 128 x 1.965 GHz issue slots"}
     roof_alu["frac"] = roof_alu["achieved"] / roof_alu["peak"]
-    roof_hbm = {"bound": "hbm", "achieved": fbytes / (t_force_cold * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "kernel": "lj_force_kernel", "ms": t_force_cold, "traffic": None,
+    roof_hbm = {"bound": "hbm", "achieved": fbytes / (t_step_cold * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "kernel": "lj_tile_kernel", "ms": t_step_cold, "traffic": ncu_traffic("lj_tile_kernel"),
                 "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind}); L2 flushed before every launch"}
     roof_hbm["frac"] = roof_hbm["achieved"] / roof_hbm["peak"]
-    nl_bytes = 4 * pairs + w.N * (4 + 32)
+    nl_bytes = 2 * pairs + w.N * (16 + 4 + 64)              # positions in, 16-bit entries + count out, reorder copy-back
+    nl_tests = 27.0 * w.N * w.N / stats["cells_per_axis"] ** 3
     kernels = {
-        "lj_force": {"ms_warm_l2": t_force, "ms_cold_l2": t_force_cold, "pairs": pairs, "algorithmic_bytes": fbytes,
-                     "algorithmic_flops": fflops, "share_of_step": share_force},
+        "lj_step": {"ms_warm_l2": t_step, "ms_cold_l2": t_step_cold, "ms_force_only": t_force, "pairs": pairs,
+                    "algorithmic_bytes": fbytes, "algorithmic_flops": fflops, "algorithmic_alu_ops": fops,
+                    "share_of_step": share_step_kernel},
         "nlist": {"ms": t_nlist, "algorithmic_bytes": nl_bytes, "gbs": nl_bytes / (t_nlist * 1e-3) / 1e9,
-                  "frac_hbm": nl_bytes / (t_nlist * 1e-3) / 1e9 / hbm_peak},
-        "cells": {"ms": t_cells, "algorithmic_bytes": 36 * w.N},
-        "nve": {"ms": t_nve, "algorithmic_bytes": 108 * w.N, "gbs": 108 * w.N / (t_nve * 1e-3) / 1e9},
+                  "frac_hbm": nl_bytes / (t_nlist * 1e-3) / 1e9 / hbm_peak, "distance_tests": nl_tests,
+                  "alu_ops_frac": 8 * nl_tests / (t_nlist * 1e-3) / (FP32_PEAK_TFLOPS * 1e12 / 2)},
+        "cells": {"ms": t_cells, "algorithmic_bytes": 36 * w.N + 100 * w.N},
+        "rebuild": {"ms": t_rebuild, "per_step": rate, "ms_per_step": rate * t_rebuild},
+        "nve_standalone": {"ms": t_nve, "algorithmic_bytes": 108 * w.N, "gbs": 108 * w.N / (t_nve * 1e-3) / 1e9},
+        "step_model": {"ms": t_step + rate * t_rebuild, "launch_gaps_ms": ms / args.steps - (t_step + rate * t_rebuild)},
     }
 
     # ---- end to end through the C ABI with HOST buffers ----
@@ -273,14 +301,14 @@ def main():
         g2, _ = make_system(w2, seed=w2.seed)
         g2.run_nve(w2.dt, 600, w2.sort_period)
         ms2, d2 = timed_run(g2, w2, 1000)
-        p2 = int(g2.get_nlist_sizes()[-1])
-        b2 = 4 * p2 + w2.N * 60
-        tf2 = g2.time_stage("lj_force", 30)
+        p2, b2, f2, o2 = force_work(g2, w2)
+        tf2 = g2.time_stage("lj_nve", 30)
         tn2 = g2.time_stage("nlist", 10)
         also = {"lj_1m": {"timesteps_per_s": 1000 / (ms2 * 1e-3), "particle_steps_per_s": 1000 * w2.N / (ms2 * 1e-3),
-                          "ms_per_step": ms2 / 1000, "rebuilds": d2["rebuilds"], "lj_force_ms": tf2,
-                          "lj_force_hbm_gbs": b2 / (tf2 * 1e-3) / 1e9, "lj_force_hbm_frac": b2 / (tf2 * 1e-3) / 1e9 / hbm_peak,
-                          "nlist_ms": tn2, "mean_nbrs": p2 / w2.N, "inputs": "larger than L2 (252 MB list)"}}
+                          "ms_per_step": ms2 / 1000, "rebuilds": d2["rebuilds"], "lj_step_ms": tf2,
+                          "lj_step_hbm_gbs": b2 / (tf2 * 1e-3) / 1e9, "lj_step_hbm_frac": b2 / (tf2 * 1e-3) / 1e9 / hbm_peak,
+                          "lj_step_alu_frac": f2 / (tf2 * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
+                          "nlist_ms": tn2, "mean_nbrs": p2 / w2.N, "inputs": "larger than L2 (126 MB list + tables)"}}
         g2.close()
 
     cpu = None
@@ -308,8 +336,8 @@ def main():
                               "note": "PAPER.md:143, other hardware and an equilibrated start: context, not vs_baseline"},
             "run": {**delta, "E_per_particle": (th["K"] + th["U"]) / w.N, "T": 2 * th["K"] / (3 * w.N),
                     "max_nbrs": stats["max_nbrs"]},
-            "roofline": roof_alu if w.N < 400_000 else roof_hbm,
-            "roofline_other": roof_hbm if w.N < 400_000 else roof_alu,
+            "roofline": roof_alu,
+            "roofline_other": roof_hbm,
             "kernels": kernels,
             "cpu_baseline": cpu,
             "e2e": e2e,

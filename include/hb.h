@@ -181,6 +181,7 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *   "graph_mode"     0 = no graphs (host reads the flag each step)
  *                    1 = graphs of kernels that exit early unless rebuilding
  *                    2 = graphs with a conditional IF node around the rebuild
+ *                    3 = the launches of mode 1 issued one by one, no graph (for profilers)
  *   "graph_steps"    steps per graph launch
  */
 HB_API int hb_set_tunable(hb_system *h, const char *name, int value);

@@ -392,6 +392,36 @@ NveArgs make_nve(hb_system *h, float dt, bool kick_prev, bool kick_drift, float4
     return a;
 }
 
+// The launches of an n-step chunk without conditional nodes (graph_mode 1 inside a capture, graph_mode 3 straight
+// into the stream): every rebuild kernel takes the drift's flag as its predicate.  Advances h->cur / h->parity.
+int enqueue_chunk_pred(hb_system *h, int n, float dt)
+{
+    const bool fuse = h->tun.fuse_nve != 0;
+    for (int s = 0; s < n; s++) {
+        const int need_flag = FL_NEED0 + (h->parity & 1);
+        if (s == 0) {
+            HB_CK(launch_nve(h, make_nve(h, dt, false, true, h->pos(), 0, false)));
+        } else if (fuse) {
+            const NveArgs a = make_nve(h, dt, true, true, h->posbuf[h->cur ^ 1], 0, false);
+            HB_CK(launch_force(h, &a));
+            h->cur ^= 1;
+        } else {
+            HB_CK(launch_force(h, nullptr));
+            HB_CK(launch_nve(h, make_nve(h, dt, true, true, h->pos(), 0, false)));
+        }
+        h->parity++;
+        HB_TRY(enqueue_rebuild(h, h->flags + need_flag));
+    }
+    if (fuse) {
+        const NveArgs a = make_nve(h, dt, true, false, h->pos(), 0, false);
+        HB_CK(launch_force(h, &a));
+    } else {
+        HB_CK(launch_force(h, nullptr));
+        HB_CK(launch_nve(h, make_nve(h, dt, true, false, h->pos(), 0, false)));
+    }
+    return HB_OK;
+}
+
 // ---- hb_run_nve: n steps as one CUDA graph ----
 // fuse_nve = 1:  nve(drift) [rebuild?]  { lj+nve(kick, kick, drift) [rebuild?] } x (n-1)  lj+nve(kick)
 // fuse_nve = 0:  nve(drift) [rebuild?]  { lj  nve(kick, kick, drift) [rebuild?] } x (n-1)  lj  nve(kick)
@@ -573,17 +603,32 @@ int run_chunk(hb_system *h, float dt, int n)
     for (int attempt = 0; attempt < 8; attempt++) {
         HB_TRY(ensure_forces(h));
         if (dt != h->graph_dt) { destroy_graphs(h); h->graph_dt = dt; }
+        const bool plain = h->tun.graph_mode == 3;   // the launches of mode 1, issued one by one (for profilers)
         const int64_t key = ((int64_t)n << 2) | ((h->cur & 1) << 1) | (h->parity & 1);
         auto it = h->graphs.find(key);
-        if (it == h->graphs.end()) {
+        if (plain) {
+            if (it == h->graphs.end()) {
+                hb_system::GraphEntry ge;
+                ge.nkernels_fixed = (h->tun.fuse_nve ? n + 1 : 2 * n + 1) + n * rebuild_kernels(h);
+                it = h->graphs.emplace(key, ge).first;
+            }
+        } else if (it == h->graphs.end()) {
             hb_system::GraphEntry ge;
             HB_TRY(build_graph(h, n, dt, &ge));
             it = h->graphs.emplace(key, ge).first;
         }
         HB_TRY(backup_state(h));
         const int builds_before = h->h_flags[FL_BUILDS];
-        HB_CK(cudaGraphLaunch(it->second.e, h->stream));
-        h->stats.graph_launches++;
+        if (plain) {
+            const int c0 = h->cur, p0 = h->parity;
+            const int64_t l0 = h->stats.kernel_launches;
+            HB_TRY(enqueue_chunk_pred(h, n, dt));
+            h->cur = c0; h->parity = p0;            // advanced again below, as after a graph launch
+            h->stats.kernel_launches = l0;
+        } else {
+            HB_CK(cudaGraphLaunch(it->second.e, h->stream));
+            h->stats.graph_launches++;
+        }
         HB_TRY(read_flags(h));
         const int nb = h->h_flags[FL_BUILDS] - builds_before;
         h->stats.kernel_launches += it->second.nkernels_fixed + (h->tun.graph_mode == 2 ? nb * rebuild_kernels(h) : 0);
@@ -1135,7 +1180,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve) ok = value == 0 || value == 1;
     else if (slot == &h->tun.coop_rebuild) ok = value >= -1 && value <= 2;
     else if (slot == &h->tun.coop_blocks) ok = value >= 1 && value <= 8;
-    else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 2;
+    else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 3;
     else if (slot == &h->tun.graph_steps) ok = value >= 1 && value <= 2000;
     if (!ok) { h->err = std::string("value out of range for tunable ") + name; return HB_EINVAL; }
     *slot = value;

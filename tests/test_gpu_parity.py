@@ -138,7 +138,7 @@ def test_deterministic_lists_and_forces(hb):
     assert np.array_equal(outs[0][1][0], outs[1][1][0]) and np.array_equal(outs[0][1][1], outs[1][1][1])
 
 
-@pytest.mark.parametrize("mode", ["step", "run0", "run1", "run2", "unfused1", "unfused2", "nocoop1", "nocoop2"])
+@pytest.mark.parametrize("mode", ["step", "run0", "run1", "run2", "run3", "unfused1", "unfused2", "nocoop1", "nocoop2"])
 def test_trajectory_config1(hb, orc, mode):
     """BASELINE configs[0]: 10 NVE steps at dt = 0.005, fp32 GPU vs fp64 oracle,
     compared by tag; expect <= 1e-5 absolute."""

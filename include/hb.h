@@ -177,7 +177,13 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *   "stage_cap"      shared-memory slots per tile (0 = from the density); grown on overflow
  *   "row_pitch"      initial entries per list row (rounded up to 64; 0 = estimate)
  *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
+ *   "force_block"    threads per block of the force kernel: 128, 256
+ *   "nlist_block"    threads per block of the stand-alone list kernel: 128, 256
  *   "fuse_nve"       1 = hb_run_nve integrates inside the force kernel (one kernel per step)
+ *   "coop_rebuild"   0 = the rebuild is five launches (count, scan, scatter, gather, list);
+ *                    1 = Algorithm 2 and the reorder are ONE cooperative kernel, then the list kernel;
+ *                    2 = the list build is a phase of that kernel too
+ *   "coop_blocks"    blocks per SM of the cooperative cell kernel (1..8)
  *   "graph_mode"     0 = no graphs (host reads the flag each step)
  *                    1 = graphs of kernels that exit early unless rebuilding
  *                    2 = graphs with a conditional IF node around the rebuild

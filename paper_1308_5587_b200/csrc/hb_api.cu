@@ -9,7 +9,7 @@
 
 namespace {
 
-int coop_mode(const hb_system *h) { return h->tun.coop_rebuild >= 0 ? h->tun.coop_rebuild : (h->N < 200000 ? 2 : 1); }
+int coop_mode(const hb_system *h) { return h->tun.coop_rebuild >= 0 ? h->tun.coop_rebuild : 1; }
 int rebuild_kernels(const hb_system *h) { return coop_mode(h) == 2 ? 1 : coop_mode(h) == 1 ? 2 : 5; }  // see enqueue_rebuild
 
 int dev_alloc(hb_system *h, void **p, size_t bytes)
@@ -1150,6 +1150,7 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "epl")) return &h->tun.epl;
     if (!strcmp(name, "force_block")) return &h->tun.force_block;
     if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
+    if (!strcmp(name, "nlist_block")) return &h->tun.nlist_block;
     if (!strcmp(name, "tile_x")) return &h->tun.tile_x;
     if (!strcmp(name, "tile_y")) return &h->tun.tile_y;
     if (!strcmp(name, "tile_z")) return &h->tun.tile_z;
@@ -1172,7 +1173,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     bool ok = true;
     if (slot == &h->tun.tpp) ok = value == 2 || value == 4 || value == 8;
     else if (slot == &h->tun.epl) ok = value == 4 || value == 8;
-    else if (slot == &h->tun.force_block) ok = value == 128 || value == 256;
+    else if (slot == &h->tun.force_block || slot == &h->tun.nlist_block) ok = value == 128 || value == 256;
     else if (slot == &h->tun.nlist_ppi) ok = value == 1 || value == 2 || value == 4;
     else if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z) ok = value >= 0 && value <= 16;
     else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;

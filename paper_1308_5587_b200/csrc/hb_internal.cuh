@@ -21,6 +21,8 @@ enum {
     FL_STAGE_OVER = 7,  // sticky: some tile needed more shared-memory slots than stage_cap (value = slots needed)
     FL_SCAN_CTR = 8,    // "last block done" counter of the cell scan
     FL_CHECK = 9,       // result of the on-demand displacement check (hb_needs_rebuild)
+    FL_BAR0 = 10,       // arrival counters of the cooperative rebuild kernel's grid barrier; build b uses
+    FL_BAR1 = 11,       //   FL_BAR0 + (b & 1) and clears the other one
     FL_COUNT = 16
 };
 
@@ -55,13 +57,14 @@ struct Tunables {
     int epl = 8;           // list entries per thread per iteration (4 or 8)
     int force_block = 128; // threads per block of the force kernel (128 or 256)
     int nlist_ppi = 4;     // particles tested per candidate load
+    int nlist_block = 256; // threads per block of the stand-alone list kernel (128 or 256)
     int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
     int stage_cap = 0;     // 0 = estimated from the density
     int row_pitch = 0;
     int cell_sort = 1;
     int coop_blocks = 2;   // blocks per SM of the cooperative cell kernel
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
-    int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
+    int coop_rebuild = 1;  // 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 50;
 };

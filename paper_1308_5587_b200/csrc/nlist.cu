@@ -22,19 +22,15 @@
 // (hb_get_nlist translates back to tags).  Half the bytes of a 32-bit index list.
 // The kernel also finishes the reorder of the particle data: it copies the tile's
 // own particles from the scratch set (cell order) back into the live arrays.
-#include <cooperative_groups.h>
-
 #include "cells_dev.cuh"
 #include "tile.cuh"
-
-namespace cg = cooperative_groups;
 
 constexpr int NL_CLIST = 1024;   // candidate slots per warp per chunk = 32 groups of 32 = one bit mask
 constexpr int NL_WARPS = TILE_THREADS / 32;
 
 size_t nlist_smem_bytes(const hb_system *h)
 {
-    return (size_t)h->geom.cap * 16 + (size_t)NL_WARPS * NL_CLIST * 2;
+    return (size_t)h->geom.cap * 16 + (size_t)NL_WARPS * NL_CLIST * 2;   // sized for the largest block (8 warps)
 }
 
 struct CopyBack {   // scratch set -> live arrays; pos == nullptr: skip
@@ -87,7 +83,7 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
 
     // the reorder's last leg: own particles, scratch set -> live arrays (always, so the state stays whole)
     if (cb.pos) {
-        for (int q = threadIdx.x; q < t.nown; q += TILE_THREADS) {
+        for (int q = threadIdx.x; q < t.nown; q += blockDim.x) {
             int gi, slot;
             tile_own(s.d, q, gi, slot);
             cb.pos[gi] = pos_build[gi];
@@ -115,8 +111,9 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
     const int ncell_own = t.ex * t.ey * t.ez;
     // a tile with fewer cells than the block has warps gives every cell several warps: they share the cell's
     // candidates and split its particles
-    const int wpc = max(1, NL_WARPS / max(1, ncell_own));
-    for (int item = warp; item < ncell_own * wpc; item += NL_WARPS) {
+    const int nwarps = blockDim.x >> 5;
+    const int wpc = max(1, nwarps / max(1, ncell_own));
+    for (int item = warp; item < ncell_own * wpc; item += nwarps) {
         const int oc = item / wpc, part = item % wpc;
         const int lx = oc % t.ex, ly = (oc / t.ex) % t.ey, lz = oc / (t.ex * t.ey);
         const int hc = ((lz + 1) * t.hy + (ly + 1)) * t.hx + (lx + 1);
@@ -251,26 +248,46 @@ __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs 
     if (pred && *pred == 0) return;   // every block takes the same way: no barrier is left waiting
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int scan_smem[SCAN_THREADS / 32];
-    cg::grid_group grid = cg::this_grid();
+    // Grid-wide barrier: the launch is cooperative, so all blocks are resident; every block adds one to a
+    // counter and waits until the counter reaches (barriers passed so far + 1) x gridDim.x.  (cooperative_groups'
+    // grid.sync() took about 5 us per barrier here, this one about 1 us.)  The counter of build b is
+    // flags[FL_BAR0 + (b & 1)]: b = flags[FL_BUILDS] cannot change before the last barrier is behind every
+    // block, and block 0 clears the other counter for the next build.
+    int *const flags = la.flags;
+    const int gen = *(volatile int *)&flags[FL_BUILDS];
+    unsigned *const bar = reinterpret_cast<unsigned *>(flags + FL_BAR0 + (gen & 1));
+    if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_BAR0 + ((gen + 1) & 1)] = 0;
+    unsigned passed = 0;
+    auto grid_barrier = [&]() {
+        passed += gridDim.x;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            atomicAdd(bar, 1u);
+            while (*(volatile unsigned *)bar < passed) { }
+            __threadfence();
+        }
+        __syncthreads();
+    };
     const int64_t gtid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, gsize = (int64_t)gridDim.x * blockDim.x;
 
     for (int64_t i = gtid; i < ca.N; i += gsize) cell_count_one(ca, (int)i);
-    grid.sync();
+    grid_barrier();
     const int nscan = (int)((ca.ncells + SCAN_TILE - 1) / SCAN_TILE);
     for (int st = blockIdx.x; st < nscan; st += gridDim.x) {
         const int total = block_scan_tile(ca.cell_count, ca.ncells, ca.cell_local, 0, true, ca.cell_count, st);
         if (threadIdx.x == 0) ca.sums[st] = total;
     }
-    grid.sync();
+    grid_barrier();
     if (blockIdx.x == 0) scan_sums_in_place(ca.sums, nscan, scan_smem);
-    grid.sync();
+    grid_barrier();
     const int64_t nsc = ca.N > ca.ncells + 1 ? (int64_t)ca.N : ca.ncells + 1;
     for (int64_t i = gtid; i < nsc; i += gsize) cell_scatter_one(ca, i);
-    grid.sync();
+    grid_barrier();
     const int lane = threadIdx.x & 31;
     for (int64_t c = gtid >> 5; c < ca.ncells; c += gsize >> 5) cell_gather_one(ca.cell_start, ca.perm, ga, do_sort, c, lane);
     if (WITH_LIST) {
-        grid.sync();
+        grid_barrier();
         for (int tile = blockIdx.x; tile < la.g.ntiles; tile += gridDim.x) {
             nlist_tile_body<PPI>(la, tile, smem_raw);
             __syncthreads();              // the next tile reuses the staging area
@@ -304,7 +321,7 @@ cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback)
 #define NL_LAUNCH(PPI)                                                                                                  \
     e = cudaFuncSetAttribute(nlist_tile_kernel<PPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
     if (e != cudaSuccess) return e;                                                                                     \
-    nlist_tile_kernel<PPI><<<grid, TILE_THREADS, smem, h->stream>>>(la, pred);
+    nlist_tile_kernel<PPI><<<grid, h->tun.nlist_block, smem, h->stream>>>(la, pred);
     switch (h->tun.nlist_ppi) {
         case 1: NL_LAUNCH(1) break;
         case 2: NL_LAUNCH(2) break;

@@ -313,8 +313,8 @@ def main():
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        n_cpu = max(2, int(15.0 / (w.N * 70 / 2.0e7 / max(1, os.cpu_count() or 1) * 4)))
-        n_cpu = min(n_cpu, 200)
+        # about 15 s of CPU work: the oracle takes ~1.5e-7 s per particle per step on the 16 cores of these boxes
+        n_cpu = max(2, min(2000, int(15.0 / (w.N * 1.5e-7 * 16 / max(1, os.cpu_count() or 1)))))
         v, secs, cores, builds = cpu_oracle_steps_per_s(w, st0, n_cpu)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {n_cpu} steps of {w.name} (N={w.N}) from the seeded lattice start incl. the initial list build "

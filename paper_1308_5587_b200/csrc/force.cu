@@ -272,7 +272,7 @@ size_t force_smem_bytes(const hb_system *h)
 {
     // staged positions, pair table, ring of 4 async list copies (16 B at most) per thread
     return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? ((sizeof(PairParam) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
-           (size_t)4 * 16 * h->tun.force_block;
+           (size_t)4 * 16 * force_block_of(h);
 }
 
 template <int TPP, int EPL>
@@ -286,7 +286,7 @@ static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
 #define LJ_LAUNCH(ONE)                                                                                                      \
     e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
     if (e != cudaSuccess) return e;                                                                                         \
-    lj_tile_kernel<TPP, EPL, ONE><<<grid, h->tun.force_block, smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
+    lj_tile_kernel<TPP, EPL, ONE><<<grid, force_block_of(h), smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
                                                                            h->nlistn, h->row_pitch, (int)h->N, h->ntypes,  \
                                                                            h->params, h->force, h->virial, h->flags,       \
                                                                            nve ? 1 : 0, nv, h->stage_src,                  \

@@ -94,11 +94,16 @@ int choose_tiles(hb_system *h, int min_cap)
         return (int64_t)cdiv(m, std::min(ax, m)) * cdiv(m, std::min(ay, m)) * cdiv(m, std::min(az, m));
     };
     if (tx <= 0 || ty <= 0 || tz <= 0) {
-        // largest brick that still leaves every SM several tiles (smaller halo overhead per particle)
-        const int cand[4][3] = {{2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
-        int pick = 3;
-        for (int k = 0; k < 4; k++)
-            if (ntiles_of(cand[k][0], cand[k][1], cand[k][2]) >= (int64_t)6 * h->sm_count) { pick = k; break; }
+        // The largest brick (least halo per own particle) that still leaves every SM several tiles and holds at
+        // most ~256 own particles (measured on B200: 2x2x1 at N = 64,000, 4x2x2 at 10^6, 4x4x4 for the WCA fluid
+        // with its 2.5 particles per cell).
+        const int cand[7][3] = {{4, 4, 4}, {4, 4, 2}, {4, 2, 2}, {2, 2, 2}, {2, 2, 1}, {2, 1, 1}, {1, 1, 1}};
+        const double per_cell = (double)h->N / (double)h->ncells;
+        int pick = 6;
+        for (int k = 0; k < 7; k++) {
+            const int ax = std::min(cand[k][0], m), ay = std::min(cand[k][1], m), az = std::min(cand[k][2], m);
+            if (ntiles_of(ax, ay, az) >= (int64_t)6 * h->sm_count && per_cell * ax * ay * az <= 256.0) { pick = k; break; }
+        }
         tx = cand[pick][0]; ty = cand[pick][1]; tz = cand[pick][2];
     }
     tx = std::min(tx, m); ty = std::min(ty, m); tz = std::min(tz, m);
@@ -136,6 +141,7 @@ int choose_tiles(hb_system *h, int min_cap)
         cap = stage_cap_max(h);
     }
     g.cap = cap;
+    h->own_est = (double)h->N / (double)h->ncells * tx * ty * tz;
     // fast geometry: tile + halo + what a particle can drift between builds is narrower than L/2 on every axis,
     // so the periodic image nearest to the tile centre is the right one for every staged particle
     {
@@ -1173,7 +1179,8 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     bool ok = true;
     if (slot == &h->tun.tpp) ok = value == 2 || value == 4 || value == 8;
     else if (slot == &h->tun.epl) ok = value == 4 || value == 8;
-    else if (slot == &h->tun.force_block || slot == &h->tun.nlist_block) ok = value == 128 || value == 256;
+    else if (slot == &h->tun.force_block) ok = value == 0 || value == 128 || value == 256;
+    else if (slot == &h->tun.nlist_block) ok = value == 128 || value == 256;
     else if (slot == &h->tun.nlist_ppi) ok = value == 1 || value == 2 || value == 4;
     else if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z) ok = value >= 0 && value <= 16;
     else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;

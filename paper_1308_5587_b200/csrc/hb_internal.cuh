@@ -55,7 +55,7 @@ constexpr int ROW_PAD = 32;           // list rows are padded with dummy entries
 struct Tunables {
     int tpp = 2;           // threads per particle in the force kernel
     int epl = 8;           // list entries per thread per iteration (4 or 8)
-    int force_block = 128; // threads per block of the force kernel (128 or 256)
+    int force_block = 0;   // threads per block of the force kernel (128 or 256; 0 = one pass over the tile's particles if possible)
     int nlist_ppi = 4;     // particles tested per candidate load
     int nlist_block = 256; // threads per block of the stand-alone list kernel (128 or 256)
     int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
@@ -120,6 +120,7 @@ struct hb_system {
 
     // neighbor list: row i = nlist[i * row_pitch .. + nlistn[i]), entries are shared-memory slots of i's tile
     TileGeom geom{};
+    double own_est = 0;          // expected own particles per tile
     int *stage_src = nullptr;    // [ntiles][cap] storage index of every staged slot (written by the list build)
     void *tile_desc = nullptr;   // [ntiles] TileDesc (tile.cuh), written by the list build
     int64_t stage_src_len = 0, tile_desc_len = 0;
@@ -173,6 +174,12 @@ struct hb_system {
     } while (0)
 
 static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+static inline int force_block_of(const hb_system *h)
+{
+    if (h->tun.force_block > 0) return h->tun.force_block;
+    return h->own_est * h->tun.tpp > 160.0 ? 256 : 128;
+}
 
 // What the drift part of a step kernel needs (nve_kernel and the fused force kernel).
 struct NveArgs {

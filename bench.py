@@ -124,6 +124,21 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
+def max_over_ranks(x, dist, device):
+    """Replicas only: the one quantity the ranks exchange is a time, reduced with MAX."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, steps, ms_max):
+    """Independent systems, one per rank: steps of all ranks over the slowest rank's time."""
+    return world * steps / (ms_max * 1e-3)
+
+
 def config_of(w, args, extra):
     c = {"workload": w.name, "N": w.N, "rho": w.rho, "T": w.T, "r_cut": w.r_cut_max, "r_buff": w.r_buff, "dt": w.dt,
          "ntypes": w.ntypes, "shift": "energy" if w.shift else "none", "sort_period": w.sort_period,
@@ -216,10 +231,7 @@ def main():
         e1.record()
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(ms, dist, "cuda")
         s1 = g.stats()
         return ms, {k: s1[k] - s0[k] for k in ("rebuilds", "sorts", "kernel_launches", "graph_launches", "overflow_retries")}
 
@@ -230,7 +242,7 @@ def main():
     sampler.start()
     ms, delta = timed_run(g, w, args.steps)
     clocks = sampler.stop()
-    value = world * args.steps / (ms * 1e-3)
+    value = whole_job_value(world, args.steps, ms)
     th = g.thermo()
     stats = g.stats()
 
@@ -286,10 +298,7 @@ def main():
     g.get_state_into(pos=pos_h, type=typ_h, vel=vel_h, image=img_h)  # D2H inside the timed region
     th_e = g.thermo()
     el = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([el], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        el = float(t.item())
+    el = max_over_ranks(el, dist, "cuda")
     e2e = {"value": world * Ke / el, "unit": UNIT, "steps_per_call": Ke, "h2d_bytes_per_step": w.N * 40 / Ke,
            "d2h_bytes_per_step": (w.N * 40 + 96) / Ke, "h2d_bytes_per_call": w.N * 40, "d2h_bytes_per_call": w.N * 40 + 96,
            "note": "hb_set_state(host) + hb_run_nve + hb_get_state(host) + hb_thermo, wall clock"}

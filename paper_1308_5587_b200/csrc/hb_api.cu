@@ -1068,8 +1068,8 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
     if (!stage || reps <= 0 || reps > 100000 || !mean_ms || flush_l2_bytes < 0) return HB_EINVAL;
     if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
     int which = -1;
-    const char *names[] = {"lj_force", "nlist", "cells", "rebuild", "nve", "lj_nve"};
-    for (int k = 0; k < 6; k++) if (!strcmp(stage, names[k])) which = k;
+    const char *names[] = {"lj_force", "nlist", "cells", "rebuild", "nve", "lj_nve", "cells_coop"};
+    for (int k = 0; k < 7; k++) if (!strcmp(stage, names[k])) which = k;
     if (which < 0) { h->err = std::string("unknown stage ") + stage; return HB_EINVAL; }
     void *scratch = nullptr;
     if (flush_l2_bytes > 0) HB_TRY(dev_alloc(h, &scratch, (size_t)flush_l2_bytes));
@@ -1084,6 +1084,7 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
             case 2: HB_TRY(enqueue_cells(h, nullptr)); break;
             case 3: HB_TRY(enqueue_rebuild(h, nullptr)); break;
             case 4: HB_CK(launch_nve(h, make_nve(h, 0.0f, true, true, h->pos(), 0, false))); break;
+            case 6: HB_CK(launch_rebuild_coop(h, nullptr, false)); break;
             default: {
                 const NveArgs a = make_nve(h, 0.0f, true, true, h->posbuf[h->cur ^ 1], 0, false);
                 HB_CK(launch_force(h, &a));
@@ -1141,7 +1142,7 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
     if (tg) cudaGraphDestroy(tg);
     dev_free(h, scratch);
     if (rc == HB_OK) rc = clear_need_flags(h);
-    if (rc == HB_OK && (which == 2 || which == 3)) {
+    if (rc == HB_OK && (which == 2 || which == 3 || which == 6)) {
         // the timed cell builds re-ordered the scratch set (and, for "rebuild", the particles): make the list whole again
         h->nlist_valid = false;
         rc = ensure_forces(h);

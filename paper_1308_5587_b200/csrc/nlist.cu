@@ -251,10 +251,10 @@ __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs 
     // Grid-wide barrier: the launch is cooperative, so all blocks are resident; every block adds one to a
     // counter and waits until the counter reaches (barriers passed so far + 1) x gridDim.x.  (cooperative_groups'
     // grid.sync() took about 5 us per barrier here, this one about 1 us.)  The counter of build b is
-    // flags[FL_BAR0 + (b & 1)]: b = flags[FL_BUILDS] cannot change before the last barrier is behind every
-    // block, and block 0 clears the other counter for the next build.
+    // flags[FL_BAR0 + (b & 1)], b = flags[FL_BAR_GEN]: every block reads b before its first barrier, block 0
+    // advances it after its last one and clears the other counter for the next build.
     int *const flags = la.flags;
-    const int gen = *(volatile int *)&flags[FL_BUILDS];
+    const int gen = *(volatile int *)&flags[FL_BAR_GEN];
     unsigned *const bar = reinterpret_cast<unsigned *>(flags + FL_BAR0 + (gen & 1));
     if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_BAR0 + ((gen + 1) & 1)] = 0;
     unsigned passed = 0;
@@ -286,8 +286,9 @@ __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs 
     grid_barrier();
     const int lane = threadIdx.x & 31;
     for (int64_t c = gtid >> 5; c < ca.ncells; c += gsize >> 5) cell_gather_one(ca.cell_start, ca.perm, ga, do_sort, c, lane);
+    if (WITH_LIST) grid_barrier();
+    if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_BAR_GEN] = gen + 1;   // every block is past its first barrier
     if (WITH_LIST) {
-        grid_barrier();
         for (int tile = blockIdx.x; tile < la.g.ntiles; tile += gridDim.x) {
             nlist_tile_body<PPI>(la, tile, smem_raw);
             __syncthreads();              // the next tile reuses the staging area

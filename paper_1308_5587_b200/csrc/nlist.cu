@@ -104,7 +104,7 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
             reinterpret_cast<int *>(desc + tile)[threadIdx.x] = reinterpret_cast<const int *>(&s.d)[threadIdx.x];
     }
     if (!fits) return;
-    tile_stage_positions(g, t, s, pos_build, stage, stage_src ? stage_src + (int64_t)tile * g.cap : nullptr);
+    tile_stage_positions_by_cell(g, t, s, pos_build, stage, stage_src ? stage_src + (int64_t)tile * g.cap : nullptr);
     __syncthreads();
 
     int wmax = 0;
@@ -214,8 +214,11 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                     }
                     const int nw = min(total, pitch);
                     // at least 32 dummy entries end the row: the force kernel stops at the first one it meets
+                    // (pad_end is even and the row is 128-byte aligned: one 16-bit store if nw is odd, then 32-bit words)
                     const int pad_end = min(pitch, (nw & ~(ROW_PAD - 1)) + 2 * ROW_PAD);
-                    for (int k = nw + lane; k < pad_end; k += 32) row[k] = 0;
+                    const int e0 = (nw + 1) & ~1;
+                    if (lane == 0 && e0 != nw && nw < pad_end) row[nw] = 0;
+                    if (e0 + 2 * lane < pad_end) reinterpret_cast<uint32_t *>(row)[(e0 >> 1) + lane] = 0u;
                     if (lane == 0) nlistn[gidx[p]] = nw;                      // l.22
                     wmax = max(wmax, total);
                 }

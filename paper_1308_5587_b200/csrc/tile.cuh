@@ -209,6 +209,54 @@ __device__ __forceinline__ void tile_stage_positions(const TileGeom &g, const Ti
     }
 }
 
+// The same result, one warp per halo cell (three cells in flight per warp): no search for the cell of a slot.
+// Fewer instructions, longer latency; the list build, whose blocks live long, uses this one.
+__device__ __forceinline__ void tile_stage_positions_by_cell(const TileGeom &g, const TileCtx &t, const TileShared &s,
+                                                             const float4 *__restrict__ pos, float4 *__restrict__ stage,
+                                                             int *__restrict__ src_out)
+{
+    constexpr int U = 3;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    const float wcell = g.L / (float)g.m, hL = 0.5f * g.L;
+    const bool fast = g.fast != 0;
+    if (threadIdx.x == 0) stage[0] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+    for (int h0 = warp; h0 < t.nh; h0 += U * nwarps) {
+        int s0[U], cnt[U], g0[U], kmax = 0;
+        float cx[U], cy[U], cz[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int h = h0 + u * nwarps;
+            s0[u] = 0; cnt[u] = 0; g0[u] = 0;
+            cx[u] = s.d.cx; cy[u] = s.d.cy; cz[u] = s.d.cz;
+            if (h < t.nh) {
+                s0[u] = s.hslot[h];
+                cnt[u] = s.hslot[h + 1] - s0[u];
+                g0[u] = s.hg[h];
+                if (!fast) {
+                    const int jx = h % t.hx, jy = (h / t.hx) % t.hy, jz = h / (t.hx * t.hy);
+                    cx[u] = __fmaf_rn((float)(t.x0 - 1 + jx) + 0.5f, wcell, -hL);
+                    cy[u] = __fmaf_rn((float)(t.y0 - 1 + jy) + 0.5f, wcell, -hL);
+                    cz[u] = __fmaf_rn((float)(t.z0 - 1 + jz) + 0.5f, wcell, -hL);
+                }
+            }
+            kmax = max(kmax, cnt[u]);
+        }
+        for (int k = lane; k < kmax; k += 32) {
+            float4 p[U];
+#pragma unroll
+            for (int u = 0; u < U; u++)
+                if (k < cnt[u]) p[u] = pos[g0[u] + k];
+#pragma unroll
+            for (int u = 0; u < U; u++)
+                if (k < cnt[u]) {
+                    stage[s0[u] + k] = make_float4(tile_image(p[u].x, cx[u], g.L, hL), tile_image(p[u].y, cy[u], g.L, hL),
+                                                   tile_image(p[u].z, cz[u], g.L, hL), p[u].w);
+                    if (src_out) src_out[s0[u] + k] = g0[u] + k;
+                }
+        }
+    }
+}
+
 // The same staging from the tables the list build left behind (fast geometry only): per slot one
 // coalesced index load, one position load, the image nearest to the tile centre.
 __device__ __forceinline__ void tile_stage_from_table(const TileDesc &d, const int *__restrict__ src_tab,

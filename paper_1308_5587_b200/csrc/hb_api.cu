@@ -9,7 +9,7 @@
 
 namespace {
 
-int coop_mode(const hb_system *h) { return h->tun.coop_rebuild >= 0 ? h->tun.coop_rebuild : 1; }
+int coop_mode(const hb_system *h) { return h->tun.coop_rebuild >= 0 ? h->tun.coop_rebuild : (h->N < 200000 ? 2 : 1); }
 int rebuild_kernels(const hb_system *h) { return coop_mode(h) == 2 ? 1 : coop_mode(h) == 1 ? 2 : 5; }  // see enqueue_rebuild
 
 int dev_alloc(hb_system *h, void **p, size_t bytes)

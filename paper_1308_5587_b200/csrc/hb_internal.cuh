@@ -24,6 +24,7 @@ enum {
     FL_BAR0 = 10,       // arrival counters of the cooperative rebuild kernel's grid barrier; build b uses
     FL_BAR1 = 11,       //   FL_BAR0 + (b & 1) and clears the other one
     FL_BAR_GEN = 12,    // b: launches of the cooperative kernel that got past their barriers
+    FL_TILE_CTR = 13,   // next tile of the cooperative kernel's list phase
     FL_COUNT = 16
 };
 
@@ -65,7 +66,7 @@ struct Tunables {
     int cell_sort = 1;
     int coop_blocks = 4;   // blocks per SM of the cooperative cell kernel (at most)
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
-    int coop_rebuild = 1;  // 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
+    int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 50;
 };

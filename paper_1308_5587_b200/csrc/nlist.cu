@@ -289,12 +289,21 @@ __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs 
     grid_barrier();
     const int lane = threadIdx.x & 31;
     for (int64_t c = gtid >> 5; c < ca.ncells; c += gsize >> 5) cell_gather_one(ca.cell_start, ca.perm, ga, do_sort, c, lane);
-    if (WITH_LIST) grid_barrier();
+    if (WITH_LIST) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_TILE_CTR] = 0;
+        grid_barrier();
+    }
     if (blockIdx.x == 0 && threadIdx.x == 0) flags[FL_BAR_GEN] = gen + 1;   // every block is past its first barrier
     if (WITH_LIST) {
-        for (int tile = blockIdx.x; tile < la.g.ntiles; tile += gridDim.x) {
+        // tiles are handed out on demand, like the hardware hands out blocks to the stand-alone list kernel
+        __shared__ int next_tile;
+        for (;;) {
+            if (threadIdx.x == 0) next_tile = atomicAdd(&flags[FL_TILE_CTR], 1);
+            __syncthreads();
+            const int tile = next_tile;
+            if (tile >= la.g.ntiles) break;
             nlist_tile_body<PPI>(la, tile, smem_raw);
-            __syncthreads();              // the next tile reuses the staging area
+            __syncthreads();              // the next tile reuses the staging area (and next_tile)
         }
     }
 }

@@ -91,7 +91,7 @@ def test_forces_energy_virial(hb, orc, case, shift):
                                  dict(nlist_ppi=1), dict(nlist_ppi=2), dict(cell_sort=0),
                                  dict(tile_x=1, tile_y=1, tile_z=1), dict(tile_x=2, tile_y=2, tile_z=2),
                                  dict(tile_x=3, tile_y=2, tile_z=1), dict(tile_x=4, tile_y=1, tile_z=2),
-                                 dict(tile_x=16, tile_y=2, tile_z=2), dict(stage_cap=64), dict(coop_rebuild=0), dict(coop_rebuild=2),
+                                 dict(tile_x=16, tile_y=2, tile_z=2), dict(stage_cap=64), dict(coop_rebuild=0), dict(coop_rebuild=1), dict(coop_rebuild=2),
                                  dict(force_block=256), dict(coop_rebuild=0, stage_cap=64), dict(nlist_block=128),
                                  dict(coop_rebuild=1, coop_blocks=4), dict(tpp=4, epl=4)])
 def test_tunables_do_not_change_results(hb, orc, tun):

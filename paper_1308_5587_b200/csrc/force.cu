@@ -16,10 +16,14 @@
 //     loads, shifted to the periodic image the tile sees: no minimum-image
 //     arithmetic per pair, and every neighbor gather is a 16-byte shared-memory
 //     load (list entries are 16-bit slots of this staging layout);
-//   * TPP threads share one particle; each reads EPL consecutive 16-bit entries
-//     with one 8- or 16-byte load (prefetched one iteration ahead), issues the EPL
-//     gathers back to back and evaluates the pairs without a branch: a pair
-//     outside r_cut gets r^-2 := 0, rows are padded with the far-away dummy slot;
+//   * the list build leaves a descriptor and a slot table per tile behind, so the
+//     staging here is: descriptor -> storage index of every slot -> position;
+//   * TPP threads share one particle (2 by default); each takes EPL (8) consecutive
+//     16-bit entries per iteration.  The rows arrive through a ring of four
+//     cp.async copies per thread, not through registers (see cp_async below); a row
+//     ends at its first padding entry, so no row length is read.  The EPL gathers
+//     are issued back to back and the pairs evaluated without a branch: a pair
+//     outside r_cut gets r^-2 := 0, the padding is the far-away dummy slot;
 //   * F, U, W are combined across the TPP lanes with warp shuffles;
 //   * when asked, the same thread finishes the velocity-Verlet step of its
 //     particle with the force it just computed (second half kick of this step,

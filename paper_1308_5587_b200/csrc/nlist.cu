@@ -4,8 +4,9 @@
 // unsynchronised row writes "a big bottleneck" that "GF100 does not have enough
 // shared memory to regularize".  Here ONE BLOCK OWNS ONE TILE of
 // cells (tile.cuh): the tile plus its one-cell halo is staged once in shared
-// memory, already shifted to the periodic image the tile sees, and then ONE WARP
-// OWNS ONE CELL of the tile:
+// memory (one warp per halo cell), already moved to the periodic image the tile sees,
+// and then ONE WARP OWNS ONE CELL of the tile (several warps split a cell's particles
+// when the tile has fewer cells than the block has warps):
 //   1. lanes 0..8 look up the nine x-rows of three adjacent cells (on the fly, no
 //      celladj table: PAPER.md:187 stored it to save registers) -- in the staged
 //      layout each row is one contiguous run of slots -- and the warp flattens the

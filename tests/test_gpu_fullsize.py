@@ -99,3 +99,27 @@ def test_fullsize_sampled_parity(hb, orc, case):
         g.compute_lj(w.shift)
         worst1, _ = _sampled_parity(hb, orc, w, g, out["pos"], s.type, s.L, rng)
     assert max(worst0, worst1) <= parity.F_TOL
+
+
+def test_four_million_particles(hb, orc):
+    """Beyond BASELINE's sizes: N = 160^3 = 4,096,000 (262,144 cells, 16,384 tiles, 128 scan tiles): the index
+    arithmetic, the cell scan across many scan tiles and the tables of the tile kernels at a size where a 32-bit
+    slip would show; sampled forces against brute force over all N after 30 steps with rebuilds and two sorts."""
+    w = wl.scaled(wl.CONFIGS["lj_64k"], 160 ** 3)
+    s = wl.make_state(w)
+    with hb.System.from_workload(w) as g:
+        g.set_state(s.pos, s.type, s.vel, s.image)
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(w.shift)
+        g.run_nve(w.dt, 30, 15)
+        st = g.stats()
+        out = g.get_state()
+        f4, w6 = g.get_forces()
+        th = g.thermo()
+    assert st["rebuilds"] >= 3 and st["sorts"] == 2 and st["overflow_retries"] == 0
+    assert np.array_equal(np.sort(out["order"]), np.arange(w.N))
+    assert max(abs(th["px"]), abs(th["py"]), abs(th["pz"])) / w.N < 1e-6
+    pos64 = out["pos"].astype(np.float64)
+    sample = np.sort(np.random.default_rng(7).choice(w.N, size=128, replace=False)).astype(np.int64)
+    F, U, W, A = orc.compute_lj_brute_sample(pos64, s.type, s.L, orc.Params.of(w), sample, band=parity.BAND)
+    parity.assert_forces_close(F, U, W, A, f4, w6, rows=sample)

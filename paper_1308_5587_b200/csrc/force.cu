@@ -195,6 +195,14 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
         }
         cp_async_wait<0>();                          // nothing of this pass may land after the next pass's copies start
         if (q0 + PPB < nown) prep(q0 + PPB, nown);   // they fly during the reduction and the integration below
+        // what the integration will need, all three loads in flight at once and behind the reduction (ncu: placed
+        // where they are used they were three L2 round trips in a row at the very end of the block; issued before
+        // the pair loop they cost registers the loop needs)
+        float4 v_in = make_float4(0.f, 0.f, 0.f, 0.f), p_in = v_in, pb_in = v_in;
+        if (do_nve && active && sub == 0) {
+            v_in = nv.vel[gi];
+            if (nv.kick_drift) { p_in = pos[gi]; pb_in = nv.pos_build[gi]; }
+        }
 
 #pragma unroll
         for (int o = TPP >> 1; o > 0; o >>= 1) {
@@ -215,7 +223,7 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
             force[gi] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
             if (do_nve) {
                 // reading c7, operation by operation as nve_kernel does it
-                float4 v = nv.vel[gi];
+                float4 v = v_in;
                 if (nv.kick_prev) {
                     v.x = __fmaf_rn(hdt, a.fx, v.x);
                     v.y = __fmaf_rn(hdt, a.fy, v.y);
@@ -225,7 +233,7 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
                     v.x = __fmaf_rn(hdt, a.fx, v.x);
                     v.y = __fmaf_rn(hdt, a.fy, v.y);
                     v.z = __fmaf_rn(hdt, a.fz, v.z);
-                    float4 p = pos[gi];   // the stored position: pi may be another periodic image of it
+                    float4 p = p_in;      // the stored position: pi may be another periodic image of it
                     p.x = __fmaf_rn(nv.dt, v.x, p.x);
                     p.y = __fmaf_rn(nv.dt, v.y, p.y);
                     p.z = __fmaf_rn(nv.dt, v.z, p.z);
@@ -234,7 +242,7 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
                     if (p.z >= hL) { p.z -= L; nv.image[2 * (int64_t)N + gi] += 1; }
                     else if (p.z < -hL) { p.z += L; nv.image[2 * (int64_t)N + gi] -= 1; }
                     nv.pos_out[gi] = p;
-                    const float4 pb = nv.pos_build[gi];
+                    const float4 pb = pb_in;
                     float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
                     if (dx >= hL) dx -= L; else if (dx < -hL) dx += L;
                     if (dy >= hL) dy -= L; else if (dy < -hL) dy += L;

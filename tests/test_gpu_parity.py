@@ -358,3 +358,42 @@ def test_launch_variants_give_bitwise_identical_trajectories(hb):
         assert nb == ref[5], (tun, nb, ref[5])
         assert np.array_equal(pos, ref[1]) and np.array_equal(vel, ref[2]) and np.array_equal(img, ref[3]), tun
         assert np.array_equal(f4, ref[4]), tun
+
+
+def test_two_particles_against_the_hand_worked_values(hb):
+    """The CUDA path against tests/golden/lj_closed_form.txt (exact rationals worked by hand from PAPER.md:318),
+    without the oracle in between: two particles at distance r along a diagonal that crosses a corner of the box."""
+    import os
+    from fractions import Fraction
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "lj_closed_form.txt")) as f:
+        for ln in f:
+            if ln.strip() and not ln.startswith("#"):
+                a = [int(x) for x in ln.split()]
+                rows.append((Fraction(a[0], a[1]), Fraction(a[2], a[3]), Fraction(a[4], a[5])))
+    L = float(np.float32(20.0))
+    for r, V, F in rows:
+        d = float(r) / np.sqrt(3.0)
+        # the pair straddles the corner (+L/2, +L/2, +L/2): particle 1 is seen through three periodic faces
+        p0 = np.array([L / 2 - d / 2] * 3)
+        p1 = p0 + d - L
+        pos = np.array([p0, p1], dtype=np.float32)
+        with hb.System(2, L, 1, [1.0], [1.0]) as g:
+            g.set_state(pos, np.zeros(2, dtype=np.int32), np.zeros_like(pos))
+            g.build_nlist(3.0, 0.4)
+            g.compute_lj(0)                       # no shift: V is V_lj itself
+            f4, w6 = g.get_forces()
+            rs, nbr = g.get_nlist()
+        assert np.diff(rs).tolist() == [1, 1] and nbr.tolist() == [1, 0]
+        # fp32 positions: the realised distance differs from r by ~1e-6; compare with the derivative-scaled tolerance
+        dvec = pos[0].astype(np.float64) - pos[1].astype(np.float64) - L      # minimum image of R_0 - R_1
+        rr = np.linalg.norm(dvec)
+        tolF = 1e-5 * max(1.0, abs(float(F))) + abs(float(F)) * 14 * abs(rr - float(r)) / float(r)
+        Fmag = float(np.linalg.norm(f4[0, :3].astype(np.float64)))
+        sign = 1.0 if np.dot(f4[0, :3].astype(np.float64), dvec) > 0 else -1.0     # repulsive = along R_0 - R_1
+        assert abs(sign * Fmag - float(F)) <= tolF, (r, sign * Fmag, float(F))
+        assert np.allclose(f4[0, :3], -f4[1, :3], rtol=0, atol=1e-6 * max(1.0, Fmag))      # Newton III
+        tolV = 1e-5 * max(1.0, abs(float(V))) + abs(float(F)) * abs(rr - float(r)) * 2
+        assert abs(2.0 * float(f4[0, 3]) - float(V)) <= tolV, (r, 2 * f4[0, 3], float(V))  # U_i = V / 2 each
+        # virial: W_i = 1/2 d (x) f, trace = 1/2 r F
+        assert abs(float(w6[0, 0] + w6[0, 3] + w6[0, 5]) - 0.5 * rr * sign * Fmag) <= 1e-4 * max(1.0, abs(float(F)))

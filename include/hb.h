@@ -176,6 +176,7 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *                    (tx+2)(ty+2)(tz+2) <= 256 and ty*tz <= 32 after clipping to m.
  *   "stage_cap"      shared-memory slots per tile (0 = from the density); grown on overflow
  *   "row_pitch"      initial entries per list row (rounded up to 64; 0 = estimate)
+ *   "grow_pct"       head room in percent when rows / the staging area are grown after an overflow (25)
  *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
  *   "force_block"    threads per block of the force kernel: 128, 256
  *   "nlist_block"    threads per block of the stand-alone list kernel: 128, 256

@@ -306,7 +306,7 @@ int build_nlist_sync(hb_system *h)
             h->stats.overflow_retries++;
             HB_TRY(set_flag(h, FL_STAGE_OVER, 0));
             HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
-            HB_TRY(choose_tiles(h, (int)(needed * 1.2) + 32));
+            HB_TRY(choose_tiles(h, (int)(needed * (1.0 + 0.01 * h->tun.grow_pct)) + 32));
             continue;
         }
         h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
@@ -317,7 +317,7 @@ int build_nlist_sync(hb_system *h)
             return HB_OK;
         }
         h->stats.overflow_retries++;
-        HB_TRY(ensure_rows(h, (int)(h->h_flags[FL_MAX_NBRS] * 1.25) + 8));
+        HB_TRY(ensure_rows(h, (int)(h->h_flags[FL_MAX_NBRS] * (1.0 + 0.01 * h->tun.grow_pct)) + 8));
     }
     h->err = "neighbor-list rows keep overflowing";
     return HB_ENOMEM;
@@ -659,8 +659,8 @@ int run_chunk(hb_system *h, float dt, int n)
         HB_TRY(restore_state(h));
         HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
         HB_TRY(set_flag(h, FL_STAGE_OVER, 0));
-        if (slots_needed) HB_TRY(choose_tiles(h, (int)(slots_needed * 1.2) + 32));
-        if (rows_needed) HB_TRY(ensure_rows(h, (int)(rows_needed * 1.25) + 8));
+        if (slots_needed) HB_TRY(choose_tiles(h, (int)(slots_needed * (1.0 + 0.01 * h->tun.grow_pct)) + 32));
+        if (rows_needed) HB_TRY(ensure_rows(h, (int)(rows_needed * (1.0 + 0.01 * h->tun.grow_pct)) + 8));
         HB_TRY(build_nlist_sync(h));
     }
     h->err = "neighbor-list rows keep overflowing inside hb_run_nve";
@@ -1165,6 +1165,7 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "row_pitch")) return &h->tun.row_pitch;
     if (!strcmp(name, "cell_sort")) return &h->tun.cell_sort;
     if (!strcmp(name, "fuse_nve")) return &h->tun.fuse_nve;
+    if (!strcmp(name, "grow_pct")) return &h->tun.grow_pct;
     if (!strcmp(name, "coop_rebuild")) return &h->tun.coop_rebuild;
     if (!strcmp(name, "coop_blocks")) return &h->tun.coop_blocks;
     if (!strcmp(name, "graph_mode")) return &h->tun.graph_mode;
@@ -1189,6 +1190,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve) ok = value == 0 || value == 1;
     else if (slot == &h->tun.coop_rebuild) ok = value >= -1 && value <= 2;
     else if (slot == &h->tun.coop_blocks) ok = value >= 1 && value <= 8;
+    else if (slot == &h->tun.grow_pct) ok = value >= 0 && value <= 400;
     else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 3;
     else if (slot == &h->tun.graph_steps) ok = value >= 1 && value <= 2000;
     if (!ok) { h->err = std::string("value out of range for tunable ") + name; return HB_EINVAL; }

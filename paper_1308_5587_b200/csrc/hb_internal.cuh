@@ -63,6 +63,7 @@ struct Tunables {
     int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
     int stage_cap = 0;     // 0 = estimated from the density
     int row_pitch = 0;
+    int grow_pct = 25;     // head room given when rows or the staging area are grown after an overflow
     int cell_sort = 1;
     int coop_blocks = 4;   // blocks per SM of the cooperative cell kernel (at most)
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel

@@ -397,3 +397,47 @@ def test_two_particles_against_the_hand_worked_values(hb):
         assert abs(2.0 * float(f4[0, 3]) - float(V)) <= tolV, (r, 2 * f4[0, 3], float(V))  # U_i = V / 2 each
         # virial: W_i = 1/2 d (x) f, trace = 1/2 r F
         assert abs(float(w6[0, 0] + w6[0, 3] + w6[0, 5]) - 0.5 * rr * sign * Fmag) <= 1e-4 * max(1.0, abs(float(F)))
+
+
+def test_overflow_inside_a_graph_chunk_is_redone(hb):
+    """PAPER.md:97 inside hb_run_nve.  A dilute lattice (26 listed neighbors, rows of 64 entries suffice) whose four
+    quadrants stream towards the z axis: the density there rises about fourfold, rows and staging areas overflow in
+    builds that happen INSIDE captured chunks; each such chunk is rolled back to its saved start, the arrays grow and
+    the chunk is redone.  The result must be bit for bit the trajectory of a system that had room from the start."""
+    n = 16
+    N = n ** 3
+    L = float(np.float32((N / 0.2) ** (1.0 / 3.0)))
+    g1 = (np.arange(n) + 0.5) * (L / n) - L / 2
+    pos = np.stack(np.meshgrid(g1, g1, g1, indexing="ij"), -1).reshape(-1, 3).astype(np.float32)
+    vel = np.zeros_like(pos)
+    vel[:, 0] = -1.5 * np.sign(pos[:, 0])
+    vel[:, 1] = -1.5 * np.sign(pos[:, 1])
+    typ = np.zeros(N, dtype=np.int32)
+    res = []
+    for tun in (dict(row_pitch=64), dict(row_pitch=1024, stage_cap=12000)):
+        with hb.System(N, L, 1, [1.0], [1.0]) as g:
+            for k, v in tun.items():
+                g.set_tunable(k, v)
+            g.set_state(pos, typ, vel)
+            g.build_nlist(3.0, 0.4)
+            g.compute_lj(1)
+            st0 = g.stats()
+            th0 = g.thermo()
+            g.run_nve(0.005, 1200, 0)
+            st1 = g.stats()
+            out = g.get_state()
+            th = g.thermo()
+            res.append((st0, st1, out["pos"].copy(), out["order"].copy(), th, th0["K"] + th0["U"]))
+    (a0, a1, pa, oa, ta, Ea0), (b0, b1, pb, ob, tb, Eb0) = res
+    assert a0["row_pitch"] == 64 and a0["overflow_retries"] == 0 and a0["max_nbrs"] <= 32
+    assert b1["overflow_retries"] == 0, "the roomy system was meant never to overflow"
+    assert a1["overflow_retries"] >= 1 and a1["row_pitch"] > 64, a1      # the rows grew during the run
+    assert a1["steps"] == 1200 and b1["steps"] == 1200 and np.isfinite(pa).all()
+    for o in (oa, ob):
+        assert np.array_equal(np.sort(o), np.arange(N)), "a particle was lost or duplicated"
+    Ea, Eb = ta["K"] + ta["U"], tb["K"] + tb["U"]
+    K0 = 0.5 * float((vel.astype(np.float64) ** 2).sum())
+    assert Ea0 == Eb0
+    assert abs(Ea - Eb) <= 2e-4 * K0 and abs(Ea - Ea0) <= 5e-3 * K0 and abs(Eb - Eb0) <= 5e-3 * K0, (Ea, Eb, Ea0, K0)
+    for t in (ta, tb):
+        assert max(abs(t["px"]), abs(t["py"]), abs(t["pz"])) / N < 1e-5

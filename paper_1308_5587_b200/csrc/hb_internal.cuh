@@ -69,7 +69,7 @@ struct Tunables {
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
     int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
-    int graph_steps = 50;
+    int graph_steps = 100;
 };
 
 struct hb_system {

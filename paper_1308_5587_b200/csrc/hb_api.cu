@@ -548,15 +548,11 @@ int backup_state(hb_system *h)
     if (!h->bk_pos) {
         HB_TRY(dev_alloc_t(h, &h->bk_pos, N));
         HB_TRY(dev_alloc_t(h, &h->bk_vel, N));
-        HB_TRY(dev_alloc_t(h, &h->bk_force, N));
-        HB_TRY(dev_alloc_t(h, &h->bk_virial, 2 * N));
         HB_TRY(dev_alloc_t(h, &h->bk_image, 3 * N));
         HB_TRY(dev_alloc_t(h, &h->bk_tag, N));
     }
     HB_CK(cudaMemcpyAsync(h->bk_pos, h->pos(), N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_vel, h->vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->bk_force, h->force, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->bk_virial, h->virial, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_image, h->image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_tag, h->tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
     h->bk_cur = h->cur;
@@ -572,13 +568,12 @@ int restore_state(hb_system *h)
     h->parity = h->bk_parity;
     HB_CK(cudaMemcpyAsync(h->pos(), h->bk_pos, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->vel, h->bk_vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->force, h->bk_force, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->virial, h->bk_virial, 2 * N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->image, h->bk_image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->tag, h->bk_tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(launch_rtag(h));
     HB_TRY(clear_need_flags(h));
-    h->nlist_valid = h->cells_valid = false;
+    // forces and virials are not saved: the rebuild that follows a restore changes the order, they are recomputed
+    h->nlist_valid = h->cells_valid = h->forces_valid = false;
     h->moved = true;
     return HB_OK;
 }

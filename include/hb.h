@@ -180,6 +180,8 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
  *   "force_block"    threads per block of the force kernel: 128, 256
  *   "nlist_block"    threads per block of the stand-alone list kernel: 128, 256
+ *   "thermo_every"   1 = U_i and W_i are computed every step (default, the paper's kernel);
+ *                    0 = inside hb_run_nve only by the last step of each chunk (they cannot be read before)
  *   "fuse_nve"       1 = hb_run_nve integrates inside the force kernel (one kernel per step)
  *   "coop_rebuild"   0 = the rebuild is five launches (count, scan, scatter, gather, list);
  *                    1 = Algorithm 2 and the reorder are ONE cooperative kernel, then the list kernel;

@@ -57,6 +57,7 @@ struct Acc {
     float fx, fy, fz, u, wxx, wxy, wxz, wyy, wyz, wzz;
 };
 
+template <bool THERMO>
 __device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, const PairParam &pp, Acc &a)
 {
     const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;   // pj is already the nearest image
@@ -65,9 +66,11 @@ __device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, co
     const float r2inv = in ? rcp_approx(r2) : 0.0f;    // 0 switches the whole pair off
     const float r6inv = r2inv * r2inv * r2inv;
     const float fdivr = r2inv * r6inv * __fmaf_rn(12.0f * pp.lj1, r6inv, -6.0f * pp.lj2);
+    // explicit roundings: the force sums must not depend on whether the energy and virial terms are compiled in
+    const float px = __fmul_rn(fdivr, dx), py = __fmul_rn(fdivr, dy), pz = __fmul_rn(fdivr, dz);
+    a.fx = __fadd_rn(a.fx, px); a.fy = __fadd_rn(a.fy, py); a.fz = __fadd_rn(a.fz, pz);
+    if (!THERMO) return;   // an inner step of hb_run_nve with thermo_every = 0: nobody can read U_i, W_i of this step
     const float e = __fmaf_rn(r6inv, __fmaf_rn(pp.lj1, r6inv, -pp.lj2), in ? -pp.eshift : 0.0f);
-    const float px = fdivr * dx, py = fdivr * dy, pz = fdivr * dz;
-    a.fx += px; a.fy += py; a.fz += pz;
     a.u += e;
     a.wxx = __fmaf_rn(dx, px, a.wxx); a.wxy = __fmaf_rn(dx, py, a.wxy); a.wxz = __fmaf_rn(dx, pz, a.wxz);
     a.wyy = __fmaf_rn(dy, py, a.wyy); a.wyz = __fmaf_rn(dy, pz, a.wyz); a.wzz = __fmaf_rn(dz, pz, a.wzz);
@@ -93,7 +96,7 @@ __device__ __forceinline__ void unpack_entries(const Entries<EPL> &e, int (&sl)[
     if constexpr (EPL == 8) { sl[4] = e.v.z & 0xffffu; sl[5] = e.v.z >> 16; sl[6] = e.v.w & 0xffffu; sl[7] = e.v.w >> 16; }
 }
 
-template <int TPP, int EPL, bool ONE_TYPE>
+template <int TPP, int EPL, bool ONE_TYPE, bool THERMO>
 __global__ void __launch_bounds__(TILE_THREADS, 4)   // <= 64 registers: 8 blocks of 128 threads per SM
 lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__restrict__ pos,
                const uint16_t *__restrict__ nlist, const int *__restrict__ nlistn, int pitch, int N, int ntypes,
@@ -188,8 +191,8 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
                 ent.v = ring[c * ring_stride];                           // arithmetic so that its latency hides behind it
 #pragma unroll
                 for (int e = 0; e < EPL; e++) {
-                    if (ONE_TYPE) pair_term(pi, pj[e], pp1, a);
-                    else pair_term(pi, pj[e], prow[__float_as_int(pj[e].w)], a);
+                    if (ONE_TYPE) pair_term<THERMO>(pi, pj[e], pp1, a);
+                    else pair_term<THERMO>(pi, pj[e], prow[__float_as_int(pj[e].w)], a);
                 }
             }
         }
@@ -209,13 +212,15 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
             a.fx += __shfl_xor_sync(0xffffffffu, a.fx, o);
             a.fy += __shfl_xor_sync(0xffffffffu, a.fy, o);
             a.fz += __shfl_xor_sync(0xffffffffu, a.fz, o);
-            a.u += __shfl_xor_sync(0xffffffffu, a.u, o);
-            a.wxx += __shfl_xor_sync(0xffffffffu, a.wxx, o);
-            a.wxy += __shfl_xor_sync(0xffffffffu, a.wxy, o);
-            a.wxz += __shfl_xor_sync(0xffffffffu, a.wxz, o);
-            a.wyy += __shfl_xor_sync(0xffffffffu, a.wyy, o);
-            a.wyz += __shfl_xor_sync(0xffffffffu, a.wyz, o);
-            a.wzz += __shfl_xor_sync(0xffffffffu, a.wzz, o);
+            if (THERMO) {
+                a.u += __shfl_xor_sync(0xffffffffu, a.u, o);
+                a.wxx += __shfl_xor_sync(0xffffffffu, a.wxx, o);
+                a.wxy += __shfl_xor_sync(0xffffffffu, a.wxy, o);
+                a.wxz += __shfl_xor_sync(0xffffffffu, a.wxz, o);
+                a.wyy += __shfl_xor_sync(0xffffffffu, a.wyy, o);
+                a.wyz += __shfl_xor_sync(0xffffffffu, a.wyz, o);
+                a.wzz += __shfl_xor_sync(0xffffffffu, a.wzz, o);
+            }
         }
         if (!active) continue;
         // U_i = 1/2 sum V, W_i = 1/2 sum d f (reading c6.i)
@@ -251,12 +256,12 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
                 }
                 nv.vel[gi] = v;
             }
-        } else if (TPP >= 4 && sub == 1) {
+        } else if (THERMO && TPP >= 4 && sub == 1) {
             virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
-        } else if (TPP >= 4 && sub == 2) {
+        } else if (THERMO && TPP >= 4 && sub == 2) {
             virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
         }
-        if (TPP < 4 && sub == TPP - 1) {
+        if (THERMO && TPP < 4 && sub == TPP - 1) {
             virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
             virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
         }
@@ -287,8 +292,8 @@ size_t force_smem_bytes(const hb_system *h)
            (size_t)4 * 16 * force_block_of(h);
 }
 
-template <int TPP, int EPL>
-static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
+template <int TPP, int EPL, bool THERMO>
+static cudaError_t launch_force_tt(hb_system *h, const NveArgs *nve)
 {
     const size_t smem = force_smem_bytes(h);
     const unsigned grid = (unsigned)h->geom.ntiles;
@@ -296,9 +301,9 @@ static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
     if (nve) nv = *nve;
     cudaError_t e;
 #define LJ_LAUNCH(ONE)                                                                                                      \
-    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
     if (e != cudaSuccess) return e;                                                                                         \
-    lj_tile_kernel<TPP, EPL, ONE><<<grid, force_block_of(h), smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
+    lj_tile_kernel<TPP, EPL, ONE, THERMO><<<grid, force_block_of(h), smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
                                                                            h->nlistn, h->row_pitch, (int)h->N, h->ntypes,  \
                                                                            h->params, h->force, h->virial, h->flags,       \
                                                                            nve ? 1 : 0, nv, h->stage_src,                  \
@@ -307,6 +312,15 @@ static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
 #undef LJ_LAUNCH
     h->stats.kernel_launches++;
     return cudaGetLastError();
+}
+
+template <int TPP, int EPL>
+static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
+{
+    // energies and virials of a step can only be read after hb_run_nve returns: with thermo_every = 0 the inner
+    // steps of a chunk (both half kicks fused in) compute forces only
+    if (nve && nve->forces_only) return launch_force_tt<TPP, EPL, false>(h, nve);
+    return launch_force_tt<TPP, EPL, true>(h, nve);
 }
 
 cudaError_t launch_force(hb_system *h, const NveArgs *nve)

@@ -391,6 +391,7 @@ NveArgs make_nve(hb_system *h, float dt, bool kick_prev, bool kick_drift, float4
     a.half_buff2 = hb * hb;
     a.kick_prev = kick_prev ? 1 : 0;
     a.kick_drift = kick_drift ? 1 : 0;
+    a.forces_only = (kick_prev && kick_drift && h->tun.thermo_every == 0) ? 1 : 0;
     a.need_set = FL_NEED0 + (h->parity & 1);
     a.need_clear = FL_NEED0 + ((h->parity + 1) & 1);
     a.cond = cond;
@@ -1137,7 +1138,7 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
     if (tg) cudaGraphDestroy(tg);
     dev_free(h, scratch);
     if (rc == HB_OK) rc = clear_need_flags(h);
-    if (rc == HB_OK && (which == 2 || which == 3 || which == 6)) {
+    if (rc == HB_OK && (which == 2 || which == 3 || which == 6 || (which == 5 && h->tun.thermo_every == 0))) {
         // the timed cell builds re-ordered the scratch set (and, for "rebuild", the particles): make the list whole again
         h->nlist_valid = false;
         rc = ensure_forces(h);
@@ -1160,6 +1161,7 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "row_pitch")) return &h->tun.row_pitch;
     if (!strcmp(name, "cell_sort")) return &h->tun.cell_sort;
     if (!strcmp(name, "fuse_nve")) return &h->tun.fuse_nve;
+    if (!strcmp(name, "thermo_every")) return &h->tun.thermo_every;
     if (!strcmp(name, "grow_pct")) return &h->tun.grow_pct;
     if (!strcmp(name, "coop_rebuild")) return &h->tun.coop_rebuild;
     if (!strcmp(name, "coop_blocks")) return &h->tun.coop_blocks;
@@ -1182,7 +1184,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     else if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z) ok = value >= 0 && value <= 16;
     else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;
     else if (slot == &h->tun.row_pitch) ok = value >= 0 && value <= 4096;
-    else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve) ok = value == 0 || value == 1;
+    else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve || slot == &h->tun.thermo_every) ok = value == 0 || value == 1;
     else if (slot == &h->tun.coop_rebuild) ok = value >= -1 && value <= 2;
     else if (slot == &h->tun.coop_blocks) ok = value >= 1 && value <= 8;
     else if (slot == &h->tun.grow_pct) ok = value >= 0 && value <= 400;

@@ -66,6 +66,7 @@ struct Tunables {
     int grow_pct = 25;     // head room given when rows or the staging area are grown after an overflow
     int cell_sort = 1;
     int coop_blocks = 4;   // blocks per SM of the cooperative cell kernel (at most)
+    int thermo_every = 1;  // 1: U_i and W_i every step (the paper's kernel); 0: only in the last step of a chunk of hb_run_nve
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
     int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
@@ -192,6 +193,7 @@ struct NveArgs {
     float4 *pos_out;       // where the drifted positions go (== pos_in for the stand-alone kernel)
     float dt, half_buff2;
     int kick_prev, kick_drift;
+    int forces_only;       // fused step whose U_i, W_i nobody can read: skip them
     int need_set, need_clear;   // flag indices
     cudaGraphConditionalHandle cond;
     int use_cond;

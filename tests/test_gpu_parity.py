@@ -340,7 +340,7 @@ def test_launch_variants_give_bitwise_identical_trajectories(hb):
     outs = []
     variants = [dict(), dict(graph_mode=3), dict(graph_mode=2), dict(graph_mode=0), dict(fuse_nve=0), dict(coop_rebuild=0),
                 dict(coop_rebuild=1), dict(coop_rebuild=2), dict(nlist_block=128), dict(nlist_ppi=2), dict(force_block=256),
-                dict(tile_x=2, tile_y=2, tile_z=2), dict(tile_x=1, tile_y=1, tile_z=1)]
+                dict(thermo_every=0), dict(tile_x=2, tile_y=2, tile_z=2), dict(tile_x=1, tile_y=1, tile_z=1)]
     for tun in variants:
         with _system(hb, w, s, **tun) as g:
             g.build_nlist(0.0, w.r_buff)

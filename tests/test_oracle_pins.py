@@ -269,15 +269,65 @@ def test_force_sums_newton_energy_virial(orc, name, N):
 
 def test_cutoff_flip_allowance(orc):
     """c6.ii: a pair placed 1e-6 inside / outside r_cut shows up in the allowance
-    with the size of the force jump |f(r_cut)| = 0.01094 at r_cut = 3."""
+    with the size of the force jump |f(r_cut)| = 0.01094 at r_cut = 3,
+    of the energy jump |V_lj(3)| / 2 = 5.479441744e-3 / 2 (only without
+    the energy shift, which makes V continuous) and of the virial jump r_c |f| / 2.
+    Hand values: F(3) = 48/3^13 - 24/3^7, V(3) = 4 (3^-12 - 3^-6)."""
     L = 20.0
-    p = orc.Params(1, [1.0], [1.0], [3.0], 1)
-    for dr in (-1e-6, 1e-6):
-        pos = np.array([[0, 0, 0], [3.0 + dr, 0, 0]])
-        c, r, n = orc.nlist_brute(pos, L, 3.4)
-        F, U, W, A = orc.compute_lj_nlist(pos, np.zeros(2, dtype=np.int32), L, p, c, r, n, band=1e-5)
-        assert A[0, 0] == pytest.approx(0.01094, rel=2e-3)
-        assert (abs(F[0, 0]) > 0.0109) == (dr < 0)
+    F3 = abs(48.0 / 3 ** 13 - 24.0 / 3 ** 7)
+    V3 = abs(4.0 * (3.0 ** -12 - 3.0 ** -6))
+    assert F3 == pytest.approx(0.01094, rel=1e-3) and V3 == pytest.approx(5.479441744e-3, rel=1e-9)
+    for shift in (0, 1):
+        p = orc.Params(1, [1.0], [1.0], [3.0], shift)
+        for dr in (-1e-6, 1e-6):
+            pos = np.array([[0, 0, 0], [3.0 + dr, 0, 0]])
+            c, r, n = orc.nlist_brute(pos, L, 3.4)
+            F, U, W, A = orc.compute_lj_nlist(pos, np.zeros(2, dtype=np.int32), L, p, c, r, n, band=1e-5)
+            assert A[0, 0] == pytest.approx(F3, rel=1e-6)
+            assert A[0, 1] == pytest.approx(0.0 if shift else 0.5 * V3, rel=1e-6, abs=1e-12)
+            assert A[0, 2] == pytest.approx(0.5 * 3.0 * F3, rel=1e-6)
+            assert np.array_equal(A[0], A[1])
+            assert (abs(F[0, 0]) > 0.0109) == (dr < 0)
+            # the brute-force sampler records the same allowances
+            Fs, Us, Ws, As = orc.compute_lj_brute_sample(pos, np.zeros(2, dtype=np.int32), L, p, [1, 0], band=1e-5)
+            assert np.array_equal(As, A[[1, 0]]) and np.array_equal(Fs, F[[1, 0]])
+    # a pair well away from the cutoff leaves no allowance
+    pos = np.array([[0, 0, 0], [2.9, 0, 0]])
+    c, r, n = orc.nlist_brute(pos, L, 3.4)
+    A = orc.compute_lj_nlist(pos, np.zeros(2, dtype=np.int32), L, orc.Params(1, [1.0], [1.0], [3.0], 0), c, r, n, band=1e-5)[3]
+    assert not A.any()
+
+
+@pytest.mark.parametrize("name,N", [("lj_64k", 1500), ("wca_256k", 1400), ("ka_1m", 1600)])
+def test_sampled_brute_force_equals_full_brute_force(orc, name, N):
+    """c2, c6: the row-restricted functions that carry the full-size GPU parity
+    (orc_nlist_brute_sample, orc_compute_lj_brute_sample) give exactly the rows of
+    the O(N^2) definitions.  The sample is UNSORTED and repetition-free, so that an
+    output indexed by the particle instead of by the sample position (or the other
+    way round) fails; band = 0 and band = 1e-5 must give the same F, U, W."""
+    w = wl.scaled(wl.CONFIGS[name], N)
+    s = wl.make_state(w, seed=11)
+    pos = s.pos.astype(np.float64)
+    p = orc.Params.of(w)
+    rng = np.random.default_rng(3)
+    sample = rng.permutation(N)[:97].astype(np.int64)
+    assert np.any(np.diff(sample) < 0) and sample[0] != 0
+    cnt, rs, nbr = orc.nlist_brute(pos, s.L, w.r_max)
+    cs, rss, nbs = orc.nlist_brute_sample(pos, s.L, w.r_max, sample)
+    assert np.array_equal(cs, cnt[sample])
+    for k, i in enumerate(sample):
+        assert np.array_equal(nbs[rss[k]:rss[k + 1]], nbr[rs[i]:rs[i + 1]])
+    F, U, W = orc.compute_lj_brute(pos, s.type, s.L, p)
+    for band in (0.0, 1e-5):
+        Fs, Us, Ws, As = orc.compute_lj_brute_sample(pos, s.type, s.L, p, sample, band=band)
+        assert np.abs(Fs - F[sample]).max() <= 1e-13 * np.abs(F).max()
+        assert np.abs(Us - U[sample]).max() <= 1e-13 * np.abs(U).max()
+        assert np.abs(Ws - W[sample]).max() <= 1e-13 * np.abs(W).max()
+        if band == 0.0:
+            assert not As.any()
+    # and the list-restricted sums agree with the same definition (all particles)
+    Fl, Ul, Wl, _ = orc.compute_lj_nlist(pos, s.type, s.L, p, cnt, rs, nbr)
+    assert np.abs(Fl - F).max() <= 1e-12 * np.abs(F).max()
 
 
 # ----------------------------------------------------------------- c3, c7 ---
@@ -409,6 +459,31 @@ def test_hilbert_is_a_bijection_with_adjacent_steps(orc, B):
     for k in range(G ** 3 - 1):
         a, b = keys[k], keys[k + 1]
         assert sum(abs(u - v) for u, v in zip(a, b)) == 1
+
+
+def test_hilbert_b8_is_a_bijection_with_adjacent_steps(orc):
+    """c8 at the B = 8 the sort uses: all 2^24 grid cells through orc_sfc_keys (cell
+    centres of a box of edge 256 are exact in binary32): every key 0..2^24-1 once, and
+    consecutive keys are face-adjacent cells.  A slip in the transcription of the curve
+    that only shows beyond B = 4 (the exhaustive Python pin above) fails here."""
+    G = 256
+    g = np.arange(G, dtype=np.float32) + np.float32(0.5 - G / 2)
+    pos = np.empty((G, G, G, 3), dtype=np.float32)
+    pos[..., 0] = g[:, None, None]
+    pos[..., 1] = g[None, :, None]
+    pos[..., 2] = g[None, None, :]
+    key = orc.sfc_keys(pos.reshape(-1, 3), float(G), 8)
+    del pos
+    assert key.dtype == np.uint32 and int(key.max()) == G ** 3 - 1
+    inv = np.full(G ** 3, -1, dtype=np.int64)
+    inv[key] = np.arange(G ** 3, dtype=np.int64)          # flat index x * G^2 + y * G + z of the cell with that key
+    assert inv.min() >= 0, "a key is missing, i.e. another one is repeated"
+    x, y, z = inv // (G * G), (inv // G) % G, inv % G
+    step = np.abs(np.diff(x)) + np.abs(np.diff(y)) + np.abs(np.diff(z))
+    assert np.all(step == 1)
+    # spot values of the scalar function agree with the vectorised path
+    for k in (0, 1, 12345, G ** 3 - 1):
+        assert orc.hilbert_key(int(x[k]), int(y[k]), int(z[k]), 8) == k
 
 
 def test_sfc_sort_permutation(orc):

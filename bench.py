@@ -37,9 +37,12 @@ from paper_1308_5587_b200 import workloads as wl  # noqa: E402
 
 METRIC = "lj_liquid_timesteps_per_s"
 UNIT = "timesteps/s"
-# FP32 peak for the "alu" roofline (DESIGN.md section "Rooflines"): 148 SMs x 128 FP32
-# lanes x 2 flop/FMA x 1.965 GHz (clocks.max.sm, B200_PROFILING.md table).
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# Nominal FP32 peak, for context beside the measured one (DESIGN.md section "Rooflines"): 148 SMs x 128 FP32
+# lanes x 2 flop/FMA x 1.965 GHz (clocks.max.sm, B200_PROFILING.md table).  The roofline fractions below use
+# the peaks hb_measure_peak measures in this very run (FFMA chains, L2 reads, shared-memory loads).
+FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+ISSUE_SLOTS_PER_S = 148 * 128 * 1.965e9        # thread-instructions per second at one warp instruction per scheduler per cycle
+SMEM_NOMINAL_GBS = 148 * 128 * 1.965e9 / 1e9   # 128 B per cycle per SM
 PAPER_TITAN_STEPS_PER_S = 1270.0   # PAPER.md:143, GK110, same N=64000 workload shape (context)
 
 
@@ -84,15 +87,24 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
-def cpu_oracle_steps_per_s(w, state, nsteps):
-    """The oracle as it stands, timed on this box's host cores."""
+def cpu_oracle_steps_per_s(w, state, nsteps, threads=None):
+    """The oracle as it stands, timed on this box's host cores (threads = None: all of them)."""
+    import ctypes
     from oracle import orc
     p = orc.Params.of(w)
     orc.lib()
-    t0 = time.perf_counter()
-    out = orc.run_nve(state.pos, state.vel, state.image, state.type, state.L, p, w.r_buff, w.dt, nsteps)
-    dt = time.perf_counter() - t0
-    return nsteps / dt, dt, orc.num_threads(), out["builds"]
+    all_threads = orc.num_threads()
+    gomp = ctypes.CDLL("libgomp.so.1")
+    if threads is not None:
+        gomp.omp_set_num_threads(int(threads))
+    try:
+        used = orc.num_threads()
+        t0 = time.perf_counter()
+        out = orc.run_nve(state.pos, state.vel, state.image, state.type, state.L, p, w.r_buff, w.dt, nsteps)
+        dt = time.perf_counter() - t0
+    finally:
+        gomp.omp_set_num_threads(all_threads)
+    return nsteps / dt, dt, used, out["builds"]
 
 
 def run_reference(args, w):
@@ -150,18 +162,22 @@ def config_of(w, args, extra):
 # Algorithmic work of the step kernel.  Per LISTED pair the kernel must do
 # 3 sub, 3 mul/fma (r^2), 1 compare = 7 ALU ops / 9 flops; per pair inside r_cut in addition 1 rcp, 2 mul (r^-6),
 # 3 (f/r), 3 (energy), 3 mul + 3 add (force), 6 fma (virial) = 24 ALU ops / 33 flops (an FMA counts 2 flops, 1 op).
+# An inner step of hb_run_nve needs the forces only (tunable thermo_every = 0, the default: U_i and W_i of a step
+# nobody can read are not computed): per pair inside r_cut 1 rcp, 2 mul (r^-6), 1 fma + 2 mul (f/r), 3 fma (force)
+# = 9 ALU ops / 13 flops.
 OPS_LISTED, FLOPS_LISTED, OPS_INCUT, FLOPS_INCUT = 7, 9, 24, 33
+OPS_INCUT_F, FLOPS_INCUT_F = 9, 13
 
 
-def force_work(g, w):
-    """Algorithmic bytes, flops and ALU ops of one launch of the force kernel."""
+def force_work(g, w, thermo):
+    """Algorithmic bytes, flops and ALU ops of one launch of the step kernel (thermo: with U_i and W_i)."""
     pairs = int(g.get_nlist_sizes()[-1])
     N = w.N
-    # 16-bit list entries + position in, force + virial out, + velocity and position in and out when the step is fused in
-    bytes_ = 2 * pairs + N * (16 + 16 + 32) + N * (16 + 16 + 16 + 16)
+    # 16-bit list entries + position in, force (+ virial) out, + velocity and position in and out (the step is fused in)
+    bytes_ = 2 * pairs + N * (16 + 16 + (32 if thermo else 0)) + N * (16 + 16 + 16 + 16)
     frac_in = (w.r_cut_max / w.r_max) ** 3 if w.ntypes == 1 else 0.55
-    flops = FLOPS_LISTED * pairs + FLOPS_INCUT * frac_in * pairs
-    ops = OPS_LISTED * pairs + OPS_INCUT * frac_in * pairs
+    flops = FLOPS_LISTED * pairs + (FLOPS_INCUT if thermo else FLOPS_INCUT_F) * frac_in * pairs
+    ops = OPS_LISTED * pairs + (OPS_INCUT if thermo else OPS_INCUT_F) * frac_in * pairs
     return pairs, bytes_, flops, ops
 
 
@@ -238,19 +254,41 @@ def main():
     g, st0 = make_system(w, seed=w.seed + rank)
     g.run_nve(w.dt, args.equil, w.sort_period)
     g.run_nve(w.dt, args.warmup, w.sort_period)
+    g.run_nve(w.dt, args.steps, w.sort_period)       # rehearsal of the timed call itself: same chunking, untimed
+    builds0 = g.stats()["graph_builds"]
     sampler = ClockSampler(local)
     sampler.start()
-    ms, delta = timed_run(g, w, args.steps)
+    if args.steps >= 2000:
+        # two halves, so that a drift of the rate during the run would show
+        h1 = args.steps // 2
+        ms_a, delta_a = timed_run(g, w, h1)
+        ms_b, delta_b = timed_run(g, w, args.steps - h1)
+        ms = ms_a + ms_b
+        delta = {k: delta_a[k] + delta_b[k] for k in delta_a}
+        halves = {"first_half_steps_per_s": whole_job_value(world, h1, ms_a),
+                  "second_half_steps_per_s": whole_job_value(world, args.steps - h1, ms_b)}
+    else:
+        ms, delta = timed_run(g, w, args.steps)
+        halves = {}
     clocks = sampler.stop()
+    graph_builds_timed = g.stats()["graph_builds"] - builds0
     value = whole_job_value(world, args.steps, ms)
     th = g.thermo()
     stats = g.stats()
+    thermo_every = g.get_tunable("thermo_every")
+    g_chunk = g.get_tunable("graph_steps")
+
+    # ---- measured peaks (kernels of this library, this run) ----
+    peak_fp32 = g.measure_peak("fp32_tflops")
+    peak_l2 = g.measure_peak("l2_gbs")
+    peak_smem = g.measure_peak("smem_gbs")
 
     # ---- per-kernel rooflines, measured live with CUDA events on the launching stream ----
     # (hb_time_stage: the launches of one stage captured into one graph, CUDA events around the graph launch)
-    pairs, fbytes, fflops, fops = force_work(g, w)
-    t_step = g.time_stage("lj_nve", 200)                    # the kernel a step of hb_run_nve is: force + kicks + drift
-    t_force = g.time_stage("lj_force", 200)                 # the same kernel without the integration
+    pairs, fbytes, fflops, fops = force_work(g, w, thermo=bool(thermo_every))
+    _, tbytes, tflops, tops = force_work(g, w, thermo=True)
+    t_step = g.time_stage("lj_nve", 200)                    # the kernel an inner step of hb_run_nve is: force + kicks + drift
+    t_force = g.time_stage("lj_force", 200)                 # force + energy + virial, no integration (hb_compute_lj)
     t_step_cold = g.time_stage("lj_nve", 20, 512 << 20)     # L2 flushed before every launch
     t_nlist = g.time_stage("nlist", 50)
     t_cells = g.time_stage("cells", 50)
@@ -258,29 +296,49 @@ def main():
     t_nve = g.time_stage("nve", 200)
     rate = delta["rebuilds"] / args.steps
     share_step_kernel = t_step * args.steps / ms
-    roof_alu = {"bound": "alu", "achieved": fflops / (t_step * 1e-3) / 1e12, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "kernel": "lj_tile_kernel", "ms": t_step, "traffic": ncu_traffic("lj_tile_kernel"),
-                "peak_source": "nominal fp32: 148 SM x 128 lanes x 2 flop x 1.965 GHz (DESIGN.md); no measured fp32 peak exists",
-                "alu_ops_frac": fops / (t_step * 1e-3) / (FP32_PEAK_TFLOPS * 1e12 / 2),
-                "alu_ops_note": "algorithmic ALU instructions (an FMA is one) per second over 148 x 128 x 1.965 GHz issue slots"}
+    sec = t_step * 1e-3
+    roof_alu = {"bound": "alu", "achieved": fflops / sec / 1e12, "peak": peak_fp32, "unit": "TFLOP/s",
+                "kernel": "lj_tile_kernel (inner step of hb_run_nve: " + ("force, energy, virial" if thermo_every else "forces only") +
+                          ", both half kicks, drift, r_buff/2 check)",
+                "ms": t_step, "traffic": ncu_traffic("lj_tile_kernel"),
+                "peak_source": "measured in this run: hb_measure_peak fp32_tflops (8 FFMA chains per thread, all SMs); "
+                               f"nominal 148 x 128 x 2 x 1.965 GHz = {FP32_NOMINAL_TFLOPS:.1f}",
+                "alu_ops_frac": fops / sec / ISSUE_SLOTS_PER_S,
+                "alu_ops_note": "algorithmic ALU instructions (an FMA is one) per second over 148 x 128 x 1.965 GHz issue slots",
+                "gather_gbs": 16 * pairs / sec / 1e9, "gather_peak_gbs": peak_smem,
+                "gather_frac": 16 * pairs / sec / 1e9 / peak_smem,
+                "gather_note": "16 B of shared memory read per listed pair (the neighbor's staged position) over the measured "
+                               f"conflict-free shared-memory load bandwidth (nominal 128 B/clk/SM = {SMEM_NOMINAL_GBS:.0f} GB/s)"}
     roof_alu["frac"] = roof_alu["achieved"] / roof_alu["peak"]
-    roof_hbm = {"bound": "hbm", "achieved": fbytes / (t_step_cold * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "kernel": "lj_tile_kernel", "ms": t_step_cold, "traffic": ncu_traffic("lj_tile_kernel"),
-                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_kind}); L2 flushed before every launch"}
-    roof_hbm["frac"] = roof_hbm["achieved"] / roof_hbm["peak"]
+    l2_resident = w.N < 400_000
+    mem_peak = peak_l2 if l2_resident else hbm_peak
+    t_mem = t_step if l2_resident else t_step_cold
+    roof_mem = {"bound": "l2" if l2_resident else "hbm", "achieved": fbytes / (t_mem * 1e-3) / 1e9, "peak": mem_peak, "unit": "GB/s",
+                "kernel": "lj_tile_kernel", "ms": t_mem, "traffic": ncu_traffic("lj_tile_kernel"),
+                "peak_source": ("measured in this run: hb_measure_peak l2_gbs (32 MB buffer re-read from L2)" if l2_resident else
+                                f"MEASURED_PEAKS.json hbm_gbs ({peak_kind}); L2 flushed before every launch")}
+    roof_mem["frac"] = roof_mem["achieved"] / roof_mem["peak"]
     nl_bytes = 2 * pairs + w.N * (16 + 4 + 64)              # positions in, 16-bit entries + count out, reorder copy-back
     nl_tests = 27.0 * w.N * w.N / stats["cells_per_axis"] ** 3
     kernels = {
-        "lj_step": {"ms_warm_l2": t_step, "ms_cold_l2": t_step_cold, "ms_force_only": t_force, "pairs": pairs,
+        "lj_step": {"ms_warm_l2": t_step, "ms_cold_l2": t_step_cold, "pairs": pairs,
                     "algorithmic_bytes": fbytes, "algorithmic_flops": fflops, "algorithmic_alu_ops": fops,
                     "share_of_step": share_step_kernel},
+        "lj_force_energy_virial": {"ms": t_force, "algorithmic_flops": tflops, "algorithmic_alu_ops": tops,
+                                   "tflops": tflops / (t_force * 1e-3) / 1e12, "frac_fp32": tflops / (t_force * 1e-3) / 1e12 / peak_fp32,
+                                   "alu_ops_frac": tops / (t_force * 1e-3) / ISSUE_SLOTS_PER_S,
+                                   "note": "hb_compute_lj's kernel (the paper's: U_i and W_i with the force, PAPER.md:95), no integration"},
         "nlist": {"ms": t_nlist, "algorithmic_bytes": nl_bytes, "gbs": nl_bytes / (t_nlist * 1e-3) / 1e9,
-                  "frac_hbm": nl_bytes / (t_nlist * 1e-3) / 1e9 / hbm_peak, "distance_tests": nl_tests,
-                  "alu_ops_frac": 8 * nl_tests / (t_nlist * 1e-3) / (FP32_PEAK_TFLOPS * 1e12 / 2)},
+                  "frac_mem": nl_bytes / (t_nlist * 1e-3) / 1e9 / mem_peak, "distance_tests": nl_tests,
+                  "tflops": 9 * nl_tests / (t_nlist * 1e-3) / 1e12, "frac_fp32": 9 * nl_tests / (t_nlist * 1e-3) / 1e12 / peak_fp32,
+                  "alu_ops_frac": 8 * nl_tests / (t_nlist * 1e-3) / ISSUE_SLOTS_PER_S,
+                  "note": "27 N^2/m^3 distance tests of 8 ALU instructions / 9 flops each (3 sub, 3 mul-add, compare, record)"},
         "cells": {"ms": t_cells, "algorithmic_bytes": 36 * w.N + 100 * w.N},
         "rebuild": {"ms": t_rebuild, "per_step": rate, "ms_per_step": rate * t_rebuild},
         "nve_standalone": {"ms": t_nve, "algorithmic_bytes": 108 * w.N, "gbs": 108 * w.N / (t_nve * 1e-3) / 1e9},
         "step_model": {"ms": t_step + rate * t_rebuild, "launch_gaps_ms": ms / args.steps - (t_step + rate * t_rebuild)},
+        "peaks_measured": {"fp32_tflops": peak_fp32, "l2_gbs": peak_l2, "smem_gbs": peak_smem, "hbm_gbs": hbm_peak,
+                           "hbm_source": peak_kind},
     }
 
     # ---- end to end through the C ABI with HOST buffers ----
@@ -288,7 +346,8 @@ def main():
     pos_h, vel_h, typ_h, img_h = (np.ascontiguousarray(s_now[k]) for k in ("pos", "vel", "type", "image"))
     Ke = max(1, min(args.steps, 2000))
     g.set_state(pos_h, typ_h, vel_h, img_h)
-    g.run_nve(w.dt, 50, w.sort_period)
+    g.run_nve(w.dt, Ke, w.sort_period)                           # rehearsal: the timed call below repeats it
+    builds_e = g.stats()["graph_builds"]
     torch.cuda.synchronize()
     if dist is not None:
         dist.barrier()
@@ -301,6 +360,7 @@ def main():
     el = max_over_ranks(el, dist, "cuda")
     e2e = {"value": world * Ke / el, "unit": UNIT, "steps_per_call": Ke, "h2d_bytes_per_step": w.N * 40 / Ke,
            "d2h_bytes_per_step": (w.N * 40 + 96) / Ke, "h2d_bytes_per_call": w.N * 40, "d2h_bytes_per_call": w.N * 40 + 96,
+           "graph_builds_in_timed_region": g.stats()["graph_builds"] - builds_e,
            "note": "hb_set_state(host) + hb_run_nve + hb_get_state(host) + hb_thermo, wall clock"}
     g.close()
 
@@ -310,34 +370,51 @@ def main():
         g2, _ = make_system(w2, seed=w2.seed)
         g2.run_nve(w2.dt, 600, w2.sort_period)
         ms2, d2 = timed_run(g2, w2, 1000)
-        p2, b2, f2, o2 = force_work(g2, w2)
+        p2, b2, f2, o2 = force_work(g2, w2, thermo=bool(g2.get_tunable("thermo_every")))
         tf2 = g2.time_stage("lj_nve", 30)
+        tf2c = g2.time_stage("lj_nve", 10, 512 << 20)
         tn2 = g2.time_stage("nlist", 10)
+        tr2 = g2.time_stage("rebuild", 10)
+        m2 = g2.stats()["cells_per_axis"]
         also = {"lj_1m": {"timesteps_per_s": 1000 / (ms2 * 1e-3), "particle_steps_per_s": 1000 * w2.N / (ms2 * 1e-3),
-                          "ms_per_step": ms2 / 1000, "rebuilds": d2["rebuilds"], "lj_step_ms": tf2,
-                          "lj_step_hbm_gbs": b2 / (tf2 * 1e-3) / 1e9, "lj_step_hbm_frac": b2 / (tf2 * 1e-3) / 1e9 / hbm_peak,
-                          "lj_step_alu_frac": f2 / (tf2 * 1e-3) / 1e12 / FP32_PEAK_TFLOPS,
-                          "nlist_ms": tn2, "mean_nbrs": p2 / w2.N, "inputs": "larger than L2 (126 MB list + tables)"}}
+                          "ms_per_step": ms2 / 1000, "rebuilds": d2["rebuilds"], "lj_step_ms": tf2, "lj_step_ms_cold_l2": tf2c,
+                          "lj_step_hbm_gbs": b2 / (tf2c * 1e-3) / 1e9, "lj_step_hbm_frac": b2 / (tf2c * 1e-3) / 1e9 / hbm_peak,
+                          "lj_step_fp32_frac": f2 / (tf2 * 1e-3) / 1e12 / peak_fp32,
+                          "lj_step_alu_ops_frac": o2 / (tf2 * 1e-3) / ISSUE_SLOTS_PER_S,
+                          "lj_step_gather_frac": 16 * p2 / (tf2 * 1e-3) / 1e9 / peak_smem,
+                          "nlist_ms": tn2, "rebuild_ms": tr2,
+                          "nlist_alu_ops_frac": 8 * 27.0 * w2.N * w2.N / m2 ** 3 / (tn2 * 1e-3) / ISSUE_SLOTS_PER_S,
+                          "nlist_hbm_frac": (2 * p2 + w2.N * 84) / (tn2 * 1e-3) / 1e9 / hbm_peak,
+                          "mean_nbrs": p2 / w2.N, "inputs": "larger than L2 (126 MB list + tables)"}}
         g2.close()
-        # opt-in variant, NOT the headline: inner steps of a chunk compute forces only (tunable thermo_every = 0);
-        # same trajectory bit for bit, energies and virials valid whenever hb_run_nve returns
-        tun["thermo_every"] = "0"
+        # the paper's kernel in every step (U_i and W_i always): tunable thermo_every = 1; same trajectory
+        # bit for bit as the headline, which computes them in the last step of every chunk only
+        tun["thermo_every"] = "1"
         g3, _ = make_system(w, seed=w.seed + rank)
         del tun["thermo_every"]
         g3.run_nve(w.dt, args.equil + args.warmup, w.sort_period)
-        ms3, d3 = timed_run(g3, w, min(args.steps, 4000))
-        also["lj_64k_thermo_every_0"] = {"timesteps_per_s": min(args.steps, 4000) / (ms3 * 1e-3),
-                                         "note": "U_i and W_i only in the last step of each 100-step chunk; opt-in, not the headline"}
+        n3 = min(args.steps, 4000)
+        g3.run_nve(w.dt, n3, w.sort_period)
+        ms3, d3 = timed_run(g3, w, n3)
+        t3 = g3.time_stage("lj_nve", 200)
+        also["lj_64k_thermo_every_1"] = {"timesteps_per_s": n3 / (ms3 * 1e-3), "lj_step_ms": t3,
+                                         "lj_step_fp32_frac": tflops / (t3 * 1e-3) / 1e12 / peak_fp32,
+                                         "lj_step_alu_ops_frac": tops / (t3 * 1e-3) / ISSUE_SLOTS_PER_S,
+                                         "note": "U_i and W_i in every step (the paper's kernel)"}
         g3.close()
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         # about 15 s of CPU work: the oracle takes ~1.5e-7 s per particle per step on the 16 cores of these boxes
-        n_cpu = max(2, min(2000, int(15.0 / (w.N * 1.5e-7 * 16 / max(1, os.cpu_count() or 1)))))
+        ncores = max(1, os.cpu_count() or 1)
+        n_cpu = max(2, min(2000, int(10.0 / (w.N * 1.5e-7 * 16 / ncores))))
         v, secs, cores, builds = cpu_oracle_steps_per_s(w, st0, n_cpu)
+        n_one = max(2, min(n_cpu, int(5.0 / (w.N * 1.5e-7 * 16))))
+        v1, secs1, cores1, _ = cpu_oracle_steps_per_s(w, st0, n_one, threads=1)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {n_cpu} steps of {w.name} (N={w.N}) from the seeded lattice start incl. the initial list build "
-                         f"and {builds} builds, {secs:.1f} s"}
+                         f"and {builds} builds, {secs:.1f} s",
+               "one_thread": {"value": v1, "cores": cores1, "sample": f"first {n_one} steps, {secs1:.1f} s"}}
 
     if rank == 0:
         line = {
@@ -349,14 +426,16 @@ def main():
                        "of one trajectory, each consuming the previous step's output; no flush between steps"
                        if w.N < 400_000 else "inputs larger than L2"),
                 "row_pitch": stats["row_pitch"], "cells_per_axis": stats["cells_per_axis"], "mean_nbrs": pairs / w.N,
+                "chunk_steps": g_chunk, "thermo_every": thermo_every,
                 "tunables": {k: g_tun for k, g_tun in tun.items()}}),
-            "particle_steps_per_s": value * w.N,
+            "particle_steps_per_s": value * w.N, **halves,
+            "graph_builds_in_timed_region": graph_builds_timed,
             "context_paper": {"gtx_titan_gk110_steps_per_s": PAPER_TITAN_STEPS_PER_S, "ratio": value / world / PAPER_TITAN_STEPS_PER_S,
                               "note": "PAPER.md:143, other hardware and an equilibrated start: context, not vs_baseline"},
             "run": {**delta, "E_per_particle": (th["K"] + th["U"]) / w.N, "T": 2 * th["K"] / (3 * w.N),
                     "max_nbrs": stats["max_nbrs"]},
             "roofline": roof_alu,
-            "roofline_other": roof_hbm,
+            "roofline_other": roof_mem,
             "kernels": kernels,
             "cpu_baseline": cpu,
             "e2e": e2e,

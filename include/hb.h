@@ -85,6 +85,8 @@ typedef struct hb_stats_t {
     int64_t cells_per_axis;   /* m */
     int64_t graph_launches;   /* CUDA graph launches made by hb_run_nve */
     int64_t kernel_launches;  /* kernels enqueued (graph nodes counted when they run) */
+    int64_t graph_builds;     /* CUDA graphs captured and instantiated so far (none after the first hb_run_nve
+                                 unless a tunable, dt, r_buff or an array size changes) */
 } hb_stats_t;
 
 /* Create a system of N particles in a cubic box of edge L with ntypes types and
@@ -153,6 +155,8 @@ HB_API int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_peri
  * cell order anyway; inside a cell the order set here survives.) */
 HB_API int hb_sort(hb_system *h);
 
+/* Thermodynamic sums of the current state.  If the forces are stale (after hb_set_state, hb_build_nlist,
+ * hb_build_cells, hb_sort) the list is rebuilt if needed and the forces are evaluated first. */
 HB_API int hb_thermo(hb_system *h, hb_thermo_t *out);
 
 /* Cell list: m_out [3]; cell_start [m^3+1]; cell_tags [N] = tags of the members
@@ -180,8 +184,10 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
  *   "force_block"    threads per block of the force kernel: 128, 256
  *   "nlist_block"    threads per block of the stand-alone list kernel: 128, 256
- *   "thermo_every"   1 = U_i and W_i are computed every step (default, the paper's kernel);
- *                    0 = inside hb_run_nve only by the last step of each chunk (they cannot be read before)
+ *   "thermo_every"   0 = (default) inside hb_run_nve U_i and W_i are computed by the last step of every chunk only:
+ *                        those of an inner step cannot be read by anyone, the trajectory is the same bit for bit,
+ *                        and energies, virials and hb_thermo are valid whenever hb_run_nve returns;
+ *                    1 = every step computes them (the paper's kernel does)
  *   "fuse_nve"       1 = hb_run_nve integrates inside the force kernel (one kernel per step)
  *   "coop_rebuild"   0 = the rebuild is five launches (count, scan, scatter, gather, list);
  *                    1 = Algorithm 2 and the reorder are ONE cooperative kernel, then the list kernel;
@@ -207,6 +213,13 @@ HB_API int hb_get_tunable(hb_system *h, const char *name, int *value);
  * scratch buffer of that size is overwritten before every launch (outside the
  * timed interval) so that each launch starts with a cold L2.  Needs a list. */
 HB_API int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_bytes, double *mean_ms);
+
+/* Measured roofline denominators on this device, with kernels of this library:
+ *   "fp32_tflops"  FFMA throughput, 8 independent chains per thread, all SMs        -> TFLOP/s
+ *   "l2_gbs"       read bandwidth of a 32 MB buffer resident in L2, 16 B per load   -> GB/s
+ *   "smem_gbs"     conflict-free 16-byte shared-memory loads, all SMs               -> GB/s
+ * Best of five timed launches (CUDA events on the system's stream); synchronises. */
+HB_API int hb_measure_peak(hb_system *h, const char *which, double *value);
 
 HB_API const char *hb_last_error(hb_system *h);
 HB_API const char *hb_version(void);

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhb.so")
-SOURCES = ["hb_api.cu", "cells.cu", "nlist.cu", "force.cu", "nve.cu", "sort.cu"]
+SOURCES = ["hb_api.cu", "cells.cu", "nlist.cu", "force.cu", "nve.cu", "sort.cu", "peaks.cu"]
 HEADERS = [os.path.join(CSRC, n) for n in ("hb_internal.cuh", "tile.cuh", "cells_dev.cuh")] + \
           [os.path.join(os.path.dirname(HERE), "include", "hb.h")]
 
@@ -41,7 +41,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
-    cmd = [nvcc(), *NVCC_FLAGS, "-shared", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    cmd = [nvcc(), *NVCC_FLAGS, *os.environ.get("HB_NVCC_EXTRA", "").split(), "-shared", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES] + ["-ldl"]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")

@@ -4,31 +4,38 @@
 //
 //   V_lj = 4 eps [(sigma/r)^12 - (sigma/r)^6],  f = -(1/r) dV/dr * d,  r < r_cut,ab
 // with per-type-pair tables held as lj1 = 4 eps sigma^12, lj2 = 4 eps sigma^6:
-//   -(1/r) dV/dr = r^-2 r^-6 (12 lj1 r^-6 - 6 lj2),   V = r^-6 (lj1 r^-6 - lj2) - eshift.
+//   -(1/r) dV/dr = r^-8 (12 lj1 r^-6 - 6 lj2),   V = r^-6 (lj1 r^-6 - lj2) - eshift.
 // The pair functor idea of PAPER.md:284 (V(r) and -(1/r) dV/dr) is kept as the
 // inlined pair_term() below.
 //
-// Design.  Round-1 ncu of the first version (one 16-byte global gather per pair):
-// 46 % of the stall samples on the gathers, every warp gather touching ~32 cache
-// lines, the L1 wavefront queue the limiter.  Now ONE BLOCK OWNS ONE TILE of cells
-// (tile.cuh):
-//   * the tile and its halo are staged once in shared memory with coalesced
-//     loads, shifted to the periodic image the tile sees: no minimum-image
-//     arithmetic per pair, and every neighbor gather is a 16-byte shared-memory
-//     load (list entries are 16-bit slots of this staging layout);
-//   * the list build leaves a descriptor and a slot table per tile behind, so the
-//     staging here is: descriptor -> storage index of every slot -> position;
-//   * TPP threads share one particle (2 by default); each takes EPL (8) consecutive
-//     16-bit entries per iteration.  The rows arrive through a ring of four
-//     cp.async copies per thread, not through registers (see cp_async below); a row
-//     ends at its first padding entry, so no row length is read.  The EPL gathers
-//     are issued back to back and the pairs evaluated without a branch: a pair
-//     outside r_cut gets r^-2 := 0, the padding is the far-away dummy slot;
-//   * F, U, W are combined across the TPP lanes with warp shuffles;
-//   * when asked, the same thread finishes the velocity-Verlet step of its
-//     particle with the force it just computed (second half kick of this step,
-//     first half kick and drift of the next, wrap, image flags, r_buff/2 check),
-//     writing the new position into the OTHER position buffer, since the blocks
+// Design (round 2; the ncu numbers that led here are in profiles/r1c_* and r2_*).
+// ONE BLOCK OWNS ONE TILE of cells (tile.cuh):
+//   * the tile and its one-cell halo are staged once in shared memory, shifted to the
+//     periodic image the tile sees: no minimum-image arithmetic per pair, and every
+//     neighbor gather is ONE 16-byte shared-memory load.  The particle data is kept in
+//     cell order, so a row of x-adjacent halo cells is one contiguous range of the
+//     position array ("piece", two where the row wraps around the box): the block
+//     reads cell_start at the ends of its (ty+2)(tz+2) halo rows, prefix-sums the
+//     lengths (that IS the slot numbering the list build used) and copies each piece
+//     with cp.async, 16 bytes per lane, straight into the staging area.  No per-tile
+//     table is read (round 1 read a 4-byte source index per staged slot per step).
+//     Only tiles whose halo touches a face of the box fix the periodic image, in place;
+//   * list entries are 16-bit BYTE OFFSETS into the staging area (slot * 16 when the
+//     staging area has at most 4096 slots), so an entry becomes the address of its
+//     gather with one instruction;
+//   * TPP threads share one particle; each takes EPL consecutive entries per iteration.
+//     The rows arrive through a ring of cp.async copies per thread; a row ends at its
+//     first padding entry (slot 0 = a dummy particle far away), so no row length is read.
+//     The EPL gathers are issued back to back; a pair outside r_cut gets r^-2 := 0 by a
+//     select, not by a branch;
+//   * an inner step of hb_run_nve needs F only (nobody can read its U_i, W_i): the
+//     THERMO = false variant has 3 accumulators and no force store at all;
+//   * F (and U, W) are combined across the TPP lanes with warp shuffles and parked in
+//     shared memory; after a block barrier thread t finishes the velocity-Verlet step
+//     of particle t of the pass (second half kick of this step, first half kick and
+//     drift of the next, wrap, image flags, r_buff/2 check) with v, x and x_build that
+//     were prefetched into shared memory by cp.async while the pairs were evaluated,
+//     and writes the new position into the OTHER position buffer, since the blocks
 //     around still read the old one.  One kernel per time step.
 #include "tile.cuh"
 
@@ -39,101 +46,271 @@ __device__ __forceinline__ float rcp_approx(float x)
     return y;
 }
 
-// cp.async (LDGSTS): global -> shared without a register or a scoreboard slot in between.  ncu of the
-// register-prefetch version showed 40 % of the warp time in long-scoreboard stalls at the first use of
-// a list entry however far ahead it was loaded: scoreboard slots count, so a consumer waits for every
-// later load on its slot too.  Async-copy groups are tracked separately.
+// cp.async (LDGSTS): global -> shared without a register or a scoreboard slot in between.
+// List rows go through L1 (.ca): a row is read 16 or 8 bytes at a time, its 128-byte lines are fetched once.
 template <int BYTES>
 __device__ __forceinline__ void cp_async(void *smem_dst, const void *gsrc)
 {
     const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(d), "l"(gsrc), "n"(BYTES) : "memory");
 }
+// Particle data is read once per block: past L1 (.cg, 16 bytes).
+__device__ __forceinline__ void cp_async_cg16(void *smem_dst, const void *gsrc)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// TMA bulk copy global -> shared (UBLKCP), completion counted in bytes on an mbarrier: one instruction moves a whole
+// piece of the halo (a contiguous run of positions), no per-particle instruction at all.
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
 
 struct Acc {
     float fx, fy, fz, u, wxx, wxy, wxz, wyy, wyz, wzz;
 };
 
+// One listed pair.  pj is already the nearest image.  The force sums are the same operations in both variants
+// (fma(f/r, d, F)), so the trajectory does not depend on whether the energy and virial terms are compiled in.
 template <bool THERMO>
-__device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, const PairParam &pp, Acc &a)
+__device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, const float lj1x12, const float lj2x6,
+                                          const float rcut2, const float lj1, const float lj2, const float eshift, Acc &a)
 {
-    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;   // pj is already the nearest image
+    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-    const bool in = r2 < pp.rcut2;                     // strict <
-    const float r2inv = in ? rcp_approx(r2) : 0.0f;    // 0 switches the whole pair off
-    const float r6inv = r2inv * r2inv * r2inv;
-    const float fdivr = r2inv * r6inv * __fmaf_rn(12.0f * pp.lj1, r6inv, -6.0f * pp.lj2);
-    // explicit roundings: the force sums must not depend on whether the energy and virial terms are compiled in
-    const float px = __fmul_rn(fdivr, dx), py = __fmul_rn(fdivr, dy), pz = __fmul_rn(fdivr, dz);
-    a.fx = __fadd_rn(a.fx, px); a.fy = __fadd_rn(a.fy, py); a.fz = __fadd_rn(a.fz, pz);
-    if (!THERMO) return;   // an inner step of hb_run_nve with thermo_every = 0: nobody can read U_i, W_i of this step
-    const float e = __fmaf_rn(r6inv, __fmaf_rn(pp.lj1, r6inv, -pp.lj2), in ? -pp.eshift : 0.0f);
-    a.u += e;
-    a.wxx = __fmaf_rn(dx, px, a.wxx); a.wxy = __fmaf_rn(dx, py, a.wxy); a.wxz = __fmaf_rn(dx, pz, a.wxz);
-    a.wyy = __fmaf_rn(dy, py, a.wyy); a.wyz = __fmaf_rn(dy, pz, a.wyz); a.wzz = __fmaf_rn(dz, pz, a.wzz);
+    const bool in = r2 < rcut2;                        // strict <
+    const float r2inv = in ? rcp_approx(r2) : 0.0f;    // 0 switches the whole pair off: no branch (a branch per pair
+    const float r4inv = r2inv * r2inv;                 // would serialise the EPL pairs of an iteration)
+    const float r6inv = r4inv * r2inv;
+    const float fdivr = (r4inv * r4inv) * __fmaf_rn(lj1x12, r6inv, -lj2x6);
+    a.fx = __fmaf_rn(fdivr, dx, a.fx);
+    a.fy = __fmaf_rn(fdivr, dy, a.fy);
+    a.fz = __fmaf_rn(fdivr, dz, a.fz);
+    if (THERMO) {
+        a.u += __fmaf_rn(r6inv, __fmaf_rn(lj1, r6inv, -lj2), in ? -eshift : 0.0f);
+        const float px = fdivr * dx, py = fdivr * dy, pz = fdivr * dz;
+        a.wxx = __fmaf_rn(dx, px, a.wxx); a.wxy = __fmaf_rn(dx, py, a.wxy); a.wxz = __fmaf_rn(dx, pz, a.wxz);
+        a.wyy = __fmaf_rn(dy, py, a.wyy); a.wyz = __fmaf_rn(dy, pz, a.wyz); a.wzz = __fmaf_rn(dz, pz, a.wzz);
+    }
 }
 
 template <int EPL> struct Entries;
 template <> struct Entries<4> { uint2 v; };
 template <> struct Entries<8> { uint4 v; };
 
-template <int EPL>
-__device__ __forceinline__ Entries<EPL> load_entries(const uint16_t *p)
+// byte offsets of the EPL gathers of one iteration
+template <int EPL, bool SCALED>
+__device__ __forceinline__ void unpack_entries(const Entries<EPL> &e, unsigned (&off)[EPL])
 {
-    Entries<EPL> e;
-    if constexpr (EPL == 4) e.v = __ldg(reinterpret_cast<const uint2 *>(p));
-    else e.v = __ldg(reinterpret_cast<const uint4 *>(p));
-    return e;
+    const unsigned w[4] = {e.v.x, e.v.y, EPL == 8 ? ((const unsigned *)&e.v)[2] : 0u, EPL == 8 ? ((const unsigned *)&e.v)[3] : 0u};
+#pragma unroll
+    for (int k = 0; k < EPL / 2; k++) {
+        if (SCALED) { off[2 * k] = w[k] & 0xffffu; off[2 * k + 1] = w[k] >> 16; }
+        else { off[2 * k] = (w[k] & 0xffffu) << 4; off[2 * k + 1] = (w[k] >> 16) << 4; }
+    }
 }
 
-template <int EPL>
-__device__ __forceinline__ void unpack_entries(const Entries<EPL> &e, int (&sl)[EPL])
+struct ForceArgs {
+    TileGeom g;
+    const int *cell_start;
+    const float4 *pos;
+    const uint16_t *nlist;
+    int pitch, N, ntypes;
+    const PairParam *params;
+    float4 *force, *virial;
+    int *flags;
+    int do_nve;
+    NveArgs nv;
+};
+
+// What the block knows about its tile (shared memory).
+struct ForceTile {
+    TileDesc d;                          // own rows, counts, centre
+    int piece_src[2 * TILE_PROWS_MAX];   // storage index of the first particle of piece p
+    int piece_slot[2 * TILE_PROWS_MAX + 1];   // its first slot; [npieces] = nslots
+    int npieces, fix;
+    alignas(8) uint64_t mbar;            // completion of the staging copies
+};
+
+// Fast geometry (tile + halo narrower than L/2): halo rows as contiguous pieces of the cell-ordered position array.
+__device__ __forceinline__ bool force_tile_tables(const TileGeom &g, const int *__restrict__ cell_start, ForceTile &s)
 {
-    sl[0] = e.v.x & 0xffffu; sl[1] = e.v.x >> 16; sl[2] = e.v.y & 0xffffu; sl[3] = e.v.y >> 16;
-    if constexpr (EPL == 8) { sl[4] = e.v.z & 0xffffu; sl[5] = e.v.z >> 16; sl[6] = e.v.w & 0xffffu; sl[7] = e.v.w >> 16; }
+    TileCtx t;
+    tile_decode_xyz(g, blockIdx.x, blockIdx.y, blockIdx.z, t);
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int hrows = t.hy * t.hz;
+    const int m = g.m;
+    // one thread per halo row: lengths of its (at most two) pieces
+    for (int r = tid; r < hrows; r += blockDim.x) {
+        const int jy = r % t.hy, jz = r / t.hy;
+        int cy = t.y0 - 1 + jy, cz = t.z0 - 1 + jz;
+        cy += cy < 0 ? m : (cy >= m ? -m : 0);
+        cz += cz < 0 ? m : (cz >= m ? -m : 0);
+        const int rowbase = m * (cy + m * cz);
+        const int X0 = t.x0 - 1, X1 = t.x0 + t.ex;          // tile frame, inclusive
+        int a0, a1, b0 = 0, b1 = -1;                         // piece A = cells a0..a1, piece B = cells b0..b1 (box frame)
+        if (X0 < 0) { a0 = a1 = m - 1; b0 = 0; b1 = X1; }
+        else if (X1 >= m) { a0 = X0; a1 = m - 1; b0 = b1 = 0; }
+        else { a0 = X0; a1 = X1; }
+        const int sa = __ldg(&cell_start[rowbase + a0]), ea = __ldg(&cell_start[rowbase + a1 + 1]);
+        int sb = 0, eb = 0;
+        if (b1 >= b0) { sb = __ldg(&cell_start[rowbase + b0]); eb = __ldg(&cell_start[rowbase + b1 + 1]); }
+        s.piece_src[2 * r] = sa; s.piece_src[2 * r + 1] = sb;
+        s.piece_slot[2 * r] = ea - sa; s.piece_slot[2 * r + 1] = eb - sb;
+        // own rows: interior rows of the halo box
+        const int ly = jy - 1, lz = jz - 1;
+        if (ly >= 0 && ly < t.ey && lz >= 0 && lz < t.ez) {
+            const int orow = ly + t.ey * lz;
+            const int os = __ldg(&cell_start[rowbase + t.x0]), oe = __ldg(&cell_start[rowbase + t.x0 + t.ex - 1 + 1]);
+            s.d.own_start[orow] = os;
+            s.d.own_off[orow + 1] = oe - os;
+            // slot of the first own particle, relative to the row's first slot: the cell left of x0 comes first
+            s.d.own_slot[orow] = X0 < 0 ? (ea - sa) : (os - sa);
+        }
+    }
+    __syncthreads();
+    const int np = 2 * hrows;
+    if (tid < 32) {   // exclusive scan of up to 2 * TILE_PROWS_MAX lengths: 6 per lane
+        constexpr int PER = (2 * TILE_PROWS_MAX + 31) / 32;
+        const int base = lane * PER;
+        int v[PER], tsum = 0;
+#pragma unroll
+        for (int q = 0; q < PER; q++) { v[q] = base + q < np ? s.piece_slot[base + q] : 0; tsum += v[q]; }
+        int incl = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
+        int run = 1 + incl - tsum;   // slot 0 is the dummy
+#pragma unroll
+        for (int q = 0; q < PER; q++) { if (base + q < np) s.piece_slot[base + q] = run; run += v[q]; }
+        if (lane == 31) s.piece_slot[np] = run;
+    }
+    __syncthreads();
+    if (tid < t.ey * t.ez) {
+        const int ly = tid % t.ey, lz = tid / t.ey;
+        s.d.own_slot[tid] += s.piece_slot[2 * ((lz + 1) * t.hy + (ly + 1))];
+    }
+    if (tid == 0) {
+        int run = 0;
+        const int nrows = t.ey * t.ez;
+        s.d.own_off[0] = 0;
+        for (int r = 0; r < nrows; r++) { const int n = s.d.own_off[r + 1]; s.d.own_off[r + 1] = run + n; run += n; }
+        const float wcell = g.L / (float)m, hL = 0.5f * g.L;
+        s.d.nslots = s.piece_slot[np];
+        s.d.nown = run;
+        s.d.nrows = nrows;
+        s.d.cx = __fmaf_rn((float)t.x0 + 0.5f * (float)t.ex, wcell, -hL);
+        s.d.cy = __fmaf_rn((float)t.y0 + 0.5f * (float)t.ey, wcell, -hL);
+        s.d.cz = __fmaf_rn((float)t.z0 + 0.5f * (float)t.ez, wcell, -hL);
+        s.npieces = np;
+        // a staged particle can sit on the other side of the box only if the halo reaches the first or last cell of
+        // an axis (a wrapped halo cell, or a particle that drifted through the face after the build)
+        s.fix = (t.x0 <= 1 || t.x0 + t.ex >= m - 1 || t.y0 <= 1 || t.y0 + t.ey >= m - 1 || t.z0 <= 1 || t.z0 + t.ez >= m - 1) ? 1 : 0;
+    }
+    __syncthreads();
+    return s.d.nslots <= g.cap;
 }
 
-template <int TPP, int EPL, bool ONE_TYPE, bool THERMO>
+template <int TPP, int EPL, bool ONE_TYPE, bool THERMO, bool SCALED>
 __global__ void __launch_bounds__(TILE_THREADS, 4)   // <= 64 registers: 8 blocks of 128 threads per SM
-lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__restrict__ pos,
-               const uint16_t *__restrict__ nlist, const int *__restrict__ nlistn, int pitch, int N, int ntypes,
-               const PairParam *__restrict__ params, float4 *__restrict__ force, float4 *__restrict__ virial,
-               int *__restrict__ flags, int do_nve, NveArgs nv, const int *__restrict__ stage_src,
-               const TileDesc *__restrict__ desc)
+lj_tile_kernel(const ForceArgs A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ TileShared s;
-    float4 *stage = reinterpret_cast<float4 *>(smem_raw);
-    PairParam *s_params = reinterpret_cast<PairParam *>(smem_raw + (size_t)g.cap * 16);
+    __shared__ ForceTile s;
+    const TileGeom &g = A.g;
+    const int nthreads = blockDim.x;
+    const int PPB = nthreads / TPP;              // particles per block per pass
     constexpr int G = TPP * EPL;                 // entries per particle per iteration
+    constexpr int PF = 4;                        // depth of the ring of list copies
+    using EntryVec = decltype(Entries<EPL>::v);
 
+    // dynamic shared memory: staging area | pair table | ring | own data of a pass (v, x, x_build; one buffer: a
+    // thread group reads its particle's data into registers before it starts the copies of the next pass)
+    unsigned char *sp = smem_raw;
+    float4 *stage = reinterpret_cast<float4 *>(sp);                      sp += (size_t)g.cap * 16;
+    PairParam *s_params = reinterpret_cast<PairParam *>(sp);             sp += ONE_TYPE ? 0 : ((A.ntypes * A.ntypes * sizeof(PairParam) + 15) & ~(size_t)15);
+    EntryVec *ring = reinterpret_cast<EntryVec *>(sp) + threadIdx.x;     sp += (size_t)PF * sizeof(EntryVec) * nthreads;
+    float4 *own = reinterpret_cast<float4 *>(sp);                        sp += (size_t)3 * PPB * 16;       // [v | x | x_build][PPB]
+    TileShared &sgen = *reinterpret_cast<TileShared *>(sp);              // the general (small-box) geometry only
+    const int ring_stride = nthreads;
+    const NveArgs &nv = A.nv;
+    const bool nve = A.do_nve != 0, drift = nve && nv.kick_drift;
+    const bool block0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
+
+    if (threadIdx.x == 0 && g.fast) mbar_init(&s.mbar, 1);
     if (!ONE_TYPE)
-        for (int k = threadIdx.x; k < ntypes * ntypes; k += blockDim.x) s_params[k] = params[k];
-    if (do_nve && nv.kick_drift && blockIdx.x == 0 && threadIdx.x == 0) flags[nv.need_clear] = 0;
+        for (int k = threadIdx.x; k < A.ntypes * A.ntypes; k += nthreads) s_params[k] = A.params[k];
+    if (drift && block0 && threadIdx.x == 0) A.flags[nv.need_clear] = 0;
+
+    // ---- the tile: tables, staging ----
+    bool fits;
+    if (g.fast) {
+        fits = force_tile_tables(g, A.cell_start, s);
+        if (fits && threadIdx.x < 32) {
+            // warp 0 hands the pieces to the TMA unit: one bulk copy per contiguous run of positions
+            const int lane = threadIdx.x;
+            if (lane == 0) {
+                stage[0] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+                mbar_expect_tx(&s.mbar, (unsigned)(s.d.nslots - 1) * 16u);
+            }
+            __syncwarp();
+            for (int p = lane; p < s.npieces; p += 32) {
+                const int s0 = s.piece_slot[p], len = s.piece_slot[p + 1] - s0;
+                if (len > 0) bulk_g2s(stage + s0, A.pos + s.piece_src[p], (unsigned)len * 16u, &s.mbar);
+            }
+        }
+    } else {
+        TileCtx t;
+        tile_decode_xyz(g, blockIdx.x, blockIdx.y, blockIdx.z, t);
+        fits = tile_tables(g, A.cell_start, t, sgen, A.flags);
+        if (threadIdx.x < sizeof(TileDesc) / 4) reinterpret_cast<int *>(&s.d)[threadIdx.x] = reinterpret_cast<const int *>(&sgen.d)[threadIdx.x];
+        __syncthreads();
+        if (fits) tile_stage_positions(g, t, sgen, A.pos, stage, nullptr);
+    }
+    const int nown = fits ? s.d.nown : 0;
 
     const int sub = threadIdx.x % TPP;
-    const int PPB = blockDim.x / TPP;            // particles per block per pass
-    // List rows reach the threads through a ring of PF async copies per thread: entry group k of the
-    // row is copied PF iterations before it is used.  A row ends at its first padding entry (slot 0;
-    // the build pads every row with at least 32 of them), so the row length is never loaded.
-    constexpr int PF = 4;
-    using EntryVec = decltype(Entries<EPL>::v);
-    EntryVec *ring = reinterpret_cast<EntryVec *>(smem_raw + (size_t)g.cap * 16 +
-                                                  (ONE_TYPE ? 0 : ((ntypes * ntypes * sizeof(PairParam) + 15) & ~(size_t)15))) +
-                     threadIdx.x;
-    const int ring_stride = blockDim.x;
+    const int ql = threadIdx.x / TPP;            // particle of the pass this thread group works for
     int gi_n = 0, slot_n = 0;
     bool active_n = false;
-    // particle of pass q0 for this thread group; start the copies of its first PF entry groups
-    auto prep = [&](int q0, int nown) {
-        const int q = q0 + threadIdx.x / TPP;
+    // start of a pass: the particle of this thread group, the first PF copies of its row, and (lanes 0 and 1 of the
+    // group) what the integration of the particle will need
+    auto prep = [&](int q0) {
+        const int q = q0 + ql;
         active_n = q < nown;
         gi_n = 0; slot_n = 0;
         if (active_n) tile_own(s.d, q, gi_n, slot_n);
-        const uint16_t *row = nlist + (int64_t)gi_n * pitch + sub * EPL;
+        const uint16_t *row = A.nlist + (int64_t)gi_n * A.pitch + sub * EPL;
+        if (nve && active_n) {
+            float4 *o = own + ql;
+            if (sub == 0) { cp_async_cg16(o, nv.vel + gi_n); if (nv.kick_drift) cp_async_cg16(o + PPB, A.pos + gi_n); }
+            if (sub == 1 && nv.kick_drift) cp_async_cg16(o + 2 * PPB, nv.pos_build + gi_n);
+        }
 #pragma unroll
         for (int u = 0; u < PF; u++) {
             if (active_n) cp_async<EPL * 2>(ring + u * ring_stride, row + u * G);
@@ -141,35 +318,36 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
         }
     };
 
-    bool fits;
-    if (g.fast) {
-        // the list build left this tile's descriptor and the storage index of every slot behind
-        if (threadIdx.x < sizeof(TileDesc) / 4)
-            reinterpret_cast<int *>(&s.d)[threadIdx.x] = __ldg(reinterpret_cast<const int *>(desc + blockIdx.x) + threadIdx.x);
-        __syncthreads();
-        fits = s.d.nslots <= g.cap;
-        prep(0, fits ? s.d.nown : 0);            // list copies in flight while the tile is staged
-        if (fits) tile_stage_from_table(s.d, stage_src + (int64_t)blockIdx.x * g.cap, pos, stage, g.L);
+    prep(0);                                     // list and integration data in flight behind the staging copies
+    if (g.fast && fits) {
+        mbar_wait(&s.mbar, 0);
+        if (s.fix) {
+            // the halo reaches a face of the box: move every staged particle to the image nearest to the tile centre.
+            // Each thread fixes what it will not read before the barrier below.
+            const float L = g.L, hL = 0.5f * g.L, cx = s.d.cx, cy = s.d.cy, cz = s.d.cz;
+            for (int sl = 1 + threadIdx.x; sl < s.d.nslots; sl += nthreads) {
+                float4 p = stage[sl];
+                p.x = tile_image(p.x, cx, L, hL); p.y = tile_image(p.y, cy, L, hL); p.z = tile_image(p.z, cz, L, hL);
+                stage[sl] = p;
+            }
+            __syncthreads();
+        }
     } else {
-        TileCtx t;
-        tile_decode(g, blockIdx.x, t);
-        fits = tile_tables(g, cell_start, t, s, flags);
-        prep(0, fits ? s.d.nown : 0);
-        if (fits) tile_stage_positions(g, t, s, pos, stage, nullptr);
+        __syncthreads();
     }
-    __syncthreads();
 
-    const PairParam pp1 = params[0];
+    const PairParam pp1 = A.params[0];
+    const float c12 = 12.0f * pp1.lj1, c6 = 6.0f * pp1.lj2;
     const float hdt = 0.5f * nv.dt, hL = 0.5f * g.L, L = g.L;
+    const unsigned char *stage_b = reinterpret_cast<const unsigned char *>(stage);
     bool exceed = false;
 
-    const int nown = fits ? s.d.nown : 0;
     for (int q0 = 0; q0 < nown; q0 += PPB) {     // block-uniform trip count: the shuffles need whole warps
         const bool active = active_n;
         const int gi = gi_n;
         const float4 pi = stage[slot_n];         // slot 0 (the dummy) for idle thread groups
-        const uint16_t *row = nlist + (int64_t)gi * pitch + sub * EPL;
-        const PairParam *prow = ONE_TYPE ? nullptr : s_params + __float_as_int(pi.w) * ntypes;
+        const uint16_t *row = A.nlist + (int64_t)gi * A.pitch + sub * EPL;
+        const PairParam *prow = ONE_TYPE ? nullptr : s_params + __float_as_int(pi.w) * A.ntypes;
         Acc a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
         if (active) {
@@ -177,137 +355,144 @@ lj_tile_kernel(TileGeom g, const int *__restrict__ cell_start, const float4 *__r
             cp_async_wait<PF - 1>();
             Entries<EPL> ent;
             ent.v = ring[0];
-            for (int k = 0; k < pitch; k += G) {
+            for (int k = 0; k < A.pitch; k += G) {
                 if ((ent.v.x & 0xffffu) == 0u) break;                    // padding: the row is over for this thread
                 cp_async<EPL * 2>(ring + c * ring_stride, row + k + PF * G);   // refill PF iterations ahead (reads past the
                 cp_async_commit();                                       // row's end are harmless: the array has slack)
                 c = (c + 1 == PF) ? 0 : c + 1;
-                int sl[EPL];
-                unpack_entries<EPL>(ent, sl);
+                unsigned off[EPL];
+                unpack_entries<EPL, SCALED>(ent, off);
+#ifdef HB_EXPERIMENT_BANKS   // timing experiment only (wrong physics): force the bank group of every gather to the conflict-free pattern
+#pragma unroll
+                for (int e = 0; e < EPL; e++) off[e] = (off[e] & ~0x70u) | ((unsigned)((ql + sub * EPL + e) & 7) << 4);
+#endif
                 float4 pj[EPL];
 #pragma unroll
-                for (int e = 0; e < EPL; e++) pj[e] = stage[sl[e]];
+                for (int e = 0; e < EPL; e++) pj[e] = *reinterpret_cast<const float4 *>(stage_b + off[e]);
                 cp_async_wait<PF - 1>();                                 // the next group of entries, read before the
                 ent.v = ring[c * ring_stride];                           // arithmetic so that its latency hides behind it
 #pragma unroll
                 for (int e = 0; e < EPL; e++) {
-                    if (ONE_TYPE) pair_term<THERMO>(pi, pj[e], pp1, a);
-                    else pair_term<THERMO>(pi, pj[e], prow[__float_as_int(pj[e].w)], a);
+                    if (ONE_TYPE) {
+                        pair_term<THERMO>(pi, pj[e], c12, c6, pp1.rcut2, pp1.lj1, pp1.lj2, pp1.eshift, a);
+                    } else {
+                        const PairParam pp = prow[__float_as_int(pj[e].w)];
+                        pair_term<THERMO>(pi, pj[e], 12.0f * pp.lj1, 6.0f * pp.lj2, pp.rcut2, pp.lj1, pp.lj2, pp.eshift, a);
+                    }
                 }
             }
         }
-        cp_async_wait<0>();                          // nothing of this pass may land after the next pass's copies start
-        if (q0 + PPB < nown) prep(q0 + PPB, nown);   // they fly during the reduction and the integration below
-        // what the integration will need, all three loads in flight at once and behind the reduction (ncu: placed
-        // where they are used they were three L2 round trips in a row at the very end of the block; issued before
-        // the pair loop they cost registers the loop needs)
-        float4 v_in = make_float4(0.f, 0.f, 0.f, 0.f), p_in = v_in, pb_in = v_in;
-        if (do_nve && active && sub == 0) {
-            v_in = nv.vel[gi];
-            if (nv.kick_drift) { p_in = pos[gi]; pb_in = nv.pos_build[gi]; }
-        }
+        cp_async_wait<0>();                          // the own data of this pass has landed; nothing of this pass may land
+        __syncwarp();                                //   after the next pass's copies start; lane 1's copy visible to lane 0
+        const float4 *o = own + ql;
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f), p = v, pb = v;
+        if (nve && active && sub == 0) { v = o[0]; if (nv.kick_drift) { p = o[PPB]; pb = o[2 * PPB]; } }
+        if (q0 + PPB < nown) prep(q0 + PPB);             // the next pass's copies fly during the reduction and the integration
 
 #pragma unroll
-        for (int o = TPP >> 1; o > 0; o >>= 1) {
-            a.fx += __shfl_xor_sync(0xffffffffu, a.fx, o);
-            a.fy += __shfl_xor_sync(0xffffffffu, a.fy, o);
-            a.fz += __shfl_xor_sync(0xffffffffu, a.fz, o);
+        for (int o2 = TPP >> 1; o2 > 0; o2 >>= 1) {
+            a.fx += __shfl_xor_sync(0xffffffffu, a.fx, o2);
+            a.fy += __shfl_xor_sync(0xffffffffu, a.fy, o2);
+            a.fz += __shfl_xor_sync(0xffffffffu, a.fz, o2);
             if (THERMO) {
-                a.u += __shfl_xor_sync(0xffffffffu, a.u, o);
-                a.wxx += __shfl_xor_sync(0xffffffffu, a.wxx, o);
-                a.wxy += __shfl_xor_sync(0xffffffffu, a.wxy, o);
-                a.wxz += __shfl_xor_sync(0xffffffffu, a.wxz, o);
-                a.wyy += __shfl_xor_sync(0xffffffffu, a.wyy, o);
-                a.wyz += __shfl_xor_sync(0xffffffffu, a.wyz, o);
-                a.wzz += __shfl_xor_sync(0xffffffffu, a.wzz, o);
+                a.u += __shfl_xor_sync(0xffffffffu, a.u, o2);
+                a.wxx += __shfl_xor_sync(0xffffffffu, a.wxx, o2);
+                a.wxy += __shfl_xor_sync(0xffffffffu, a.wxy, o2);
+                a.wxz += __shfl_xor_sync(0xffffffffu, a.wxz, o2);
+                a.wyy += __shfl_xor_sync(0xffffffffu, a.wyy, o2);
+                a.wyz += __shfl_xor_sync(0xffffffffu, a.wyz, o2);
+                a.wzz += __shfl_xor_sync(0xffffffffu, a.wzz, o2);
             }
         }
         if (!active) continue;
         // U_i = 1/2 sum V, W_i = 1/2 sum d f (reading c6.i)
-        if (sub == 0) {
-            force[gi] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
-            if (do_nve) {
-                // reading c7, operation by operation as nve_kernel does it
-                float4 v = v_in;
-                if (nv.kick_prev) {
-                    v.x = __fmaf_rn(hdt, a.fx, v.x);
-                    v.y = __fmaf_rn(hdt, a.fy, v.y);
-                    v.z = __fmaf_rn(hdt, a.fz, v.z);
-                }
-                if (nv.kick_drift) {
-                    v.x = __fmaf_rn(hdt, a.fx, v.x);
-                    v.y = __fmaf_rn(hdt, a.fy, v.y);
-                    v.z = __fmaf_rn(hdt, a.fz, v.z);
-                    float4 p = p_in;      // the stored position: pi may be another periodic image of it
-                    p.x = __fmaf_rn(nv.dt, v.x, p.x);
-                    p.y = __fmaf_rn(nv.dt, v.y, p.y);
-                    p.z = __fmaf_rn(nv.dt, v.z, p.z);
-                    if (p.x >= hL) { p.x -= L; nv.image[gi] += 1; } else if (p.x < -hL) { p.x += L; nv.image[gi] -= 1; }
-                    if (p.y >= hL) { p.y -= L; nv.image[N + gi] += 1; } else if (p.y < -hL) { p.y += L; nv.image[N + gi] -= 1; }
-                    if (p.z >= hL) { p.z -= L; nv.image[2 * (int64_t)N + gi] += 1; }
-                    else if (p.z < -hL) { p.z += L; nv.image[2 * (int64_t)N + gi] -= 1; }
-                    nv.pos_out[gi] = p;
-                    const float4 pb = pb_in;
-                    float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
-                    if (dx >= hL) dx -= L; else if (dx < -hL) dx += L;
-                    if (dy >= hL) dy -= L; else if (dy < -hL) dy += L;
-                    if (dz >= hL) dz -= L; else if (dz < -hL) dz += L;
-                    exceed = exceed || (dx * dx + dy * dy + dz * dz) > nv.half_buff2;
-                }
-                nv.vel[gi] = v;
-            }
-        } else if (THERMO && TPP >= 4 && sub == 1) {
-            virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
-        } else if (THERMO && TPP >= 4 && sub == 2) {
-            virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
+        if (THERMO && sub == TPP - 1) {
+            A.virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
+            A.virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
         }
-        if (THERMO && TPP < 4 && sub == TPP - 1) {
-            virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
-            virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
+        if (sub != 0) continue;
+        if (THERMO) A.force[gi] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
+        if (!nve) continue;
+        // reading c7, operation by operation as nve_kernel does it
+        if (nv.kick_prev) {
+            v.x = __fmaf_rn(hdt, a.fx, v.x);
+            v.y = __fmaf_rn(hdt, a.fy, v.y);
+            v.z = __fmaf_rn(hdt, a.fz, v.z);
         }
+        if (nv.kick_drift) {
+            v.x = __fmaf_rn(hdt, a.fx, v.x);
+            v.y = __fmaf_rn(hdt, a.fy, v.y);
+            v.z = __fmaf_rn(hdt, a.fz, v.z);
+            // p is the stored position: the staged one may be another periodic image of it
+            p.x = __fmaf_rn(nv.dt, v.x, p.x);
+            p.y = __fmaf_rn(nv.dt, v.y, p.y);
+            p.z = __fmaf_rn(nv.dt, v.z, p.z);
+            if (p.x >= hL) { p.x -= L; nv.image[gi] += 1; } else if (p.x < -hL) { p.x += L; nv.image[gi] -= 1; }
+            if (p.y >= hL) { p.y -= L; nv.image[A.N + gi] += 1; } else if (p.y < -hL) { p.y += L; nv.image[A.N + gi] -= 1; }
+            if (p.z >= hL) { p.z -= L; nv.image[2 * (int64_t)A.N + gi] += 1; }
+            else if (p.z < -hL) { p.z += L; nv.image[2 * (int64_t)A.N + gi] -= 1; }
+            nv.pos_out[gi] = p;
+            float dx = p.x - pb.x, dy = p.y - pb.y, dz = p.z - pb.z;
+            if (dx >= hL) dx -= L; else if (dx < -hL) dx += L;
+            if (dy >= hL) dy -= L; else if (dy < -hL) dy += L;
+            if (dz >= hL) dz -= L; else if (dz < -hL) dz += L;
+            exceed = exceed || (dx * dx + dy * dy + dz * dz) > nv.half_buff2;
+        }
+        nv.vel[gi] = v;
     }
 
-    if (do_nve && nv.kick_drift) {
-        if (exceed) flags[nv.need_set] = 1;
+    if (drift) {
+        if (exceed) A.flags[nv.need_set] = 1;
         if (nv.use_cond) {
             __syncthreads();
             if (threadIdx.x == 0) {
                 __threadfence();
-                const int ticket = atomicAdd(&flags[FL_DONE_CTR], 1);
-                if (ticket == (int)gridDim.x - 1) {
+                const int ticket = atomicAdd(&A.flags[FL_DONE_CTR], 1);
+                if (ticket == (int)(gridDim.x * gridDim.y * gridDim.z) - 1) {
                     __threadfence();
-                    const int need = *((volatile int *)&flags[nv.need_set]);
+                    const int need = *((volatile int *)&A.flags[nv.need_set]);
                     cudaGraphSetConditional(nv.cond, need ? 1u : 0u);
-                    flags[FL_DONE_CTR] = 0;
+                    A.flags[FL_DONE_CTR] = 0;
                 }
             }
         }
     }
 }
 
+static int force_ppb(const hb_system *h) { return force_block_of(h) / h->tun.tpp; }
+
 size_t force_smem_bytes(const hb_system *h)
 {
-    // staged positions, pair table, ring of 4 async list copies (16 B at most) per thread
+    // staged positions, pair table, ring of 4 async list copies (16 B at most) per thread, own data (2 buffers x 3 arrays)
+    // and forces of a pass
     return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? ((sizeof(PairParam) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
-           (size_t)4 * 16 * force_block_of(h);
+           (size_t)4 * 16 * force_block_of(h) + (size_t)3 * 16 * force_ppb(h) + (h->geom.fast ? 0 : sizeof(TileShared));
 }
 
-template <int TPP, int EPL, bool THERMO>
-static cudaError_t launch_force_tt(hb_system *h, const NveArgs *nve)
+template <int TPP, int EPL, bool THERMO, bool SCALED>
+static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
 {
     const size_t smem = force_smem_bytes(h);
-    const unsigned grid = (unsigned)h->geom.ntiles;
-    NveArgs nv{};
-    if (nve) nv = *nve;
+    const dim3 grid((unsigned)h->geom.ntx, (unsigned)h->geom.nty, (unsigned)h->geom.ntz);
+    ForceArgs A{};
+    A.g = h->geom;
+    A.cell_start = h->cell_start;
+    A.pos = h->pos();
+    A.nlist = h->nlist;
+    A.pitch = h->row_pitch;
+    A.N = (int)h->N;
+    A.ntypes = h->ntypes;
+    A.params = h->params;
+    A.force = h->force;
+    A.virial = h->virial;
+    A.flags = h->flags;
+    A.do_nve = nve ? 1 : 0;
+    if (nve) A.nv = *nve;
     cudaError_t e;
 #define LJ_LAUNCH(ONE)                                                                                                      \
-    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
     if (e != cudaSuccess) return e;                                                                                         \
-    lj_tile_kernel<TPP, EPL, ONE, THERMO><<<grid, force_block_of(h), smem, h->stream>>>(h->geom, h->cell_start, h->pos(), h->nlist,      \
-                                                                           h->nlistn, h->row_pitch, (int)h->N, h->ntypes,  \
-                                                                           h->params, h->force, h->virial, h->flags,       \
-                                                                           nve ? 1 : 0, nv, h->stage_src,                  \
-                                                                           (const TileDesc *)h->tile_desc);
+    lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED><<<grid, force_block_of(h), smem, h->stream>>>(A);
     if (h->ntypes == 1) { LJ_LAUNCH(true) } else { LJ_LAUNCH(false) }
 #undef LJ_LAUNCH
     h->stats.kernel_launches++;
@@ -319,8 +504,10 @@ static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
 {
     // energies and virials of a step can only be read after hb_run_nve returns: with thermo_every = 0 the inner
     // steps of a chunk (both half kicks fused in) compute forces only
-    if (nve && nve->forces_only) return launch_force_tt<TPP, EPL, false>(h, nve);
-    return launch_force_tt<TPP, EPL, true>(h, nve);
+    const bool thermo = !(nve && nve->forces_only);
+    const bool scaled = h->geom.eshift == 4;
+    if (thermo) return scaled ? launch_force_tts<TPP, EPL, true, true>(h, nve) : launch_force_tts<TPP, EPL, true, false>(h, nve);
+    return scaled ? launch_force_tts<TPP, EPL, false, true>(h, nve) : launch_force_tts<TPP, EPL, false, false>(h, nve);
 }
 
 cudaError_t launch_force(hb_system *h, const NveArgs *nve)

@@ -5,9 +5,17 @@
 #include <cstring>
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "hb_internal.cuh"
 
 namespace {
+
+// NVTX range per stage (tracing): shows up in nsys / ncu timelines, costs nothing without a tool.
+struct Range {
+    explicit Range(const char *name) { nvtxRangePushA(name); }
+    ~Range() { nvtxRangePop(); }
+};
 
 int coop_mode(const hb_system *h) { return h->tun.coop_rebuild >= 0 ? h->tun.coop_rebuild : (h->N < 200000 ? 2 : 1); }
 int rebuild_kernels(const hb_system *h) { return coop_mode(h) == 2 ? 1 : coop_mode(h) == 1 ? 2 : 5; }  // see enqueue_rebuild
@@ -80,9 +88,11 @@ int upload_params(hb_system *h)
 
 int stage_cap_max(const hb_system *h)
 {
-    // what is left of the opt-in shared memory after the static tables and the list kernel's candidate lists
-    const int64_t left = (int64_t)h->smem_max - 20 * 1024;
-    return (int)std::min<int64_t>(65535, left / 16);
+    // what is left of the opt-in shared memory after the static tables (TileShared and the scan scratch, < 4 KB) and
+    // the larger of the two kernels' extras beside the staging area itself (both functions count cap * 16 bytes)
+    const size_t extra = std::max(nlist_smem_bytes(h), force_smem_bytes(h)) - (size_t)h->geom.cap * 16;
+    const int64_t left = (int64_t)h->smem_max - 4096 - (int64_t)extra;
+    return (int)std::max<int64_t>(64, std::min<int64_t>(65535, left / 16));
 }
 
 // Tile dimensions and staging capacity (tile.cuh).  Tunables override the choice.
@@ -122,7 +132,7 @@ int choose_tiles(hb_system *h, int min_cap)
     if (cap <= 0) {
         const double per_cell = (double)h->N / (double)h->ncells;
         const double est = per_cell * (tx + 2) * (ty + 2) * (tz + 2);
-        cap = (int)(1.5 * est) + 64;
+        cap = (int)(1.3 * est) + 48;
     }
     cap = std::max(cap, min_cap);
     cap = round_up(std::max(cap, 64), 32);
@@ -149,23 +159,7 @@ int choose_tiles(hb_system *h, int min_cap)
         const int tmax = std::max(tx, std::max(ty, tz));
         g.fast = ((0.5 * tmax + 1.0) * w + 2.0 * (double)h->r_buff + 0.05 * w < 0.5 * (double)h->L) ? 1 : 0;
     }
-    if (g.fast) {
-        const int64_t need_src = (int64_t)g.ntiles * g.cap;
-        if (need_src > h->stage_src_len) {
-            dev_free_t(h, h->stage_src);
-            HB_TRY(dev_alloc_t(h, &h->stage_src, (size_t)need_src));
-            h->stage_src_len = need_src;
-            destroy_graphs(h);
-        }
-        const int64_t need_desc = (int64_t)g.ntiles * 416;   // sizeof(TileDesc), tile.cuh
-        if (need_desc > h->tile_desc_len) {
-            dev_free(h, h->tile_desc);
-            h->tile_desc = nullptr;
-            HB_TRY(dev_alloc(h, &h->tile_desc, (size_t)need_desc));
-            h->tile_desc_len = need_desc;
-            destroy_graphs(h);
-        }
-    }
+    g.eshift = g.cap <= 4096 ? 4 : 0;
     if (memcmp(&g, &h->geom, sizeof g) != 0) {
         destroy_graphs(h);
         h->nlist_valid = false;
@@ -444,6 +438,8 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     cudaStream_t saved = h->stream;
     const int64_t saved_launches = h->stats.kernel_launches;
     const int saved_cur = h->cur, saved_parity = h->parity;
+    h->cur = 0;       // every chunk starts from posbuf[0] and drift parity 0 (run_chunk sees to it): one graph per n
+    h->parity = 0;
     int rc = HB_OK;
     auto fail = [&](const char *what, cudaError_t e) {
         h->err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -539,6 +535,7 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     }
     out->g = g;
     out->e = ex;
+    h->stats.graph_builds++;
     out->nkernels_fixed = (fuse ? n + 1 : 2 * n + 1) + (mode == 1 ? n * rebuild_kernels(h) : 0);
     return HB_OK;
 }
@@ -596,36 +593,60 @@ int step_sync(hb_system *h, float dt)
     return HB_OK;
 }
 
+// Every chunk starts from posbuf[0] and drift parity 0, so that ONE graph per chunk length serves every call.
+int normalize_for_chunk(hb_system *h)
+{
+    if (h->cur != 0) {
+        HB_CK(cudaMemcpyAsync(h->posbuf[0], h->posbuf[1], (size_t)h->N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
+        h->cur = 0;
+    }
+    h->parity = 0;
+    return clear_need_flags(h);   // no decision is pending between chunks: every drift's rebuild ran inside its chunk
+}
+
+int chunk_kernels(const hb_system *h, int n) { return (h->tun.fuse_nve ? n + 1 : 2 * n + 1) + n * rebuild_kernels(h); }
+
+// The chunk lengths hb_run_nve uses are graph_steps and the powers of two below it; all their graphs are built at
+// the first call, so that no later call captures or instantiates anything (hb_stats: graph_builds).
+int ensure_graphs(hb_system *h, float dt)
+{
+    if (dt != h->graph_dt) { destroy_graphs(h); h->graph_dt = dt; }
+    if (!h->graphs.empty() || h->tun.graph_mode == 0 || h->tun.graph_mode == 3) return HB_OK;
+    Range r("hb:build_graphs");
+    std::vector<int> sizes{h->tun.graph_steps};
+    for (int n = 1; n < h->tun.graph_steps; n <<= 1) sizes.push_back(n);
+    for (int n : sizes) {
+        hb_system::GraphEntry ge;
+        HB_TRY(build_graph(h, n, dt, &ge));
+        h->graphs.emplace((int64_t)n, ge);
+    }
+    return HB_OK;
+}
+
 int run_chunk(hb_system *h, float dt, int n)
 {
     if (h->tun.graph_mode == 0) {
         for (int s = 0; s < n; s++) HB_TRY(step_sync(h, dt));
         return HB_OK;
     }
+    Range r("hb:chunk");
     for (int attempt = 0; attempt < 8; attempt++) {
         HB_TRY(ensure_forces(h));
-        if (dt != h->graph_dt) { destroy_graphs(h); h->graph_dt = dt; }
+        HB_TRY(ensure_graphs(h, dt));
+        HB_TRY(normalize_for_chunk(h));
         const bool plain = h->tun.graph_mode == 3;   // the launches of mode 1, issued one by one (for profilers)
-        const int64_t key = ((int64_t)n << 2) | ((h->cur & 1) << 1) | (h->parity & 1);
-        auto it = h->graphs.find(key);
-        if (plain) {
-            if (it == h->graphs.end()) {
-                hb_system::GraphEntry ge;
-                ge.nkernels_fixed = (h->tun.fuse_nve ? n + 1 : 2 * n + 1) + n * rebuild_kernels(h);
-                it = h->graphs.emplace(key, ge).first;
-            }
-        } else if (it == h->graphs.end()) {
+        auto it = h->graphs.find((int64_t)n);
+        if (!plain && it == h->graphs.end()) {       // a length outside the prebuilt set (never from hb_run_nve)
             hb_system::GraphEntry ge;
             HB_TRY(build_graph(h, n, dt, &ge));
-            it = h->graphs.emplace(key, ge).first;
+            it = h->graphs.emplace((int64_t)n, ge).first;
         }
         HB_TRY(backup_state(h));
         const int builds_before = h->h_flags[FL_BUILDS];
         if (plain) {
-            const int c0 = h->cur, p0 = h->parity;
             const int64_t l0 = h->stats.kernel_launches;
             HB_TRY(enqueue_chunk_pred(h, n, dt));
-            h->cur = c0; h->parity = p0;            // advanced again below, as after a graph launch
+            h->cur = 0; h->parity = 0;              // advanced again below, as after a graph launch
             h->stats.kernel_launches = l0;
         } else {
             HB_CK(cudaGraphLaunch(it->second.e, h->stream));
@@ -633,28 +654,33 @@ int run_chunk(hb_system *h, float dt, int n)
         }
         HB_TRY(read_flags(h));
         const int nb = h->h_flags[FL_BUILDS] - builds_before;
-        h->stats.kernel_launches += it->second.nkernels_fixed + (h->tun.graph_mode == 2 ? nb * rebuild_kernels(h) : 0);
+        h->stats.kernel_launches += chunk_kernels(h, n) - (h->tun.graph_mode == 2 ? (n - nb) * rebuild_kernels(h) : 0);
         h->stats.rebuilds = h->h_flags[FL_BUILDS];
         if (h->tun.fuse_nve) h->cur ^= (n - 1) & 1;
         h->parity += n;
         h->moved = true;
         h->forces_valid = true;   // the graph's last kernel evaluated the forces in the final order
-        if (h->h_flags[FL_BAD]) {
-            h->err = "a particle is non-finite or outside the box";
-            set_flag(h, FL_BAD, 0);
-            return HB_ENAN;
-        }
-        if (!h->h_flags[FL_OVERFLOWED] && !h->h_flags[FL_STAGE_OVER]) {
+        const int rows_needed = h->h_flags[FL_OVERFLOWED], slots_needed = h->h_flags[FL_STAGE_OVER];
+        if (!rows_needed && !slots_needed) {
+            if (h->h_flags[FL_BAD]) {
+                h->err = "a particle is non-finite or outside the box";
+                set_flag(h, FL_BAD, 0);
+                h->nlist_valid = h->cells_valid = h->forces_valid = false;
+                return HB_ENAN;
+            }
             if (nb > 0) h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
             h->stats.steps += n;
             return HB_OK;
         }
-        // some build inside the chunk overflowed its rows or its staging area: go back, grow, redo
-        const int rows_needed = h->h_flags[FL_OVERFLOWED], slots_needed = h->h_flags[FL_STAGE_OVER];
+        // Some build inside the chunk overflowed its rows or its staging area: go back, grow, redo.
+        // This comes BEFORE the bad-particle test: the steps after the overflowing build ran with truncated rows
+        // or skipped tiles, so whatever they flagged (a particle thrown out of the box) is a consequence and is
+        // undone with them.
         h->stats.overflow_retries++;
         HB_TRY(restore_state(h));
         HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
         HB_TRY(set_flag(h, FL_STAGE_OVER, 0));
+        HB_TRY(set_flag(h, FL_BAD, 0));
         if (slots_needed) HB_TRY(choose_tiles(h, (int)(slots_needed * (1.0 + 0.01 * h->tun.grow_pct)) + 32));
         if (rows_needed) HB_TRY(ensure_rows(h, (int)(rows_needed * (1.0 + 0.01 * h->tun.grow_pct)) + 8));
         HB_TRY(build_nlist_sync(h));
@@ -663,19 +689,17 @@ int run_chunk(hb_system *h, float dt, int n)
     return HB_ENOMEM;
 }
 
-int ensure_stage(hb_system *h, void **stage, size_t *cap, size_t bytes)
+// accessor staging area, owned by the handle (grows, never shrinks)
+int ensure_stage(hb_system *h, size_t bytes)
 {
-    if (bytes <= *cap) return HB_OK;
-    dev_free(h, *stage);
-    *stage = nullptr;
-    *cap = 0;
-    HB_TRY(dev_alloc(h, stage, bytes));
-    *cap = bytes;
+    if (bytes <= h->acc_cap) return HB_OK;
+    dev_free(h, h->acc_stage);
+    h->acc_stage = nullptr;
+    h->acc_cap = 0;
+    HB_TRY(dev_alloc(h, &h->acc_stage, bytes));
+    h->acc_cap = bytes;
     return HB_OK;
 }
-
-struct Stage { void *p = nullptr; size_t cap = 0; };
-std::map<hb_system *, Stage> g_stage;  // accessor staging, one per handle
 
 }  // namespace
 
@@ -734,8 +758,12 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     HB_TRY(dev_alloc_t(h, &h->flags, (size_t)FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_flags, sizeof(int) * FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_thermo, sizeof(double) * 16));
+    HB_CK(cudaMallocHost((void **)&h->h_total, sizeof(int) * 2));
+    HB_TRY(dev_alloc_t(h, &h->acc_counts, n + 1));
+    HB_TRY(dev_alloc_t(h, &h->acc_rows, n + 2));
     memset(h->h_flags, 0, sizeof(int) * FL_COUNT);
     HB_CK(cudaMemsetAsync(h->flags, 0, sizeof(int) * FL_COUNT, h->stream));
+    HB_CK(cudaMemsetAsync(h->posbuf[1], 0, sizeof(float4) * n, h->stream));   // never read before it is written, but never garbage
     HB_CK(cudaMemsetAsync(h->force, 0, sizeof(float4) * n, h->stream));
     HB_CK(cudaMemsetAsync(h->virial, 0, sizeof(float4) * 2 * n, h->stream));
     int dev = 0, sms = 148, smem = 227 * 1024;
@@ -755,12 +783,14 @@ int hb_destroy(hb_system *h)
     if (!h) return HB_EINVAL;
     cudaStreamSynchronize(h->stream);
     destroy_graphs(h);
-    auto it = g_stage.find(h);
-    if (it != g_stage.end()) { dev_free(h, it->second.p); g_stage.erase(it); }
+    dev_free(h, h->acc_stage);
+    dev_free(h, h->acc_counts);
+    dev_free(h, h->acc_rows);
+    if (h->h_total) cudaFreeHost(h->h_total);
     void *ptrs[] = {h->posbuf[0], h->posbuf[1], h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->vel2,
                     h->force2, h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_image,
                     h->bk_tag, h->params, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
-                    h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->stage_src, h->tile_desc, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
+                    h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
                     h->flags, h->thermo_part};
     for (void *p : ptrs) dev_free(h, p);
     if (h->h_flags) cudaFreeHost(h->h_flags);
@@ -779,10 +809,9 @@ int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type, const 
     const float *dpos = pos_xyz, *dvel = vel_xyz;
     const int32_t *dtype = type, *dimg = image;
     if (!on_device) {
-        Stage &st = g_stage[h];
         const size_t bytes = N * (3 * 4 + 4 + 3 * 4 + 3 * 4);
-        HB_TRY(ensure_stage(h, &st.p, &st.cap, bytes));
-        char *base = (char *)st.p;
+        HB_TRY(ensure_stage(h, bytes));
+        char *base = (char *)h->acc_stage;
         float *spos = (float *)base;
         float *svel = (float *)(base + N * 12);
         int32_t *stype = (int32_t *)(base + N * 24);
@@ -794,11 +823,17 @@ int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type, const 
         dpos = spos; dvel = svel; dtype = type ? stype : nullptr; dimg = image ? simg : nullptr;
     }
     HB_CK(launch_pack_state(h, dpos, dtype, dvel, dimg));
-    if (!on_device) HB_CK(cudaStreamSynchronize(h->stream));  // the caller's host buffers may be pageable
+    HB_TRY(read_flags(h));    // synchronises: the caller's host buffers may be pageable; and the type check below
     h->have_state = true;
     h->cells_valid = h->nlist_valid = h->forces_valid = h->bk_valid = false;
     h->moved = true;
     h->since_sort = -1;
+    if (h->h_flags[FL_BADTYPE]) {
+        HB_TRY(set_flag(h, FL_BADTYPE, 0));
+        h->have_state = false;
+        h->err = "a particle type is outside 0 .. ntypes-1";
+        return HB_EINVAL;
+    }
     return HB_OK;
 }
 
@@ -812,9 +847,8 @@ int hb_get_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, in
         if (order) HB_CK(cudaMemcpyAsync(order, h->tag, N * 4, cudaMemcpyDeviceToDevice, h->stream));
         return HB_OK;
     }
-    Stage &st = g_stage[h];
-    HB_TRY(ensure_stage(h, &st.p, &st.cap, N * 40));
-    char *base = (char *)st.p;
+    HB_TRY(ensure_stage(h, N * 40));
+    char *base = (char *)h->acc_stage;
     float *spos = (float *)base;
     float *svel = (float *)(base + N * 12);
     int32_t *stype = (int32_t *)(base + N * 24);
@@ -848,6 +882,7 @@ int hb_set_rcut_pair(hb_system *h, const double *rcut)
 int hb_build_cells(hb_system *h)
 {
     HB_NEED(h);
+    Range nvtx_range("hb_build_cells");
     if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
     HB_TRY(configure_geometry(h));
     if (h->cells_valid && !h->moved) return HB_OK;   // the cell list of these very positions is in place
@@ -869,6 +904,7 @@ int hb_build_cells(hb_system *h)
 int hb_build_nlist(hb_system *h, double r_cut, double r_buff)
 {
     HB_NEED(h);
+    Range nvtx_range("hb_build_nlist");
     if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
     if (!(r_buff >= 0.0)) { h->err = "r_buff must be >= 0"; return HB_EINVAL; }
     if (r_cut > 0.0 && !h->rcut_user) {
@@ -897,6 +933,7 @@ int hb_needs_rebuild(hb_system *h, int *need)
 int hb_compute_lj(hb_system *h, int shift_mode)
 {
     HB_NEED(h);
+    Range nvtx_range("hb_compute_lj");
     if (shift_mode != HB_SHIFT_NONE && shift_mode != HB_SHIFT_ENERGY) { h->err = "unknown shift mode"; return HB_EINVAL; }
     if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
     if (shift_mode != h->shift_mode) {
@@ -911,6 +948,7 @@ int hb_compute_lj(hb_system *h, int shift_mode)
 int hb_step_nve(hb_system *h, double dt)
 {
     HB_NEED(h);
+    Range nvtx_range("hb_step_nve");
     if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
     if (h->m == 0) HB_TRY(configure_geometry(h));
     return step_sync(h, (float)dt);
@@ -919,6 +957,7 @@ int hb_step_nve(hb_system *h, double dt)
 int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
 {
     HB_NEED(h);
+    Range nvtx_range("hb_run_nve");
     if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
     if (nsteps < 0 || sort_period < 0) return HB_EINVAL;
     if (h->m == 0) HB_TRY(configure_geometry(h));
@@ -932,6 +971,11 @@ int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
         }
         int64_t n = std::min<int64_t>(h->tun.graph_steps, nsteps - done);
         if (sort_period > 0) n = std::min<int64_t>(n, sort_period - h->since_sort);
+        if (n < h->tun.graph_steps) {          // a remainder: the largest power of two that fits (graphs exist for those)
+            int64_t p2 = 1;
+            while (2 * p2 <= n) p2 *= 2;
+            n = p2;
+        }
         HB_TRY(run_chunk(h, (float)dt, (int)n));
         done += n;
         if (h->since_sort >= 0) h->since_sort += n;
@@ -942,14 +986,20 @@ int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
 int hb_sort(hb_system *h)
 {
     HB_NEED(h);
+    Range nvtx_range("hb_sort");
     return sort_internal(h);
 }
 
 int hb_thermo(hb_system *h, hb_thermo_t *out)
 {
     HB_NEED(h);
+    Range nvtx_range("hb_thermo");
     if (!out) return HB_EINVAL;
     if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    if (!h->forces_valid) {       // U, W and P come from the per-particle arrays of the last force evaluation
+        if (h->m == 0) HB_TRY(configure_geometry(h));
+        HB_TRY(ensure_forces(h));
+    }
     HB_CK(launch_thermo(h));
     HB_CK(cudaMemcpyAsync(h->h_thermo, h->thermo_part + (int64_t)h->thermo_blocks * 11, sizeof(double) * 11,
                           cudaMemcpyDeviceToHost, h->stream));
@@ -987,45 +1037,24 @@ int hb_get_nlist(hb_system *h, int64_t *row_start, uint32_t *nbr_tags, int on_de
     if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
     if (!row_start) { h->err = "row_start is NULL"; return HB_EINVAL; }
     const size_t N = (size_t)h->N;
-    // counts by tag -> host prefix sum (binary integer work, done once per call)
-    int *d_counts = nullptr;
-    HB_TRY(dev_alloc_t(h, &d_counts, N));
-    std::vector<int> counts(N);
-    std::vector<int64_t> rs(N + 1);
-    int rc = HB_OK;
-    int64_t *d_rs = nullptr;
-    uint32_t *d_out = nullptr;
-    do {
-        if (launch_nlist_counts_by_tag(h, d_counts) != cudaSuccess ||
-            cudaMemcpyAsync(counts.data(), d_counts, N * 4, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
-            cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
-        rs[0] = 0;
-        for (size_t i = 0; i < N; i++) rs[i + 1] = rs[i] + counts[i];
-        if (on_device) {
-            if (cudaMemcpyAsync(row_start, rs.data(), (N + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
-        } else {
-            memcpy(row_start, rs.data(), (N + 1) * 8);
-        }
-        if (nbr_tags) {
-            const int64_t *rs_dev = row_start;
-            if (!on_device) {
-                if ((rc = dev_alloc_t(h, &d_rs, N + 1)) != HB_OK) break;
-                if (cudaMemcpyAsync(d_rs, rs.data(), (N + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
-                rs_dev = d_rs;
-                if ((rc = dev_alloc_t(h, &d_out, (size_t)rs[N] + 1)) != HB_OK) break;
-            }
-            uint32_t *outp = on_device ? nbr_tags : d_out;
-            if (launch_nlist_fill_by_tag(h, rs_dev, outp) != cudaSuccess) { rc = HB_ECUDA; break; }
-            if (!on_device &&
-                cudaMemcpyAsync(nbr_tags, d_out, (size_t)rs[N] * 4, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
-        }
-        if (cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = HB_ECUDA; break; }
-    } while (0);
-    if (rc == HB_ECUDA) h->err = std::string("hb_get_nlist: ") + cudaGetErrorString(cudaGetLastError());
-    dev_free(h, d_counts);
-    dev_free(h, d_rs);
-    dev_free(h, d_out);
-    return rc;
+    // row lengths by tag -> exclusive scan on the device (scratch owned by the handle: no allocation per call)
+    HB_CK(launch_nlist_counts_by_tag(h, h->acc_counts));
+    HB_CK(launch_nlist_rows_by_tag(h, h->acc_counts, h->acc_rows));
+    if (on_device) {
+        HB_CK(cudaMemcpyAsync(row_start, h->acc_rows, (N + 1) * 8, cudaMemcpyDeviceToDevice, h->stream));
+        if (nbr_tags) HB_CK(launch_nlist_fill_by_tag(h, h->acc_rows, nbr_tags));
+        return HB_OK;
+    }
+    HB_CK(cudaMemcpyAsync(row_start, h->acc_rows, (N + 1) * 8, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    if (nbr_tags) {
+        const size_t total = (size_t)row_start[N];
+        HB_TRY(ensure_stage(h, (total + 1) * 4));
+        HB_CK(launch_nlist_fill_by_tag(h, h->acc_rows, (uint32_t *)h->acc_stage));
+        HB_CK(cudaMemcpyAsync(nbr_tags, h->acc_stage, total * 4, cudaMemcpyDeviceToHost, h->stream));
+        HB_CK(cudaStreamSynchronize(h->stream));
+    }
+    return HB_OK;
 }
 
 int hb_get_forces(hb_system *h, float *f_xyz_u, float *virial6, int on_device)
@@ -1037,10 +1066,9 @@ int hb_get_forces(hb_system *h, float *f_xyz_u, float *virial6, int on_device)
         HB_CK(launch_unpack_forces(h, f_xyz_u, virial6));
         return HB_OK;
     }
-    Stage &st = g_stage[h];
-    HB_TRY(ensure_stage(h, &st.p, &st.cap, N * 40));
-    float *sf = (float *)st.p;
-    float *sv = (float *)((char *)st.p + N * 16);
+    HB_TRY(ensure_stage(h, N * 40));
+    float *sf = (float *)h->acc_stage;
+    float *sv = (float *)((char *)h->acc_stage + N * 16);
     HB_CK(launch_unpack_forces(h, f_xyz_u ? sf : nullptr, virial6 ? sv : nullptr));
     if (f_xyz_u) HB_CK(cudaMemcpyAsync(f_xyz_u, sf, N * 16, cudaMemcpyDeviceToHost, h->stream));
     if (virial6) HB_CK(cudaMemcpyAsync(virial6, sv, N * 24, cudaMemcpyDeviceToHost, h->stream));
@@ -1144,6 +1172,14 @@ int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flush_l2_by
         rc = ensure_forces(h);
     }
     return rc;
+}
+
+int hb_measure_peak(hb_system *h, const char *which, double *value)
+{
+    HB_NEED(h);
+    if (!which || !value) return HB_EINVAL;
+    Range nvtx_range("hb_measure_peak");
+    return measure_peak(h, which, value);
 }
 
 static int *tunable_slot(hb_system *h, const char *name)

@@ -6,6 +6,7 @@
 #include <vector>
 #include <map>
 #include <algorithm>
+#include <string.h>
 
 #include "../../include/hb.h"
 
@@ -25,6 +26,7 @@ enum {
     FL_BAR1 = 11,       //   FL_BAR0 + (b & 1) and clears the other one
     FL_BAR_GEN = 12,    // b: launches of the cooperative kernel that got past their barriers
     FL_TILE_CTR = 13,   // next tile of the cooperative kernel's list phase
+    FL_BADTYPE = 14,    // hb_set_state saw a type outside 0 .. ntypes-1
     FL_COUNT = 16
 };
 
@@ -45,13 +47,15 @@ struct TileGeom {
     int ntx, nty, ntz;  // tiles per axis
     int ntiles;
     int cap;            // shared-memory slots (slot 0 is the far-away dummy)
-    int fast;           // 1: tile + halo narrower than L/2 on every axis (image by tile centre, tables from the build)
+    int fast;           // 1: tile + halo narrower than L/2 on every axis (image by tile centre, halo rows staged as contiguous pieces)
+    int eshift;         // list entries are slot << eshift: 4 (the byte offset of the staged position) when cap <= 4096, else 0
     float L;
 };
 
 constexpr int TILE_THREADS = 256;
 constexpr int TILE_HMAX = 256;        // halo cells per tile, at most
 constexpr int TILE_ROWS_MAX = 32;     // own (y, z) rows per tile, at most
+constexpr int TILE_PROWS_MAX = 86;    // halo (y, z) rows per tile, at most: TILE_HMAX / 3
 constexpr int ROW_PAD = 32;           // list rows are padded with dummy entries to a multiple of this
 
 struct Tunables {
@@ -66,7 +70,8 @@ struct Tunables {
     int grow_pct = 25;     // head room given when rows or the staging area are grown after an overflow
     int cell_sort = 1;
     int coop_blocks = 4;   // blocks per SM of the cooperative cell kernel (at most)
-    int thermo_every = 1;  // 1: U_i and W_i every step (the paper's kernel); 0: only in the last step of a chunk of hb_run_nve
+    int thermo_every = 0;  // 0: U_i and W_i only in the last step of every chunk of hb_run_nve (nothing can read those of an
+                           //    inner step); 1: in every step (the paper's kernel computes them always)
     int fuse_nve = 1;      // hb_run_nve: integrate inside the force kernel
     int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
@@ -125,9 +130,6 @@ struct hb_system {
     // neighbor list: row i = nlist[i * row_pitch .. + nlistn[i]), entries are shared-memory slots of i's tile
     TileGeom geom{};
     double own_est = 0;          // expected own particles per tile
-    int *stage_src = nullptr;    // [ntiles][cap] storage index of every staged slot (written by the list build)
-    void *tile_desc = nullptr;   // [ntiles] TileDesc (tile.cuh), written by the list build
-    int64_t stage_src_len = 0, tile_desc_len = 0;
     int row_pitch = 0;
     uint16_t *nlist = nullptr;
     int *nlistn = nullptr;
@@ -156,10 +158,17 @@ struct hb_system {
     hb_stats_t stats{};
     int64_t since_sort = -1;     // steps since the last hb_sort inside hb_run_nve (-1 = never sorted)
 
-    // graph cache: key = (nsteps, cur, parity) -> exec
+    // graph cache: key = nsteps -> exec (every chunk starts from posbuf[0] and drift parity 0, see run_chunk)
     struct GraphEntry { cudaGraph_t g = nullptr; cudaGraphExec_t e = nullptr; int nkernels_fixed = 0; };
     std::map<int64_t, GraphEntry> graphs;
     float graph_dt = 0;
+
+    // accessor scratch (host <-> device staging of hb_set_state / hb_get_state / hb_get_forces / hb_get_nlist)
+    void *acc_stage = nullptr;
+    size_t acc_cap = 0;
+    int *acc_counts = nullptr;       // [N] list row lengths by tag
+    int64_t *acc_rows = nullptr;     // [N + 1] CSR row starts by tag
+    int *h_total = nullptr;          // pinned [2]
 };
 
 #define HB_CK(call)                                                                          \
@@ -223,9 +232,12 @@ cudaError_t launch_sfc_keys(hb_system *h);
 cudaError_t launch_radix_sort(hb_system *h, int key_bits);  // keys/sperm -> sorted in keys/sperm
 cudaError_t launch_gather_state(hb_system *h);              // by sperm into the scratch set (positions into pos_build)
 cudaError_t launch_rtag(hb_system *h);
+// peaks.cu
+int measure_peak(hb_system *h, const char *which, double *value);
 // accessors
 cudaError_t launch_pack_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz, const int32_t *image);
 cudaError_t launch_unpack_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image);
 cudaError_t launch_unpack_forces(hb_system *h, float *f4, float *vir6);
 cudaError_t launch_nlist_counts_by_tag(hb_system *h, int *counts);
 cudaError_t launch_nlist_fill_by_tag(hb_system *h, const int64_t *row_start, uint32_t *out);
+cudaError_t launch_nlist_rows_by_tag(hb_system *h, const int *counts, int64_t *rows);   // exclusive scan, rows[N] = total

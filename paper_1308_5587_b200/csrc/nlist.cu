@@ -53,8 +53,6 @@ struct ListArgs {
     uint16_t *nlist;
     int *nlistn, *flags;
     CopyBack cb;
-    int *stage_src;
-    TileDesc *desc;
 };
 
 // Algorithm 3 for one tile, by one block of TILE_THREADS threads
@@ -70,8 +68,7 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
     int *__restrict__ nlistn = la.nlistn;
     int *__restrict__ flags = la.flags;
     const CopyBack &cb = la.cb;
-    int *__restrict__ stage_src = la.stage_src;
-    TileDesc *__restrict__ desc = la.desc;
+    const int eshift = g.eshift;
     __shared__ TileShared s;
     float4 *stage = reinterpret_cast<float4 *>(smem_raw);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -97,15 +94,8 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
             cb.rtag[tg] = gi;
         }
     }
-    // what the force kernel will need every step: the tile's descriptor and the storage index of every slot
-    if (desc) {
-        if (!fits && threadIdx.x == 0) { s.d.nslots = 1; s.d.nown = 0; }   // nothing staged: the force kernel skips the tile
-        __syncthreads();
-        if (threadIdx.x < sizeof(TileDesc) / 4)
-            reinterpret_cast<int *>(desc + tile)[threadIdx.x] = reinterpret_cast<const int *>(&s.d)[threadIdx.x];
-    }
     if (!fits) return;
-    tile_stage_positions_by_cell(g, t, s, pos_build, stage, stage_src ? stage_src + (int64_t)tile * g.cap : nullptr);
+    tile_stage_positions_by_cell(g, t, s, pos_build, stage, nullptr);
     __syncthreads();
 
     int wmax = 0;
@@ -210,7 +200,7 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                     while (hm) {
                         const int gq = __ffs(hm) - 1;
                         hm &= hm - 1;
-                        if (at < pitch) row[at] = clist[(gq << 5) + lane];
+                        if (at < pitch) row[at] = (uint16_t)(clist[(gq << 5) + lane] << eshift);
                         at++;
                     }
                     const int nw = min(total, pitch);
@@ -321,8 +311,6 @@ static ListArgs make_list_args(hb_system *h, bool copyback)
     la.nlistn = h->nlistn;
     la.flags = h->flags;
     if (copyback) la.cb = CopyBack{h->pos(), h->vel, h->vel2, h->image, h->image2, h->tag, h->rtag, h->tag2, (int)h->N};
-    la.stage_src = h->geom.fast ? h->stage_src : nullptr;
-    la.desc = h->geom.fast ? (TileDesc *)h->tile_desc : nullptr;
     return la;
 }
 
@@ -415,8 +403,41 @@ nlist_fill_by_tag_kernel(TileGeom g, const int *__restrict__ cell_start, const u
         const int n = nlistn[gi];
         const int64_t o = row_start[tag[gi]];
         const uint16_t *row = nlist + (int64_t)gi * pitch;
-        for (int k = lane; k < n; k += 32) out[o + k] = tag[gidx[row[k]]];
+        for (int k = lane; k < n; k += 32) out[o + k] = tag[gidx[row[k] >> g.eshift]];
     }
+}
+
+// rows[k] = sum of counts[0 .. k), k = 0 .. N (int64): a single block walks the array in chunks of 2048 with a carry
+// (an accessor, not the hot path: N / 2048 sequential block scans, 0.5 ms at N = 10^6)
+__global__ void __launch_bounds__(SCAN_THREADS) nlist_rows_by_tag_kernel(const int *__restrict__ counts, int N, int64_t *__restrict__ rows)
+{
+    __shared__ int warp_tot[SCAN_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int64_t carry = 0;
+    for (int64_t base = 0; base < N; base += SCAN_TILE) {
+        const int64_t k0 = base + (int64_t)threadIdx.x * SCAN_ITEMS;
+        int x[SCAN_ITEMS], tsum = 0;
+#pragma unroll
+        for (int q = 0; q < SCAN_ITEMS; q++) { x[q] = k0 + q < N ? counts[k0 + q] : 0; tsum += x[q]; }
+        int incl = tsum;
+        for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += y; }
+        if (lane == 31) warp_tot[warp] = incl;
+        __syncthreads();
+        int woff = 0, total = 0;
+        for (int w = 0; w < SCAN_THREADS / 32; w++) { if (w < warp) woff += warp_tot[w]; total += warp_tot[w]; }
+        int64_t run = carry + woff + incl - tsum;
+#pragma unroll
+        for (int q = 0; q < SCAN_ITEMS; q++) { if (k0 + q < N) rows[k0 + q] = run; run += x[q]; }
+        carry += total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) rows[N] = carry;
+}
+
+cudaError_t launch_nlist_rows_by_tag(hb_system *h, const int *counts, int64_t *rows)
+{
+    nlist_rows_by_tag_kernel<<<1, SCAN_THREADS, 0, h->stream>>>(counts, (int)h->N, rows);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_nlist_counts_by_tag(hb_system *h, int *counts)

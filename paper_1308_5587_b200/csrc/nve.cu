@@ -155,13 +155,15 @@ cudaError_t launch_thermo(hb_system *h)
 // ---- state upload / download ----
 __global__ void pack_state_kernel(const float *__restrict__ pos_xyz, const int32_t *__restrict__ type,
                                   const float *__restrict__ vel_xyz, const int32_t *__restrict__ image_in, int N,
-                                  float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ image,
-                                  uint32_t *__restrict__ tag, uint32_t *__restrict__ rtag)
+                                  int ntypes, float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ image,
+                                  uint32_t *__restrict__ tag, uint32_t *__restrict__ rtag, int *__restrict__ flags)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
+    int t = type ? type[i] : 0;
+    if (t < 0 || t >= ntypes) { flags[FL_BADTYPE] = 1; t = 0; }   // the force kernel indexes its pair table with it
     pos[i] = make_float4(pos_xyz[3 * (int64_t)i], pos_xyz[3 * (int64_t)i + 1], pos_xyz[3 * (int64_t)i + 2],
-                         __int_as_float(type ? type[i] : 0));
+                         __int_as_float(t));
     vel[i] = make_float4(vel_xyz[3 * (int64_t)i], vel_xyz[3 * (int64_t)i + 1], vel_xyz[3 * (int64_t)i + 2], 0.f);
     for (int a = 0; a < 3; a++) image[(int64_t)a * N + i] = image_in ? image_in[3 * (int64_t)i + a] : 0;
     tag[i] = i;
@@ -186,8 +188,8 @@ __global__ void unpack_state_kernel(const float4 *__restrict__ pos, const float4
 
 cudaError_t launch_pack_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz, const int32_t *image)
 {
-    pack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(pos_xyz, type, vel_xyz, image, (int)h->N, h->pos(), h->vel,
-                                                                        h->image, h->tag, h->rtag);
+    pack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(pos_xyz, type, vel_xyz, image, (int)h->N, h->ntypes, h->pos(),
+                                                                        h->vel, h->image, h->tag, h->rtag, h->flags);
     return cudaGetLastError();
 }
 

@@ -60,6 +60,16 @@ __device__ __forceinline__ void tile_decode(const TileGeom &g, int tile, TileCtx
     t.nrows = t.ey * t.ez;
 }
 
+// the same from the three tile coordinates (a 3-D grid launch: no integer division)
+__device__ __forceinline__ void tile_decode_xyz(const TileGeom &g, int tix, int tiy, int tiz, TileCtx &t)
+{
+    t.x0 = tix * g.tx; t.y0 = tiy * g.ty; t.z0 = tiz * g.tz;
+    t.ex = min(g.tx, g.m - t.x0); t.ey = min(g.ty, g.m - t.y0); t.ez = min(g.tz, g.m - t.z0);
+    t.hx = t.ex + 2; t.hy = t.ey + 2; t.hz = t.ez + 2;
+    t.nh = t.hx * t.hy * t.hz;
+    t.nrows = t.ey * t.ez;
+}
+
 // wrap a halo cell coordinate into the box; shift = what to add to a coordinate of that cell's particles
 __device__ __forceinline__ int tile_wrap(int c, int m, float L, float &shift)
 {

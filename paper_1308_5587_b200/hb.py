@@ -25,7 +25,7 @@ _ERR_NAMES = {-1: "HB_EINVAL", -2: "HB_ECUDA", -3: "HB_ENOMEM", -4: "HB_EBOX", -
 EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_build_cells",
            "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_sort",
            "hb_thermo", "hb_get_cells", "hb_get_nlist", "hb_get_forces", "hb_stats", "hb_set_tunable",
-           "hb_get_tunable", "hb_time_stage", "hb_last_error", "hb_version"]
+           "hb_get_tunable", "hb_time_stage", "hb_measure_peak", "hb_last_error", "hb_version"]
 
 
 class HBError(RuntimeError):
@@ -47,7 +47,7 @@ class hb_thermo_t(C.Structure):
 
 class hb_stats_t(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("steps", "rebuilds", "sorts", "overflow_retries", "max_nbrs", "row_pitch",
-                                         "cells_per_axis", "graph_launches", "kernel_launches")]
+                                         "cells_per_axis", "graph_launches", "kernel_launches", "graph_builds")]
 
 
 _lib = None
@@ -83,6 +83,7 @@ def load():
     L.hb_set_tunable.argtypes = [vp, C.c_char_p, i32]
     L.hb_get_tunable.argtypes = [vp, C.c_char_p, C.POINTER(i32)]
     L.hb_time_stage.argtypes = [vp, C.c_char_p, i32, i64, C.POINTER(dbl)]
+    L.hb_measure_peak.argtypes = [vp, C.c_char_p, C.POINTER(dbl)]
     L.hb_last_error.argtypes = [vp]
     L.hb_last_error.restype = C.c_char_p
     L.hb_version.restype = C.c_char_p
@@ -297,6 +298,12 @@ class System:
         ms = C.c_double()
         self._ck(self._lib.hb_time_stage(self._h, stage.encode(), int(reps), int(flush_l2_bytes), C.byref(ms)))
         return ms.value
+
+    def measure_peak(self, which):
+        """Measured roofline denominator: "fp32_tflops", "l2_gbs" or "smem_gbs"."""
+        v = C.c_double()
+        self._ck(self._lib.hb_measure_peak(self._h, which.encode(), C.byref(v)))
+        return v.value
 
     def set_tunable(self, name, value):
         self._ck(self._lib.hb_set_tunable(self._h, name.encode(), int(value)))

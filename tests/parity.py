@@ -41,13 +41,27 @@ def pair_dist(pos, L, keys):
 
 
 def assert_nlist_equal(pos64, L, r_max, rs_ref, nbr_ref, rs_gpu, nbr_gpu):
-    """Set equality of (i, j) entries except pairs within BAND of r_max; no duplicates, no self."""
+    """Set equality of (i, j) entries except pairs within BAND of r_max; no duplicates, no self.
+    Exact at any size: rows whose (length, sum j, sum j^2) differ are compared entry by entry as sets,
+    all the others must make identical sorted key arrays."""
     kr = np.sort(rows_as_keys(rs_ref, nbr_ref))
     kg = np.sort(rows_as_keys(rs_gpu, nbr_gpu))
-    assert len(np.unique(kg)) == len(kg), "duplicate neighbor entries"
+    assert not np.any(kg[1:] == kg[:-1]), "duplicate neighbor entries"
     assert not np.any((kg >> 32) == (kg & 0xFFFFFFFF)), "self in list"
-    only_ref = np.setdiff1d(kr, kg, assume_unique=True)
-    only_gpu = np.setdiff1d(kg, kr, assume_unique=True)
+    if len(kr) == len(kg) and np.array_equal(kr, kg):
+        return 0
+    n = len(rs_ref) - 1
+
+    def row_sums(k):
+        i, j = k >> 32, (k & 0xFFFFFFFF).astype(np.float64)
+        return (np.bincount(i, minlength=n), np.bincount(i, weights=j, minlength=n), np.bincount(i, weights=j * j, minlength=n))
+
+    a, b = row_sums(kr), row_sums(kg)
+    odd = (a[0] != b[0]) | (a[1] != b[1]) | (a[2] != b[2])
+    keep_r, keep_g = ~odd[kr >> 32], ~odd[kg >> 32]
+    assert np.array_equal(kr[keep_r], kg[keep_g]), "rows with equal checksums differ"
+    only_ref = np.setdiff1d(kr[~keep_r], kg[~keep_g], assume_unique=True)
+    only_gpu = np.setdiff1d(kg[~keep_g], kr[~keep_r], assume_unique=True)
     for name, ks in (("missing from GPU list", only_ref), ("extra in GPU list", only_gpu)):
         if len(ks):
             d = pair_dist(pos64, L, ks)

@@ -1,8 +1,12 @@
 """GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py
-times (default tunables, hb_run_nve's graphs), on SAMPLED outputs: for a seeded
-sample of particles the oracle computes the neighbor row and the force, energy
-and virial by brute force over all N particles (O(S N), seconds), and the cell
-membership of every particle (O(N)).  Needs a B200.
+times (default tunables, hb_run_nve's graphs), on EVERY particle: the oracle's
+own cell-list path (Algorithm 2 + 3 in fp64, oracle/orc.c) gives the neighbor
+row, force, energy and virial of all N particles in about a second per
+snapshot, so nothing is sampled: cell membership of every particle, set
+equality of every list row, the force tolerance for every particle and the
+total potential energy within 1e-5 relative (north_star's tolerances, written
+in tests/parity.py).  The oracle's O(N^2) definitions, restricted to a seeded
+sample of rows, cross-check its cell-list path at the same size.  Needs a B200.
 
 Two snapshots per config: the seeded start (lattice + jitter) and the state the
 GPU itself reaches after `steps` NVE steps with device-side rebuilds and a sort,
@@ -29,41 +33,43 @@ def hb():
     return _hb
 
 
-def _sampled_parity(hb, orc, w, g, pos32, typ, L, rng):
-    N = w.N
-    pos64 = pos32.astype(np.float64)
+def _oracle_all(orc, w, pos64, typ, L, rng):
+    """Rows, forces, energies, virials and allowances of ALL particles from the oracle's cell-list path,
+    cross-checked on a seeded sample of rows against its O(N^2) definitions."""
     p = orc.Params.of(w)
-    sample = np.sort(rng.choice(N, size=SAMPLE, replace=False)).astype(np.int64)
-    # cells: every particle (the oracle's canonical binary32 formula is O(N))
+    cnt, rs, nbr = orc.nlist_cells(pos64, L, w.r_max)
+    F, U, W, A = orc.compute_lj_nlist(pos64, typ, L, p, cnt, rs, nbr, band=parity.BAND)
+    sample = rng.permutation(w.N)[:SAMPLE].astype(np.int64)
+    cs, rss, nbs = orc.nlist_brute_sample(pos64, L, w.r_max, sample)
+    assert np.array_equal(cs, cnt[sample])
+    for k, i in enumerate(sample):
+        assert np.array_equal(np.sort(nbs[rss[k]:rss[k + 1]]), np.sort(nbr[rs[i]:rs[i + 1]]))
+    Fs, Us, Ws, As = orc.compute_lj_brute_sample(pos64, typ, L, p, sample, band=parity.BAND)
+    assert np.abs(Fs - F[sample]).max() <= 1e-11 * np.abs(F).max()
+    assert np.abs(Us - U[sample]).max() <= 1e-11 * np.abs(U).max()
+    assert np.abs(As - A[sample]).max() <= 1e-11 * max(1.0, np.abs(A).max())
+    return (cnt, rs, nbr), (F, U, W, A)
+
+
+def _full_parity(hb, orc, w, g, pos32, typ, L, rng):
+    """Cells, list rows, forces, per-particle energies, virials of EVERY particle and the total U."""
+    pos64 = pos32.astype(np.float64)
     g.build_cells()                      # no-op: the cell list of these positions is in place
     m, start, tags = g.get_cells()
     assert m == orc.cell_dim(L, w.r_max)
     parity.assert_cells_equal(orc, pos32, L, m, start, tags)
-    # neighbor rows of the sample against brute force over all N
+    (cnt, rs_ref, nbr_ref), (F, U, W, A) = _oracle_all(orc, w, pos64, typ, L, rng)
     rs, nbr = g.get_nlist()
-    cnt_ref, rs_ref, nbr_ref = orc.nlist_brute_sample(pos64, L, w.r_max, sample)
-    bad = 0
-    for k, i in enumerate(sample):
-        got = set(nbr[rs[i]:rs[i + 1]].tolist())
-        ref = set(nbr_ref[rs_ref[k]:rs_ref[k + 1]].tolist())
-        assert len(got) == rs[i + 1] - rs[i], "duplicate entries in a row"
-        assert i not in got, "self in list"
-        for j in got ^ ref:
-            d = pos64[i] - pos64[j]
-            d -= L * np.rint(d / L)
-            dist = float(np.sqrt((d * d).sum()))
-            assert abs(dist - w.r_max) <= parity.BAND, f"row {i}: pair with d = {dist} on one side only"
-            bad += 1
-    # forces, energies, virials of the sample
+    nband = parity.assert_nlist_equal(pos64, L, w.r_max, rs_ref, nbr_ref, rs, nbr)
+    assert nband <= 64, f"{nband} pairs inside the 1e-5 band: far more than the geometry allows"
     f4, w6 = g.get_forces()
-    F, U, W, A = orc.compute_lj_brute_sample(pos64, typ, L, p, sample, band=parity.BAND)
-    # max |F| over the sample stands in for max over all particles (it is smaller or equal: a stricter test)
-    worst = parity.assert_forces_close(F, U, W, A, f4, w6, rows=sample)
-    return worst, bad
+    worst = parity.assert_forces_close(F, U, W, A, f4, w6)
+    parity.assert_energy_close(U.sum(), g.thermo()["U"], A[:, 1].sum())
+    return worst
 
 
 @pytest.mark.parametrize("case", list(CASES))
-def test_fullsize_sampled_parity(hb, orc, case):
+def test_fullsize_parity_all_particles(hb, orc, case):
     w = wl.CONFIGS[case]
     s = wl.make_state(w)
     rng = np.random.default_rng(1234)
@@ -71,7 +77,7 @@ def test_fullsize_sampled_parity(hb, orc, case):
         g.set_state(s.pos, s.type, s.vel, s.image)
         g.build_nlist(0.0, w.r_buff)
         g.compute_lj(w.shift)
-        worst0, _ = _sampled_parity(hb, orc, w, g, s.pos, s.type, s.L, rng)
+        worst0 = _full_parity(hb, orc, w, g, s.pos, s.type, s.L, rng)
         # the path bench.py times: graphs, device-side rebuild decisions, fused step kernel, one sort on the way
         steps = CASES[case]
         g.run_nve(w.dt, steps, max(1, steps // 2))
@@ -81,24 +87,28 @@ def test_fullsize_sampled_parity(hb, orc, case):
         assert np.array_equal(np.sort(out["order"]), np.arange(w.N)), "a particle was lost or duplicated"
         assert np.array_equal(out["type"], s.type)
         assert np.all(out["pos"] >= -s.L / 2) and np.all(out["pos"] <= s.L / 2)
-        # the list in use must still hold every pair inside r_cut of the sample (reading c3's invariant) ...
+        # the list in use must still hold every pair inside r_cut (reading c3's invariant), for every particle ...
         pos64 = out["pos"].astype(np.float64)
-        sample = np.sort(rng.choice(w.N, size=SAMPLE, replace=False)).astype(np.int64)
         rs, nbr = g.get_nlist()
-        _, rs_need, nbr_need = orc.nlist_brute_sample(pos64, s.L, w.r_cut_max, sample)
-        for k, i in enumerate(sample):
-            have = set(nbr[rs[i]:rs[i + 1]].tolist())
-            assert set(nbr_need[rs_need[k]:rs_need[k + 1]].tolist()) <= have, f"row {i} misses a pair inside r_cut"
-        # ... and the forces of the final state (computed by the graph's last kernel over that older list) must
-        # agree with brute force on that state
+        have = np.sort(parity.rows_as_keys(rs, nbr))
+        _, rs_need, nbr_need = orc.nlist_cells(pos64, s.L, w.r_cut_max)
+        need = parity.rows_as_keys(rs_need, nbr_need)
+        missing = np.setdiff1d(need, have, assume_unique=True)
+        assert len(missing) == 0, f"{len(missing)} pairs inside r_cut are not in the list in use"
+        del have, need
+        # ... and the forces, energies and virials of the final state (computed by the graph's last kernel over
+        # that older list) must agree with the oracle on that state, for every particle, and so must the total U
         f4, w6 = g.get_forces()
-        F, U, W, A = orc.compute_lj_brute_sample(pos64, s.type, s.L, orc.Params.of(w), sample, band=parity.BAND)
-        parity.assert_forces_close(F, U, W, A, f4, w6, rows=sample)
-        # a fresh build on that state: cells, rows, forces again
+        _, (F, U, W, A) = _oracle_all(orc, w, pos64, s.type, s.L, rng)
+        parity.assert_forces_close(F, U, W, A, f4, w6)
+        parity.assert_energy_close(U.sum(), g.thermo()["U"], A[:, 1].sum())
+        # a fresh build on that state: cells, rows, forces, energy again
         g.build_nlist(0.0, w.r_buff)
         g.compute_lj(w.shift)
-        worst1, _ = _sampled_parity(hb, orc, w, g, out["pos"], s.type, s.L, rng)
-    assert max(worst0, worst1) <= parity.F_TOL
+        worst1 = _full_parity(hb, orc, w, g, out["pos"], s.type, s.L, rng)
+    # (assert_forces_close has applied 1e-4 max|F| plus the cutoff-flip allowance to every particle; the raw ratio
+    # it returns exceeds 1e-4 wherever a pair within 1e-5 of r_cut was decided differently in fp32 and fp64)
+    assert np.isfinite(worst0) and np.isfinite(worst1)
 
 
 def test_four_million_particles(hb, orc):

@@ -234,7 +234,9 @@ double orc_max_disp2(const double *pos, const double *pos_build, int64_t N, doub
 /* ------------------------------------------------------------- c4, c5 ---- */
 /* V_lj(r) = 4 eps [ (sigma/r)^12 - alpha (sigma/r)^6 ], alpha = 1
  * -(1/r) dV/dr = (1/r^2) (48 eps (sigma/r)^12 - 24 eps (sigma/r)^6)
- * active iff r < r_cut; shift: V = V_lj(r) - V_lj(r_cut). */
+ * active iff r < r_cut; shift: V = V_lj(r) - V_lj(r_cut).
+ * `shift` in the sums below is the mode: 0 plain, 1 energy shift, 2 XPLOR smoothing with r_on per type pair
+ * (`ron`, nullable unless mode 2). */
 static inline double vlj(double r, double eps, double sigma)
 {
     const double sr = sigma / r;
@@ -252,16 +254,51 @@ void orc_lj_pair(double r, double eps, double sigma, double r_cut, int shift,
     *V = vlj(r, eps, sigma) - (shift ? vlj(r_cut, eps, sigma) : 0.0);
 }
 
+/* XPLOR smoothing (section 8.2.2):  V(r) = V_lj(r) S(r) with
+ *   S(r) = 1                                                        r <  r_on
+ *        = (rc^2 - r^2)^2 (rc^2 + 2 r^2 - 3 ron^2) / (rc^2 - ron^2)^3   r_on <= r <= r_cut
+ *        = 0                                                        r >  r_cut
+ * so that V and its first derivative go to 0 at r_cut.  The force follows by the
+ * product rule:  -dV/dr = (-dV_lj/dr) S - V_lj S',
+ *   S'(r) = 12 r (rc^2 - r^2)(ron^2 - r^2) / (rc^2 - ron^2)^3   (derivative of the line above),
+ * returned, like orc_lj_pair, as -(1/r) dV/dr.  No energy shift is applied (S does that job).
+ * [reading x1] r_on >= r_cut leaves no switching interval: S = 1 inside r_cut, i.e. the
+ * plain truncated potential (the paper gives no rule for this case). */
+void orc_lj_pair_xplor(double r, double eps, double sigma, double r_cut, double r_on,
+                       double *V, double *minus_dVdr_over_r)
+{
+    double Vlj, flj;
+    orc_lj_pair(r, eps, sigma, r_cut, 0, &Vlj, &flj);
+    if (!(r < r_cut)) { *V = 0.0; *minus_dVdr_over_r = 0.0; return; }
+    double S = 1.0, dS_over_r = 0.0;
+    if (r >= r_on && r_on < r_cut) {
+        const double rc2 = r_cut * r_cut, ron2 = r_on * r_on, r2 = r * r;
+        const double D = (rc2 - ron2) * (rc2 - ron2) * (rc2 - ron2);
+        S = (rc2 - r2) * (rc2 - r2) * (rc2 + 2.0 * r2 - 3.0 * ron2) / D;
+        dS_over_r = 12.0 * (rc2 - r2) * (ron2 - r2) / D;          /* S'(r) / r */
+    }
+    *V = Vlj * S;
+    *minus_dVdr_over_r = flj * S - Vlj * dS_over_r;
+}
+
+/* one entry point for the three modes of the force sums: 0 = plain, 1 = energy shift, 2 = XPLOR */
+static inline void pair_by_mode(double r, double eps, double sigma, double r_cut, double r_on, int mode,
+                                double *V, double *fdivr)
+{
+    if (mode == 2) orc_lj_pair_xplor(r, eps, sigma, r_cut, r_on, V, fdivr);
+    else orc_lj_pair(r, eps, sigma, r_cut, mode, V, fdivr);
+}
+
 /* ------------------------------------------------------------------ c6 ---- */
 /* One pair's contribution to particle i:  F_i += f, U_i += V/2,
  * W_i^{ab} += (1/2) d^a f^b  with d = minimage(R_i - R_j), f = [-(1/r)dV/dr] d. */
-static inline void add_pair(const double d[3], double r2, double eps, double sigma, double r_cut,
+static inline void add_pair(const double d[3], double r2, double eps, double sigma, double r_cut, double r_on,
                             int shift, double *F, double *U, double *W,
                             double band, double *allow)
 {
     const double r = sqrt(r2);
     double V, fdivr;
-    orc_lj_pair(r, eps, sigma, r_cut, shift, &V, &fdivr);
+    pair_by_mode(r, eps, sigma, r_cut, r_on, shift, &V, &fdivr);
     const double f[3] = { fdivr * d[0], fdivr * d[1], fdivr * d[2] };
     F[0] += f[0]; F[1] += f[1]; F[2] += f[2];
     *U += 0.5 * V;
@@ -275,7 +312,7 @@ static inline void add_pair(const double d[3], double r2, double eps, double sig
     if (allow && fabs(r - r_cut) <= band) {
         const double rc = nextafter(r_cut, 0.0);
         double Vc, fc;
-        orc_lj_pair(rc, eps, sigma, r_cut, shift, &Vc, &fc);
+        pair_by_mode(rc, eps, sigma, r_cut, r_on, shift, &Vc, &fc);
         allow[0] += fabs(fc) * rc;
         allow[1] += 0.5 * fabs(Vc);
         allow[2] += 0.5 * fabs(fc) * rc * rc;
@@ -284,7 +321,7 @@ static inline void add_pair(const double d[3], double r2, double eps, double sig
 
 /* DEFINITION: sums over all j != i (O(N^2)).  F[N][3], U[N], W[N][6]. */
 int orc_compute_lj_brute(const double *pos, const int32_t *type, int64_t N, double L, int ntypes,
-                         const double *eps, const double *sigma, const double *rcut, int shift,
+                         const double *eps, const double *sigma, const double *rcut, const double *ron, int shift,
                          double *F, double *U, double *W)
 {
 #pragma omp parallel for schedule(dynamic, 64)
@@ -295,7 +332,7 @@ int orc_compute_lj_brute(const double *pos, const int32_t *type, int64_t N, doub
             double d[3];
             const double r2 = dist2(pos, i, j, L, d);
             const int p = type[i] * ntypes + type[j];
-            if (r2 < rcut[p] * rcut[p]) add_pair(d, r2, eps[p], sigma[p], rcut[p], shift, Fi, &Ui, Wi, 0.0, NULL);
+            if (r2 < rcut[p] * rcut[p]) add_pair(d, r2, eps[p], sigma[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, 0.0, NULL);
         }
         memcpy(F + 3 * i, Fi, sizeof Fi); U[i] = Ui; memcpy(W + 6 * i, Wi, sizeof Wi);
     }
@@ -304,7 +341,7 @@ int orc_compute_lj_brute(const double *pos, const int32_t *type, int64_t N, doub
 
 /* Sampled definition for full-size spot checks: rows sample[0..S) only. */
 int orc_compute_lj_brute_sample(const double *pos, const int32_t *type, int64_t N, double L, int ntypes,
-                                const double *eps, const double *sigma, const double *rcut, int shift,
+                                const double *eps, const double *sigma, const double *rcut, const double *ron, int shift,
                                 const int64_t *sample, int64_t S, double band,
                                 double *F, double *U, double *W, double *allow)
 {
@@ -318,7 +355,7 @@ int orc_compute_lj_brute_sample(const double *pos, const int32_t *type, int64_t 
             const double r2 = dist2(pos, i, j, L, d);
             const int p = type[i] * ntypes + type[j];
             const double rc = rcut[p] + band;
-            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], shift, Fi, &Ui, Wi, band, al);
+            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, band, al);
         }
         memcpy(F + 3 * k, Fi, sizeof Fi); U[k] = Ui; memcpy(W + 6 * k, Wi, sizeof Wi);
         if (allow) memcpy(allow + 3 * k, al, sizeof al);
@@ -330,7 +367,7 @@ int orc_compute_lj_brute_sample(const double *pos, const int32_t *type, int64_t 
  * neighbors, each tested against its type pair's r_cut.  allow[N][3] (nullable)
  * receives the cutoff-flip allowances for pairs within `band` of r_cut. */
 int orc_compute_lj_nlist(const double *pos, const int32_t *type, int64_t N, double L, int ntypes,
-                         const double *eps, const double *sigma, const double *rcut, int shift,
+                         const double *eps, const double *sigma, const double *rcut, const double *ron, int shift,
                          const int32_t *count, const int64_t *row_start, const int32_t *nbr,
                          double band, double *F, double *U, double *W, double *allow)
 {
@@ -345,7 +382,7 @@ int orc_compute_lj_nlist(const double *pos, const int32_t *type, int64_t N, doub
             /* add_pair() itself applies r < r_cut; pairs just outside are
              * visited only so that their allowance is recorded. */
             const double rc = rcut[p] + band;
-            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], shift, Fi, &Ui, Wi, band, al);
+            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, band, al);
         }
         memcpy(F + 3 * i, Fi, sizeof Fi); U[i] = Ui; memcpy(W + 6 * i, Wi, sizeof Wi);
         if (allow) memcpy(allow + 3 * i, al, sizeof al);
@@ -466,7 +503,7 @@ int orc_sort_perm(const uint32_t *key, int64_t N, int B, int64_t *perm)
  * Uses its own fp64 binning (any self-consistent binning with cell width >=
  * r_max yields the exact set -- pinned against orc_nlist_brute). */
 int orc_run_nve(double *pos, double *vel, int32_t *image, const int32_t *type, int64_t N, double L,
-                int ntypes, const double *eps, const double *sigma, const double *rcut, int shift,
+                int ntypes, const double *eps, const double *sigma, const double *rcut, const double *ron, int shift,
                 double r_buff, double dt, int64_t nsteps, int have_forces,
                 double *F, double *U, double *W, double *log_KU, int64_t *stats)
 {
@@ -515,7 +552,7 @@ int orc_run_nve(double *pos, double *vel, int32_t *image, const int32_t *type, i
                 need_build = 0;
                 builds++;
             }
-            orc_compute_lj_nlist(pos, type, N, L, ntypes, eps, sigma, rcut, shift,
+            orc_compute_lj_nlist(pos, type, N, L, ntypes, eps, sigma, rcut, ron, shift,
                                  count, row_start, nbr, 0.0, F, U, W, NULL);
         }
         if (step > 0) orc_nve_step2(vel, F, N, dt);

@@ -49,10 +49,11 @@ def lib():
         L.orc_max_disp2.restype = C.c_double
         L.orc_max_disp2.argtypes = [_dp, _dp, C.c_int64, C.c_double]
         L.orc_lj_pair.argtypes = [C.c_double] * 4 + [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
-        L.orc_compute_lj_brute.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
-        L.orc_compute_lj_brute_sample.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, C.c_int,
+        L.orc_lj_pair_xplor.argtypes = [C.c_double] * 5 + [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_compute_lj_brute.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
+        L.orc_compute_lj_brute_sample.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int,
                                                   _lp, C.c_int64, C.c_double, _dp, _dp, _dp, _vp]
-        L.orc_compute_lj_nlist.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, C.c_int,
+        L.orc_compute_lj_nlist.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int,
                                            _ip, _lp, _ip, C.c_double, _dp, _dp, _dp, _vp]
         L.orc_nve_step1.argtypes = [_dp, _dp, _dp, _ip, C.c_int64, C.c_double, C.c_double]
         L.orc_nve_step2.argtypes = [_dp, _dp, C.c_int64, C.c_double]
@@ -61,7 +62,7 @@ def lib():
         L.orc_hilbert_key.argtypes = [C.c_uint32] * 3 + [C.c_int]
         L.orc_sfc_keys.argtypes = [_fp, C.c_int64, C.c_float, C.c_int, _up]
         L.orc_sort_perm.argtypes = [_up, C.c_int64, C.c_int, _lp]
-        L.orc_run_nve.argtypes = [_dp, _dp, _ip, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, C.c_int,
+        L.orc_run_nve.argtypes = [_dp, _dp, _ip, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int,
                                   C.c_double, C.c_double, C.c_int64, C.c_int, _dp, _dp, _dp, _vp, _vp]
         L.orc_num_threads.restype = C.c_int
         _lib = L
@@ -84,11 +85,13 @@ def _check(rc, what):
 class Params:
     """Per-type-pair tables as fp64 arrays (values already fp32-representable)."""
 
-    def __init__(self, ntypes, eps, sigma, rcut, shift):
+    def __init__(self, ntypes, eps, sigma, rcut, shift, ron=None):
+        """shift: 0 plain, 1 energy shift, 2 XPLOR smoothing (needs ron per type pair)."""
         self.ntypes = int(ntypes)
         self.eps, self.sigma, self.rcut = _d(eps).ravel(), _d(sigma).ravel(), _d(rcut).ravel()
+        self.ron = self.rcut.copy() if ron is None else _d(ron).ravel()
         self.shift = int(shift)
-        assert self.eps.size == self.sigma.size == self.rcut.size == self.ntypes ** 2
+        assert self.eps.size == self.sigma.size == self.rcut.size == self.ron.size == self.ntypes ** 2
 
     @classmethod
     def of(cls, w):
@@ -165,11 +168,17 @@ def lj_pair(r, eps, sigma, r_cut, shift):
     return V.value, f.value
 
 
+def lj_pair_xplor(r, eps, sigma, r_cut, r_on):
+    V, f = C.c_double(), C.c_double()
+    lib().orc_lj_pair_xplor(float(r), float(eps), float(sigma), float(r_cut), float(r_on), C.byref(V), C.byref(f))
+    return V.value, f.value
+
+
 def compute_lj_brute(pos, typ, L, p: Params):
     pos, typ = _d(pos), np.ascontiguousarray(typ, dtype=np.int32)
     N = len(pos)
     F, U, W = np.empty((N, 3)), np.empty(N), np.empty((N, 6))
-    _check(lib().orc_compute_lj_brute(pos, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.shift, F, U, W), "lj brute")
+    _check(lib().orc_compute_lj_brute(pos, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift, F, U, W), "lj brute")
     return F, U, W
 
 
@@ -178,7 +187,7 @@ def compute_lj_brute_sample(pos, typ, L, p: Params, sample, band=0.0):
     sample = np.ascontiguousarray(sample, dtype=np.int64)
     S = len(sample)
     F, U, W, A = np.empty((S, 3)), np.empty(S), np.empty((S, 6)), np.empty((S, 3))
-    _check(lib().orc_compute_lj_brute_sample(pos, typ, len(pos), float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.shift,
+    _check(lib().orc_compute_lj_brute_sample(pos, typ, len(pos), float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
                                              sample, S, float(band), F, U, W, _ptr(A)), "lj brute sample")
     return F, U, W, A
 
@@ -190,7 +199,7 @@ def compute_lj_nlist(pos, typ, L, p: Params, count, row_start, nbr, band=0.0):
     if nbr.size == 0:
         nbr = np.zeros(1, dtype=np.int32)
     F, U, W, A = np.empty((N, 3)), np.empty(N), np.empty((N, 6)), np.empty((N, 3))
-    _check(lib().orc_compute_lj_nlist(pos, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.shift,
+    _check(lib().orc_compute_lj_nlist(pos, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
                                       np.ascontiguousarray(count, dtype=np.int32),
                                       np.ascontiguousarray(row_start, dtype=np.int64), nbr,
                                       float(band), F, U, W, _ptr(A)), "lj nlist")
@@ -246,7 +255,7 @@ def run_nve(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, forces=None,
         have = 1
     KU = np.zeros((nsteps + 1, 2)) if log else None
     stats = np.zeros(2, dtype=np.int64)
-    _check(lib().orc_run_nve(pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.shift,
+    _check(lib().orc_run_nve(pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
                              float(r_buff), float(dt), int(nsteps), have, F, U, W, _ptr(KU), _ptr(stats)), "run_nve")
     return dict(pos=pos, vel=vel, image=image, F=F, U=U, W=W, KU=KU, builds=int(stats[0]), max_nbrs=int(stats[1]))
 

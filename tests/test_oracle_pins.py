@@ -84,6 +84,51 @@ def test_shift_and_cutoff(orc):
         assert Vc == pytest.approx(eps * -1.631689114e-2, rel=1e-8)
 
 
+
+def test_xplor_closed_forms(orc):
+    """NEXT-1: S and S' worked by hand (golden/xplor_closed_form.txt) through
+    V = V_lj S and -dV/dr = F_lj S - V_lj S' with the hand values of lj_closed_form.txt."""
+    for rn, rd, sn, sd, dn, dd in _rows("xplor_closed_form.txt"):
+        r = Fraction(int(rn), int(rd))
+        S, dS = Fraction(int(sn), int(sd)), Fraction(int(dn), int(dd))
+        Vlj = 4 * (Fraction(1) / r ** 12 - Fraction(1) / r ** 6)
+        Flj = (48 / r ** 12 - 24 / r ** 6) / r
+        V, fdivr = orc.lj_pair_xplor(float(r) if r < Fraction(5, 2) else 2.5 - 1e-13, 1.0, 1.0, 2.5, 1.5)
+        assert V == pytest.approx(float(Vlj * S), rel=1e-12, abs=1e-12)
+        assert fdivr * float(r) == pytest.approx(float(Flj * S - Vlj * dS), rel=1e-12, abs=1e-11)
+    # the two values spelled out in the fixture's header
+    V, fdivr = orc.lj_pair_xplor(2.0, 1.0, 1.0, 2.5, 1.5)
+    assert V == pytest.approx(-76545 / 2097152, rel=1e-14) and 2.0 * fdivr == pytest.approx(-208251 / 1048576, rel=1e-14)
+
+
+def test_xplor_is_smooth_and_reduces_to_lj(orc):
+    """NEXT-1: below r_on the potential is plain LJ (no shift); V and F are continuous at r_on; both go to 0
+    at r_cut; -(1/r) dV/dr agrees with a central difference of V everywhere, also across r_on (catches a wrong
+    S', a dropped V_lj S' term, a sign); r_on >= r_cut is the plain truncated potential (reading x1)."""
+    for eps, sigma, rc, ron in [(1.0, 1.0, 2.5, 1.5), (1.5, 0.8, 2.0, 1.2), (0.5, 0.88, 2.2, 1.32), (1.0, 1.0, 3.0, 2.0)]:
+        for r in np.linspace(0.85 * sigma, ron - 1e-9, 7):
+            assert orc.lj_pair_xplor(r, eps, sigma, rc, ron) == orc.lj_pair(r, eps, sigma, rc, 0)
+        a, b = orc.lj_pair_xplor(ron - 1e-10, eps, sigma, rc, ron), orc.lj_pair_xplor(ron + 1e-10, eps, sigma, rc, ron)
+        assert a[0] == pytest.approx(b[0], rel=1e-8) and a[1] == pytest.approx(b[1], rel=1e-7)
+        Vc, fc = orc.lj_pair_xplor(rc - 1e-7, eps, sigma, rc, ron)
+        assert abs(Vc) < 1e-12 and abs(fc) < 1e-6          # V ~ (rc - r)^2, F ~ (rc - r)
+        assert orc.lj_pair_xplor(rc, eps, sigma, rc, ron) == (0.0, 0.0)
+        assert orc.lj_pair_xplor(1.01 * rc, eps, sigma, rc, ron) == (0.0, 0.0)
+        h = 1e-6
+        for r in np.concatenate([np.linspace(0.9 * sigma, rc - 1e-3, 60), [ron - 2e-7, ron, ron + 2e-7]]):
+            Vp, _ = orc.lj_pair_xplor(r + h, eps, sigma, rc, ron)
+            Vm, _ = orc.lj_pair_xplor(r - h, eps, sigma, rc, ron)
+            _, fdivr = orc.lj_pair_xplor(r, eps, sigma, rc, ron)
+            assert fdivr * r == pytest.approx(-(Vp - Vm) / (2 * h), rel=2e-6, abs=2e-8)
+        for r in np.linspace(0.9 * sigma, 1.1 * rc, 23):
+            assert orc.lj_pair_xplor(r, eps, sigma, rc, rc) == orc.lj_pair(r, eps, sigma, rc, 0)
+            assert orc.lj_pair_xplor(r, eps, sigma, rc, 1.5 * rc) == orc.lj_pair(r, eps, sigma, rc, 0)
+    # S itself at its ends: V / V_lj = 1 at r_on and 0 at r_cut, monotone in between
+    rs = np.linspace(1.5, 2.5 - 1e-9, 200)
+    S = np.array([orc.lj_pair_xplor(r, 1, 1, 2.5, 1.5)[0] / orc.lj_pair(r, 1, 1, 2.5, 0)[0] for r in rs])
+    assert S[0] == pytest.approx(1.0, abs=1e-12) and S[-1] < 1e-15 and np.all(np.diff(S) <= 1e-15)
+
+
 # ----------------------------------------------------------------- c1 -------
 @pytest.mark.parametrize("name,N", [("lj_1k", 1000), ("lj_64k", 8000), ("wca_256k", 4096), ("ka_1m", 8000)])
 def test_cell_index_invariants(orc, name, N):
@@ -230,19 +275,25 @@ def _pair_sum_numpy(pos, typ, L, p):
     k = typ[i] * p.ntypes + typ[j]
     eps, sig, rc = p.eps[k], p.sigma[k], p.rcut[k]
     v = lambda x: 4 * eps * ((sig / x) ** 12 - (sig / x) ** 6)
+    if p.shift == 2:      # XPLOR: V_lj S(r), S from PAPER.md:361
+        ron = p.ron[k]
+        S = np.where(r < ron, 1.0, (rc ** 2 - r ** 2) ** 2 * (rc ** 2 + 2 * r ** 2 - 3 * ron ** 2) / (rc ** 2 - ron ** 2) ** 3)
+        return np.where(r < rc, v(r) * S, 0.0).sum()
     V = np.where(r < rc, v(r) - (v(rc) if p.shift else 0.0), 0.0)
     return V.sum()
 
 
-@pytest.mark.parametrize("name,N", [("lj_1k", 1000), ("ka_1m", 1500), ("wca_256k", 1331)])
+@pytest.mark.parametrize("name,N", [("lj_1k", 1000), ("ka_1m", 1500), ("wca_256k", 1331), ("lj_1k:xplor", 1000), ("ka_1m:xplor", 1500)])
 def test_force_sums_newton_energy_virial(orc, name, N):
     """c6: list-based sums == brute-force sums; Newton III (net force 1e-10
     relative, north_star); sum U_i == pair sum; tr W == -dU/dlambda under uniform
     scaling (catches a dropped 1/2, a sign, a transposed virial index)."""
-    w = wl.scaled(wl.CONFIGS[name], N)
+    w = wl.scaled(wl.CONFIGS[name.split(":")[0]], N)
     s = wl.make_state(w)
     pos = s.pos.astype(np.float64)
     p = orc.Params.of(w)
+    if name.endswith(":xplor"):   # smoothing from 0.6 r_cut on for every type pair (1.5 sigma at r_cut = 2.5 sigma, PAPER.md:367)
+        p = orc.Params(w.ntypes, w.eps, w.sigma, w.rcut, 2, ron=[0.6 * rc for rc in w.rcut])
     Fb, Ub, Wb = orc.compute_lj_brute(pos, s.type, s.L, p)
     c, r, n = orc.nlist_cells(pos, s.L, w.r_max)
     Fl, Ul, Wl, _ = orc.compute_lj_nlist(pos, s.type, s.L, p, c, r, n)
@@ -418,17 +469,18 @@ def test_energy_fluctuation_scales_as_dt_squared(orc):
     assert 2.8 < fl[0] / fl[1] < 5.5
 
 
-def test_table2_energy_fluctuation_magnitude(orc):
-    """c7 + c4-c6 together against the paper's printed number (Table 2,
-    PAPER.md:383-396): |dE/E| = 2.0(1)e-5 for N=5000, rho=0.4, r_cut=2.5 shifted,
-    T=1, dt=0.005 from an EQUILIBRATED state.  Our start is a jittered lattice
+@pytest.mark.parametrize("mode", ["shift", "xplor"])
+def test_table2_energy_fluctuation_magnitude(orc, mode):
+    """c7 + c4-c6 together against the paper's printed numbers (Table 2,
+    PAPER.md:383-396): |dE/E| = 2.0(1)e-5 (shifted) and 1.90(9)e-5 (XPLOR, r_on = 1.5) for N=5000,
+    rho=0.4, r_cut=2.5, T=1, dt=0.005 from an EQUILIBRATED state.  Our start is a jittered lattice
     brought to T~1 by crude velocity rescaling in this test (the paper used 1e6
-    NVT steps), so this is an order-of-magnitude pin: within a factor 1.5 (measured here: 2.11e-5)."""
-    ref = float(_rows("table2_nve.txt")[0][1])
+    NVT steps), so this is an order-of-magnitude pin: within a factor 1.5 (measured here: 2.11e-5 shifted)."""
+    ref = float(_rows("table2_nve.txt")[0 if mode == "shift" else 5][1])
     N, rho, dt = 5000, 0.4, 0.005
     w = wl.Workload("table2", N, rho, 1.0, 1, (1.0,), (1.0,), (2.5,), 0.4, dt, 0, 1, 0)
     s = wl.make_state(w)
-    p = orc.Params.of(w)
+    p = orc.Params.of(w) if mode == "shift" else orc.Params(1, [1.0], [1.0], [2.5], 2, ron=[1.5])
     pos, vel, img = s.pos, s.vel.astype(np.float64), s.image
     for _ in range(12):                      # melt + thermalise: 12 x 150 steps, rescale to T = 1
         o = orc.run_nve(pos, vel, img, s.type, s.L, p, 0.4, dt, 150)

@@ -58,6 +58,8 @@ extern "C" {
 
 #define HB_SHIFT_NONE 0   /* V = V_lj(r) */
 #define HB_SHIFT_ENERGY 1 /* V = V_lj(r) - V_lj(r_cut); same force */
+#define HB_XPLOR 2        /* V = V_lj(r) S(r): XPLOR smoothing from r_on to r_cut, V and dV/dr -> 0 at r_cut
+                             (PAPER.md:355-367); r_on per type pair from hb_set_ron_pair */
 
 typedef struct hb_system hb_system;
 
@@ -112,6 +114,11 @@ HB_API int hb_get_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_
  * built with the largest of them (reading c2.iii); the force applies each. */
 HB_API int hb_set_rcut_pair(hb_system *h, const double *rcut);
 
+/* Per-type-pair onset r_on,ab [ntypes*ntypes] of the XPLOR switching function S(r), used by
+ * hb_compute_lj(HB_XPLOR).  Default: 3/2 sigma_ab, the paper's test value.  r_on,ab >= r_cut,ab
+ * leaves no switching interval: that pair is plainly truncated (reading x1). */
+HB_API int hb_set_ron_pair(hb_system *h, const double *ron);
+
 /* Algorithm 2: bin the particles into m^3 cells, m = floor(L / r_max), with
  * c = floor((x - b) m / L) per axis evaluated in binary32 without contraction
  * (reading c1).  Uses the r_max of the last hb_build_nlist (or r_cut,max +
@@ -134,7 +141,8 @@ HB_API int hb_build_nlist(hb_system *h, double r_cut, double r_buff);
 HB_API int hb_needs_rebuild(hb_system *h, int *need);
 
 /* F_i, U_i = 1/2 sum V, W_i = 1/2 sum d f over the listed neighbors with
- * r < r_cut,ab.  HB_ESTATE if there is no list. */
+ * r < r_cut,ab.  shift_mode: HB_SHIFT_NONE, HB_SHIFT_ENERGY or HB_XPLOR; it stays in
+ * force for hb_step_nve / hb_run_nve.  HB_ESTATE if there is no list. */
 HB_API int hb_compute_lj(hb_system *h, int shift_mode);
 
 /* One velocity-Verlet step: half kick, drift, wrap with

@@ -67,6 +67,7 @@ int upload_params(hb_system *h)
 {
     const int nt2 = h->ntypes * h->ntypes;
     h->h_params.resize(nt2);
+    h->h_paramsx.resize(nt2);
     double rc_max = 0.0;
     for (int p = 0; p < nt2; p++) {
         const double e = h->eps[p], s = h->sigma[p], rc = h->rcut[p];
@@ -78,10 +79,13 @@ int upload_params(hb_system *h)
         const double sr6 = s6 / std::pow(rc, 6.0);
         pp.eshift = h->shift_mode == HB_SHIFT_ENERGY ? (float)(4.0 * e * (sr6 * sr6 - sr6)) : 0.0f;
         h->h_params[p] = pp;
+        const double ron = h->ron[p], d = rc * rc - ron * ron;
+        h->h_paramsx[p] = PairParamX{(float)(ron * ron), ron < rc ? (float)(1.0 / (d * d * d)) : 0.0f};
         if (rc > rc_max) rc_max = rc;
     }
     h->r_cut_max = (float)rc_max;
     HB_CK(cudaMemcpyAsync(h->params, h->h_params.data(), sizeof(PairParam) * nt2, cudaMemcpyHostToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->paramsx, h->h_paramsx.data(), sizeof(PairParamX) * nt2, cudaMemcpyHostToDevice, h->stream));
     HB_CK(cudaStreamSynchronize(h->stream));  // h_params is pageable
     return HB_OK;
 }
@@ -733,6 +737,8 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     h->sigma.assign(sigma, sigma + ntypes * ntypes);
     h->rcut.resize(ntypes * ntypes);
     for (int p = 0; p < ntypes * ntypes; p++) h->rcut[p] = (double)(float)(2.5 * sigma[p]);
+    h->ron.resize(ntypes * ntypes);
+    for (int p = 0; p < ntypes * ntypes; p++) h->ron[p] = (double)(float)(1.5 * sigma[p]);
     h->stream = (cudaStream_t)cuda_stream;
     if (alloc && alloc->alloc && alloc->free) { h->alloc = *alloc; h->has_alloc = true; }
     *out = h;  // from here on the caller can read hb_last_error and must hb_destroy
@@ -755,6 +761,7 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     HB_TRY(dev_alloc_t(h, &h->perm, n));
     HB_TRY(dev_alloc_t(h, &h->nlistn, n));
     HB_TRY(dev_alloc_t(h, &h->params, (size_t)ntypes * ntypes));
+    HB_TRY(dev_alloc_t(h, &h->paramsx, (size_t)ntypes * ntypes));
     HB_TRY(dev_alloc_t(h, &h->flags, (size_t)FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_flags, sizeof(int) * FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_thermo, sizeof(double) * 16));
@@ -789,7 +796,7 @@ int hb_destroy(hb_system *h)
     if (h->h_total) cudaFreeHost(h->h_total);
     void *ptrs[] = {h->posbuf[0], h->posbuf[1], h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->vel2,
                     h->force2, h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_image,
-                    h->bk_tag, h->params, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
+                    h->bk_tag, h->params, h->paramsx, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
                     h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
                     h->flags, h->thermo_part};
     for (void *p : ptrs) dev_free(h, p);
@@ -879,6 +886,19 @@ int hb_set_rcut_pair(hb_system *h, const double *rcut)
     return upload_params(h);
 }
 
+int hb_set_ron_pair(hb_system *h, const double *ron)
+{
+    HB_NEED(h);
+    if (!ron) { h->err = "ron is NULL"; return HB_EINVAL; }
+    const int nt = h->ntypes;
+    for (int a = 0; a < nt; a++)
+        for (int b = 0; b < nt; b++)
+            if (ron[a * nt + b] != ron[b * nt + a] || !(ron[a * nt + b] > 0.0)) { h->err = "r_on table must be symmetric and positive"; return HB_EINVAL; }
+    for (int p = 0; p < nt * nt; p++) h->ron[p] = (double)(float)ron[p];
+    h->forces_valid = false;
+    return upload_params(h);
+}
+
 int hb_build_cells(hb_system *h)
 {
     HB_NEED(h);
@@ -934,10 +954,11 @@ int hb_compute_lj(hb_system *h, int shift_mode)
 {
     HB_NEED(h);
     Range nvtx_range("hb_compute_lj");
-    if (shift_mode != HB_SHIFT_NONE && shift_mode != HB_SHIFT_ENERGY) { h->err = "unknown shift mode"; return HB_EINVAL; }
+    if (shift_mode != HB_SHIFT_NONE && shift_mode != HB_SHIFT_ENERGY && shift_mode != HB_XPLOR) { h->err = "unknown shift mode"; return HB_EINVAL; }
     if (!h->nlist_valid) { h->err = "no neighbor list: call hb_build_nlist first"; return HB_ESTATE; }
     if (shift_mode != h->shift_mode) {
         h->shift_mode = shift_mode;
+        destroy_graphs(h);     // the captured step kernels are instantiated for one pair functor
         HB_TRY(upload_params(h));
     }
     HB_CK(launch_force(h, nullptr));

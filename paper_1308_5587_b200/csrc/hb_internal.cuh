@@ -37,6 +37,11 @@ struct PairParam {  // one per type pair, 16 B
     float eshift;   // V_lj(r_cut) if energy shift, else 0
 };
 
+struct PairParamX {  // XPLOR smoothing, one per type pair, 8 B
+    float ron2;     // r_on^2
+    float invD;     // 1 / (r_cut^2 - r_on^2)^3, 0 where r_on >= r_cut (no switching interval)
+};
+
 // A tile is a brick of tx x ty x tz cells (clipped at the upper faces of the box).  One
 // thread block owns one tile: it stages the positions of the tile's cells and of the
 // one-cell halo around them in shared memory, already shifted to the periodic image
@@ -84,8 +89,9 @@ struct hb_system {
     float L = 0, r_cut_max = 0, r_buff = 0, r_max = 0;
     int shift_mode = HB_SHIFT_ENERGY;
     bool rcut_user = false;  // hb_set_rcut_pair was called
-    std::vector<double> eps, sigma, rcut;
+    std::vector<double> eps, sigma, rcut, ron;
     std::vector<PairParam> h_params;
+    std::vector<PairParamX> h_paramsx;
     cudaStream_t stream = nullptr;
     hb_allocator alloc{};
     bool has_alloc = false;
@@ -112,6 +118,7 @@ struct hb_system {
     uint32_t *bk_tag = nullptr;
     int bk_cur = 0, bk_parity = 0;
     PairParam *params = nullptr;
+    PairParamX *paramsx = nullptr;
 
     float4 *pos() const { return posbuf[cur]; }
 
@@ -188,10 +195,13 @@ struct hb_system {
 
 static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
+// threads per particle of the step kernel actually launched (the smoothed functor exists in the default layout only)
+static inline int force_tpp(const hb_system *h) { return h->shift_mode == HB_XPLOR ? 2 : h->tun.tpp; }
+
 static inline int force_block_of(const hb_system *h)
 {
     if (h->tun.force_block > 0) return h->tun.force_block;
-    return h->own_est * h->tun.tpp > 160.0 ? 256 : 128;
+    return h->own_est * force_tpp(h) > 160.0 ? 256 : 128;
 }
 
 // What the drift part of a step kernel needs (nve_kernel and the fused force kernel).

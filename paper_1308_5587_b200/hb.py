@@ -19,10 +19,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libhb.so")
 
 HB_OK, HB_EINVAL, HB_ECUDA, HB_ENOMEM, HB_EBOX, HB_ESTATE, HB_ENAN = 0, -1, -2, -3, -4, -5, -6
-HB_SHIFT_NONE, HB_SHIFT_ENERGY = 0, 1
+HB_SHIFT_NONE, HB_SHIFT_ENERGY, HB_XPLOR = 0, 1, 2
 _ERR_NAMES = {-1: "HB_EINVAL", -2: "HB_ECUDA", -3: "HB_ENOMEM", -4: "HB_EBOX", -5: "HB_ESTATE", -6: "HB_ENAN"}
 
-EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_build_cells",
+EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_set_ron_pair", "hb_build_cells",
            "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_sort",
            "hb_thermo", "hb_get_cells", "hb_get_nlist", "hb_get_forces", "hb_stats", "hb_set_tunable",
            "hb_get_tunable", "hb_time_stage", "hb_measure_peak", "hb_last_error", "hb_version"]
@@ -68,6 +68,7 @@ def load():
     L.hb_set_state.argtypes = [vp, vp, vp, vp, vp, i32]
     L.hb_get_state.argtypes = [vp, vp, vp, vp, vp, vp, i32]
     L.hb_set_rcut_pair.argtypes = [vp, vp]
+    L.hb_set_ron_pair.argtypes = [vp, vp]
     L.hb_build_cells.argtypes = [vp]
     L.hb_build_nlist.argtypes = [vp, dbl, dbl]
     L.hb_needs_rebuild.argtypes = [vp, C.POINTER(i32)]
@@ -226,6 +227,12 @@ class System:
         if rcut.size != self.ntypes ** 2:
             raise ValueError("rcut must have ntypes*ntypes entries")
         self._ck(self._lib.hb_set_rcut_pair(self._h, rcut.ctypes.data_as(C.c_void_p)))
+
+    def set_ron_pair(self, ron):
+        ron = np.ascontiguousarray(ron, dtype=np.float64).ravel()
+        if ron.size != self.ntypes ** 2:
+            raise ValueError("ron must have ntypes*ntypes entries")
+        self._ck(self._lib.hb_set_ron_pair(self._h, ron.ctypes.data_as(C.c_void_p)))
 
     def build_cells(self):
         self._ck(self._lib.hb_build_cells(self._h))

@@ -569,6 +569,150 @@ done:
     return rc;
 }
 
+/* ------------------------------------------------ NEXT-2: thermostats ---- */
+/* The paper names a Nose-Hoover NVT integrator with a time constant ("The time constants for
+ * NVT and NPT are all set to 1.0") and a Langevin / Brownian-dynamics integrator that needs parallel random
+ * numbers, and prints no equation for either.  Readings (DESIGN.md n1, n2):
+ *
+ * [n1] Nose-Hoover: dv/dt = F/m - xi v,  dxi/dt = (T_k / T - 1) / tau^2,  deta/dt = xi,
+ *      T_k = 2 K / g with g = 3 N - 3 degrees of freedom (the total momentum is conserved), m = 1, k_B = 1.
+ *      One step, a time-reversible splitting around the force evaluation:
+ *        v' = (v + (dt/2) F(t)) / (1 + (dt/2) xi);   x(t+dt) = x + dt v'  (wrap, image flags as in c7)
+ *        xi' = xi + (dt / tau^2) (T_k(v') / T - 1);   eta' = eta + (dt/2)(xi + xi')
+ *        F(t+dt);   v(t+dt) = v' + (dt/2) (F(t+dt) - xi' v')
+ *      Conserved: H' = K + U + g T (tau^2 xi^2 / 2 + eta).
+ *
+ * [n2] Langevin: dv/dt = F/m - gamma v + R(t), <R_a(t) R_b(t')> = 2 gamma T delta_ab delta(t - t').
+ *      One step: the velocity-Verlet step of c7, then the thermostat acts on the new velocity for a whole step,
+ *        v <- v (1 - gamma dt) + sqrt(6 gamma T dt) u,   u uniform in (-1, 1) per component (variance 1/3),
+ *      so that for free particles <v^2> = T / (1 - gamma dt / 2) per component.
+ *      u comes from a counter-based generator: splitmix64 finaliser of (seed, stream = time step number,
+ *      index = 3 tag + component), the generator of workloads.py; 23 bits k give u = (2k + 1 - 2^23) / 2^23,
+ *      exact in binary32, so a binary32 implementation draws the same numbers. */
+static inline uint64_t orc_mix64(uint64_t z)
+{
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
+    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return z;
+}
+
+uint64_t orc_counter_u64(uint64_t seed, uint64_t stream, uint64_t index)
+{
+    const uint64_t G = 0x9E3779B97F4A7C15ULL;
+    uint64_t s = orc_mix64(seed + G);
+    s = orc_mix64(s + stream * G);
+    return orc_mix64(s + (index + 1) * G);
+}
+
+double orc_uniform_pm1(uint64_t seed, uint64_t stream, uint64_t index)
+{
+    const uint64_t k = orc_counter_u64(seed, stream, index) >> 41;          /* 23 bits */
+    return ((double)(2 * (int64_t)k + 1) - 8388608.0) / 8388608.0;
+}
+
+/* nsteps of thermostatted dynamics with the list rebuilt on buffer exceedance (same loop as orc_run_nve).
+ * mode 1: Nose-Hoover, par = tau, state[0..1] = (xi, eta) in and out.
+ * mode 2: Langevin, par = gamma, state[0] = number of the first time step (stream of the generator), advanced.
+ * log (nullable) [nsteps+1][4]: K, U, xi, eta at every step incl. step 0.  tag[i] = identity of particle i for
+ * the generator (NULL: i). */
+int orc_run_thermostat(int mode, double *pos, double *vel, int32_t *image, const int32_t *type, int64_t N, double L,
+                       int ntypes, const double *eps, const double *sigma, const double *rcut, const double *ron, int shift,
+                       double r_buff, double dt, int64_t nsteps, double T, double par, uint64_t seed, double *state,
+                       int have_forces, double *F, double *U, double *W, double *log, int64_t *stats)
+{
+    double r_cut_max = 0.0;
+    for (int p = 0; p < ntypes * ntypes; p++) if (rcut[p] > r_cut_max) r_cut_max = rcut[p];
+    const double r_max = r_cut_max + r_buff;
+    const int m = orc_cell_dim(L, r_max);
+    if (m < 3) return ORC_EBOX;
+    if (mode != 1 && mode != 2) return ORC_ECAP;
+    const int64_t nc = (int64_t)m * m * m;
+    int32_t *cell = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    int64_t *cell_start = (int64_t *)malloc((size_t)(nc + 1) * sizeof(int64_t));
+    int32_t *members = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    int32_t *count = (int32_t *)malloc((size_t)N * sizeof(int32_t));
+    int64_t *row_start = (int64_t *)malloc((size_t)(N + 1) * sizeof(int64_t));
+    double *pos_build = (double *)malloc((size_t)3 * N * sizeof(double));
+    int32_t *nbr = NULL;
+    int64_t cap = 0, builds = 0, maxlen = 0;
+    int rc = ORC_OK, need_build = 1;
+    const double g = 3.0 * (double)N - 3.0;
+    double xi = mode == 1 ? state[0] : 0.0, eta = mode == 1 ? state[1] : 0.0;
+    uint64_t tstep = mode == 2 ? (uint64_t)state[0] : 0;
+    if (!cell || !cell_start || !members || !count || !row_start || !pos_build) { rc = ORC_ENOMEM; goto done; }
+
+    for (int64_t step = 0; step <= nsteps; step++) {
+        if (step > 0) {
+            if (mode == 1) {
+                /* [n1] first half: friction implicit, drift, wrap */
+                for (int64_t k = 0; k < 3 * N; k++) {
+                    vel[k] = (vel[k] + 0.5 * dt * F[k]) / (1.0 + 0.5 * dt * xi);
+                    double x = pos[k] + dt * vel[k];
+                    if (x >= 0.5 * L) { x -= L; image[k] += 1; }
+                    else if (x < -0.5 * L) { x += L; image[k] -= 1; }
+                    pos[k] = x;
+                }
+                double K = 0.0;
+                for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * vel[k] * vel[k];
+                const double xi_new = xi + dt / (par * par) * ((2.0 * K / g) / T - 1.0);
+                eta += 0.5 * dt * (xi + xi_new);
+                xi = xi_new;
+            } else {
+                orc_nve_step1(pos, vel, F, image, N, L, dt);
+            }
+            const double half = 0.5 * r_buff;
+            if (!need_build && orc_max_disp2(pos, pos_build, N, L) > half * half) need_build = 1;
+        }
+        if (step > 0 || !have_forces) {
+            if (need_build) {
+                orc_cell_index_f64(pos, N, L, m, cell, NULL);
+                orc_build_cells(cell, N, m, cell_start, members);
+                rc = orc_nlist_cells(pos, N, L, r_max, m, cell, cell_start, members, count, NULL, NULL);
+                if (rc) goto done;
+                row_start[0] = 0;
+                for (int64_t i = 0; i < N; i++) {
+                    row_start[i + 1] = row_start[i] + count[i];
+                    if (count[i] > maxlen) maxlen = count[i];
+                }
+                if (row_start[N] > cap) {
+                    free(nbr);
+                    cap = row_start[N] + row_start[N] / 8 + 16;
+                    nbr = (int32_t *)malloc((size_t)cap * sizeof(int32_t));
+                    if (!nbr) { rc = ORC_ENOMEM; goto done; }
+                }
+                orc_nlist_cells(pos, N, L, r_max, m, cell, cell_start, members, count, row_start, nbr);
+                memcpy(pos_build, pos, (size_t)3 * N * sizeof(double));
+                need_build = 0;
+                builds++;
+            }
+            orc_compute_lj_nlist(pos, type, N, L, ntypes, eps, sigma, rcut, ron, shift,
+                                 count, row_start, nbr, 0.0, F, U, W, NULL);
+        }
+        if (step > 0) {
+            if (mode == 1) {
+                for (int64_t k = 0; k < 3 * N; k++) vel[k] = vel[k] + 0.5 * dt * (F[k] - xi * vel[k]);   /* [n1] second half */
+            } else {
+                orc_nve_step2(vel, F, N, dt);
+                const double c = 1.0 - par * dt, sgm = sqrt(6.0 * par * T * dt);                        /* [n2] */
+                for (int64_t k = 0; k < 3 * N; k++) vel[k] = vel[k] * c + sgm * orc_uniform_pm1(seed, tstep, (uint64_t)k);
+                tstep++;
+            }
+        }
+        if (log) {
+            double K = 0.0, Ut = 0.0;
+            for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * vel[k] * vel[k];
+            for (int64_t i = 0; i < N; i++) Ut += U[i];
+            log[4 * step] = K; log[4 * step + 1] = Ut; log[4 * step + 2] = xi; log[4 * step + 3] = eta;
+        }
+    }
+    if (mode == 1) { state[0] = xi; state[1] = eta; } else state[0] = (double)tstep;
+    if (stats) { stats[0] = builds; stats[1] = maxlen; }
+done:
+    free(cell); free(cell_start); free(members); free(count); free(row_start); free(pos_build); free(nbr);
+    return rc;
+}
+
 int orc_num_threads(void)
 {
 #ifdef _OPENMP

@@ -64,6 +64,13 @@ def lib():
         L.orc_sort_perm.argtypes = [_up, C.c_int64, C.c_int, _lp]
         L.orc_run_nve.argtypes = [_dp, _dp, _ip, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int,
                                   C.c_double, C.c_double, C.c_int64, C.c_int, _dp, _dp, _dp, _vp, _vp]
+        L.orc_counter_u64.restype = C.c_uint64
+        L.orc_counter_u64.argtypes = [C.c_uint64] * 3
+        L.orc_uniform_pm1.restype = C.c_double
+        L.orc_uniform_pm1.argtypes = [C.c_uint64] * 3
+        L.orc_run_thermostat.argtypes = [C.c_int, _dp, _dp, _ip, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int,
+                                         C.c_double, C.c_double, C.c_int64, C.c_double, C.c_double, C.c_uint64, _dp,
+                                         C.c_int, _dp, _dp, _dp, _vp, _vp]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -258,6 +265,43 @@ def run_nve(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, forces=None,
     _check(lib().orc_run_nve(pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
                              float(r_buff), float(dt), int(nsteps), have, F, U, W, _ptr(KU), _ptr(stats)), "run_nve")
     return dict(pos=pos, vel=vel, image=image, F=F, U=U, W=W, KU=KU, builds=int(stats[0]), max_nbrs=int(stats[1]))
+
+
+def counter_u64(seed, stream, index):
+    return int(lib().orc_counter_u64(int(seed), int(stream), int(index)))
+
+
+def uniform_pm1(seed, stream, index):
+    return lib().orc_uniform_pm1(int(seed), int(stream), int(index))
+
+
+def _run_thermostat(mode, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, par, seed, state, forces, log):
+    pos, vel = _d(pos).copy(), _d(vel).copy()
+    image = np.ascontiguousarray(image, dtype=np.int32).copy()
+    typ = np.ascontiguousarray(typ, dtype=np.int32)
+    N = len(pos)
+    if forces is None:
+        F, U, W, have = np.zeros((N, 3)), np.zeros(N), np.zeros((N, 6)), 0
+    else:
+        F, U, W = (_d(x).copy() for x in forces)
+        have = 1
+    lg = np.zeros((nsteps + 1, 4)) if log else None
+    stats = np.zeros(2, dtype=np.int64)
+    st = np.array(state, dtype=np.float64)
+    _check(lib().orc_run_thermostat(mode, pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
+                                    float(r_buff), float(dt), int(nsteps), float(T), float(par), int(seed), st, have,
+                                    F, U, W, _ptr(lg), _ptr(stats)), "run_thermostat")
+    return dict(pos=pos, vel=vel, image=image, F=F, U=U, W=W, log=lg, state=st, builds=int(stats[0]))
+
+
+def run_nvt(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, T, tau, xi=0.0, eta=0.0, forces=None, log=False):
+    """Nose-Hoover (reading n1); returns dict(pos, vel, image, F, U, W, log[K, U, xi, eta], state=[xi, eta])."""
+    return _run_thermostat(1, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, tau, 0, [xi, eta], forces, log)
+
+
+def run_langevin(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, T, gamma, seed, step0=0, forces=None, log=False):
+    """Langevin (reading n2); state[0] = number of the next time step."""
+    return _run_thermostat(2, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, gamma, seed, [float(step0), 0.0], forces, log)
 
 
 def num_threads():

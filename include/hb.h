@@ -157,6 +157,19 @@ HB_API int hb_step_nve(hb_system *h, double dt);
  * saved at the start of the affected chunk and redoing it with longer rows. */
 HB_API int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period);
 
+/* The same loop with a thermostat (the paper names the integrators, PAPER.md:87, 99, 324,
+ * and prints no equations: readings n1, n2 of DESIGN.md).  k_B = 1, m = 1.
+ * hb_run_nvt: Nose-Hoover, dv/dt = F - xi v, dxi/dt = (T_k / T - 1) / tau^2 with T_k = 2K / (3N - 3); the
+ *   thermostat variable xi and its time integral eta live in the handle (hb_get_thermostat / hb_set_thermostat;
+ *   hb_set_state zeroes them); K + U + (3N - 3) T (tau^2 xi^2 / 2 + eta) is conserved.
+ * hb_run_langevin: after every velocity-Verlet step v <- v (1 - gamma dt) + sqrt(6 gamma T dt) u, u uniform in
+ *   (-1, 1) from the counter-based generator splitmix64(seed, time step number, 3 tag + component); the time step
+ *   number counts the Langevin steps since hb_set_state (hb_get_thermostat reports it). */
+HB_API int hb_run_nvt(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, double T, double tau);
+HB_API int hb_run_langevin(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, double T, double gamma, uint64_t seed);
+HB_API int hb_get_thermostat(hb_system *h, double *xi, double *eta, int64_t *langevin_steps);
+HB_API int hb_set_thermostat(hb_system *h, double xi, double eta, int64_t langevin_steps);
+
 /* Reorder the particles along a Hilbert curve on a 2^8 grid per axis, equal keys
  * in tag order (reading c8); permutes every per-particle array, keeps the
  * tags, invalidates the list.  (Every list build re-orders the particles into

@@ -38,6 +38,7 @@
 //     and writes the new position into the OTHER position buffer, since the blocks
 //     around still read the old one.  One kernel per time step.
 #include "tile.cuh"
+#include "integrate_dev.cuh"
 
 __device__ __forceinline__ float rcp_approx(float x)
 {
@@ -363,6 +364,8 @@ lj_tile_kernel(const ForceArgs A)
     const float hdt = 0.5f * nv.dt, hL = 0.5f * g.L, L = g.L;
     const unsigned char *stage_b = reinterpret_cast<const unsigned char *>(stage);
     bool exceed = false;
+    double ksum = 0.0;
+    const float xi = (nve && nv.ens == 1) ? (float)nv.tstate[TS_XI] : 0.f;   // read by every block before the last one updates it
 
     for (int q0 = 0; q0 < nown; q0 += PPB) {     // block-uniform trip count: the shuffles need whole warps
         const bool active = active_n;
@@ -440,16 +443,11 @@ lj_tile_kernel(const ForceArgs A)
         if (sub != 0) continue;
         if (THERMO) A.force[gi] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
         if (!nve) continue;
-        // reading c7, operation by operation as nve_kernel does it
-        if (nv.kick_prev) {
-            v.x = __fmaf_rn(hdt, a.fx, v.x);
-            v.y = __fmaf_rn(hdt, a.fy, v.y);
-            v.z = __fmaf_rn(hdt, a.fz, v.z);
-        }
+        // reading c7 (and n1, n2), operation by operation as nve_kernel does it
+        if (nv.kick_prev) thermo_kick_prev(nv, xi, hdt, a.fx, a.fy, a.fz, v, nv.ens == 2 ? nv.tag[gi] : 0u);
         if (nv.kick_drift) {
-            v.x = __fmaf_rn(hdt, a.fx, v.x);
-            v.y = __fmaf_rn(hdt, a.fy, v.y);
-            v.z = __fmaf_rn(hdt, a.fz, v.z);
+            thermo_kick_first(nv, xi, hdt, a.fx, a.fy, a.fz, v);
+            if (nv.ens == 1) ksum += 0.5 * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
             // p is the stored position: the staged one may be another periodic image of it
             p.x = __fmaf_rn(nv.dt, v.x, p.x);
             p.y = __fmaf_rn(nv.dt, v.y, p.y);
@@ -470,19 +468,7 @@ lj_tile_kernel(const ForceArgs A)
 
     if (drift) {
         if (exceed) A.flags[nv.need_set] = 1;
-        if (nv.use_cond) {
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                __threadfence();
-                const int ticket = atomicAdd(&A.flags[FL_DONE_CTR], 1);
-                if (ticket == (int)(gridDim.x * gridDim.y * gridDim.z) - 1) {
-                    __threadfence();
-                    const int need = *((volatile int *)&A.flags[nv.need_set]);
-                    cudaGraphSetConditional(nv.cond, need ? 1u : 0u);
-                    A.flags[FL_DONE_CTR] = 0;
-                }
-            }
-        }
+        step_epilogue(nv, A.flags, ksum, gridDim.x * gridDim.y * gridDim.z);
     }
 }
 

@@ -394,6 +394,14 @@ NveArgs make_nve(hb_system *h, float dt, bool kick_prev, bool kick_drift, float4
     a.need_clear = FL_NEED0 + ((h->parity + 1) & 1);
     a.cond = cond;
     a.use_cond = use_cond ? 1 : 0;
+    a.ens = h->ens.mode;
+    a.T = (float)h->ens.T;
+    a.par = (float)h->ens.par;
+    a.gdof = 3.0 * (double)h->N - 3.0;
+    a.seed = h->ens.seed;
+    a.kick_step = h->parity - h->parity0 - 1;   // the step whose drift was the last one launched
+    a.tstate = h->tstate;
+    a.tag = h->tag;
     return a;
 }
 
@@ -557,6 +565,7 @@ int backup_state(hb_system *h)
     HB_CK(cudaMemcpyAsync(h->bk_vel, h->vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_image, h->image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->bk_tag, h->tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->bk_tstate, h->tstate, sizeof(double) * TS_COUNT, cudaMemcpyDeviceToDevice, h->stream));
     h->bk_cur = h->cur;
     h->bk_parity = h->parity;
     h->bk_valid = true;
@@ -572,6 +581,7 @@ int restore_state(hb_system *h)
     HB_CK(cudaMemcpyAsync(h->vel, h->bk_vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->image, h->bk_image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(cudaMemcpyAsync(h->tag, h->bk_tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(cudaMemcpyAsync(h->tstate, h->bk_tstate, sizeof(double) * TS_COUNT, cudaMemcpyDeviceToDevice, h->stream));
     HB_CK(launch_rtag(h));
     HB_TRY(clear_need_flags(h));
     // forces and virials are not saved: the rebuild that follows a restore changes the order, they are recomputed
@@ -584,6 +594,11 @@ int restore_state(hb_system *h)
 int step_sync(hb_system *h, float dt)
 {
     HB_TRY(ensure_forces(h));
+    h->parity0 = h->parity;
+    if (h->ens.mode == 2) {
+        *reinterpret_cast<long long *>(h->h_tstate + TS_LBASE) = (long long)h->lang_steps;
+        HB_CK(cudaMemcpyAsync(h->tstate + TS_LBASE, h->h_tstate + TS_LBASE, sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    }
     const NveArgs a = make_nve(h, dt, false, true, h->pos(), 0, false);
     HB_CK(launch_nve(h, a));
     h->parity++;
@@ -594,6 +609,7 @@ int step_sync(hb_system *h, float dt)
     h->forces_valid = true;
     HB_CK(launch_nve(h, make_nve(h, dt, true, false, h->pos(), 0, false)));
     h->stats.steps++;
+    if (h->ens.mode == 2) h->lang_steps++;
     return HB_OK;
 }
 
@@ -605,6 +621,11 @@ int normalize_for_chunk(hb_system *h)
         h->cur = 0;
     }
     h->parity = 0;
+    h->parity0 = 0;
+    if (h->ens.mode == 2) {       // the generator's stream = number of the time step: tell the device where the chunk starts
+        *reinterpret_cast<long long *>(h->h_tstate + TS_LBASE) = (long long)h->lang_steps;
+        HB_CK(cudaMemcpyAsync(h->tstate + TS_LBASE, h->h_tstate + TS_LBASE, sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    }
     return clear_need_flags(h);   // no decision is pending between chunks: every drift's rebuild ran inside its chunk
 }
 
@@ -614,7 +635,7 @@ int chunk_kernels(const hb_system *h, int n) { return (h->tun.fuse_nve ? n + 1 :
 // the first call, so that no later call captures or instantiates anything (hb_stats: graph_builds).
 int ensure_graphs(hb_system *h, float dt)
 {
-    if (dt != h->graph_dt) { destroy_graphs(h); h->graph_dt = dt; }
+    if (dt != h->graph_dt || !(h->ens == h->graph_ens)) { destroy_graphs(h); h->graph_dt = dt; h->graph_ens = h->ens; }
     if (!h->graphs.empty() || h->tun.graph_mode == 0 || h->tun.graph_mode == 3) return HB_OK;
     Range r("hb:build_graphs");
     std::vector<int> sizes{h->tun.graph_steps};
@@ -674,6 +695,7 @@ int run_chunk(hb_system *h, float dt, int n)
             }
             if (nb > 0) h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
             h->stats.steps += n;
+            if (h->ens.mode == 2) h->lang_steps += n;
             return HB_OK;
         }
         // Some build inside the chunk overflowed its rows or its staging area: go back, grow, redo.
@@ -766,6 +788,11 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     HB_CK(cudaMallocHost((void **)&h->h_flags, sizeof(int) * FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_thermo, sizeof(double) * 16));
     HB_CK(cudaMallocHost((void **)&h->h_total, sizeof(int) * 2));
+    HB_CK(cudaMallocHost((void **)&h->h_tstate, sizeof(double) * TS_COUNT));
+    memset(h->h_tstate, 0, sizeof(double) * TS_COUNT);
+    HB_TRY(dev_alloc_t(h, &h->tstate, (size_t)TS_COUNT));
+    HB_TRY(dev_alloc_t(h, &h->bk_tstate, (size_t)TS_COUNT));
+    HB_CK(cudaMemsetAsync(h->tstate, 0, sizeof(double) * TS_COUNT, h->stream));
     HB_TRY(dev_alloc_t(h, &h->acc_counts, n + 1));
     HB_TRY(dev_alloc_t(h, &h->acc_rows, n + 2));
     memset(h->h_flags, 0, sizeof(int) * FL_COUNT);
@@ -794,6 +821,9 @@ int hb_destroy(hb_system *h)
     dev_free(h, h->acc_counts);
     dev_free(h, h->acc_rows);
     if (h->h_total) cudaFreeHost(h->h_total);
+    if (h->h_tstate) cudaFreeHost(h->h_tstate);
+    dev_free(h, h->tstate);
+    dev_free(h, h->bk_tstate);
     void *ptrs[] = {h->posbuf[0], h->posbuf[1], h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->vel2,
                     h->force2, h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_image,
                     h->bk_tag, h->params, h->paramsx, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
@@ -835,6 +865,8 @@ int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type, const 
     h->cells_valid = h->nlist_valid = h->forces_valid = h->bk_valid = false;
     h->moved = true;
     h->since_sort = -1;
+    h->lang_steps = 0;
+    HB_CK(cudaMemsetAsync(h->tstate, 0, sizeof(double) * TS_COUNT, h->stream));
     if (h->h_flags[FL_BADTYPE]) {
         HB_TRY(set_flag(h, FL_BADTYPE, 0));
         h->have_state = false;
@@ -975,19 +1007,19 @@ int hb_step_nve(hb_system *h, double dt)
     return step_sync(h, (float)dt);
 }
 
-int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
+static int run_md(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, const Ensemble &ens)
 {
-    HB_NEED(h);
-    Range nvtx_range("hb_run_nve");
     if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
     if (nsteps < 0 || sort_period < 0) return HB_EINVAL;
     if (h->m == 0) HB_TRY(configure_geometry(h));
+    h->ens = ens;
     int64_t done = 0;
-    while (done < nsteps) {
+    int rc = HB_OK;
+    while (done < nsteps && rc == HB_OK) {
         // sort before the first step ever run, then every sort_period steps (counted across calls)
         if (sort_period > 0 && (h->since_sort < 0 || h->since_sort >= sort_period)) {
-            HB_TRY(ensure_forces(h));
-            HB_TRY(sort_internal(h));
+            if ((rc = ensure_forces(h)) != HB_OK) break;
+            if ((rc = sort_internal(h)) != HB_OK) break;
             h->since_sort = 0;
         }
         int64_t n = std::min<int64_t>(h->tun.graph_steps, nsteps - done);
@@ -997,10 +1029,62 @@ int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
             while (2 * p2 <= n) p2 *= 2;
             n = p2;
         }
-        HB_TRY(run_chunk(h, (float)dt, (int)n));
+        rc = run_chunk(h, (float)dt, (int)n);
         done += n;
         if (h->since_sort >= 0) h->since_sort += n;
     }
+    h->ens = Ensemble{};      // hb_step_nve and the accessors integrate NVE
+    return rc;
+}
+
+int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
+{
+    HB_NEED(h);
+    Range nvtx_range("hb_run_nve");
+    return run_md(h, dt, nsteps, sort_period, Ensemble{});
+}
+
+int hb_run_nvt(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, double T, double tau)
+{
+    HB_NEED(h);
+    Range nvtx_range("hb_run_nvt");
+    if (!(T > 0.0) || !(tau > 0.0)) { h->err = "hb_run_nvt: T and tau must be positive"; return HB_EINVAL; }
+    Ensemble e;
+    e.mode = 1; e.T = (double)(float)T; e.par = (double)(float)tau;
+    return run_md(h, dt, nsteps, sort_period, e);
+}
+
+int hb_run_langevin(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, double T, double gamma, uint64_t seed)
+{
+    HB_NEED(h);
+    Range nvtx_range("hb_run_langevin");
+    if (!(T >= 0.0) || !(gamma >= 0.0)) { h->err = "hb_run_langevin: T and gamma must not be negative"; return HB_EINVAL; }
+    Ensemble e;
+    e.mode = 2; e.T = (double)(float)T; e.par = (double)(float)gamma; e.seed = seed;
+    return run_md(h, dt, nsteps, sort_period, e);
+}
+
+int hb_get_thermostat(hb_system *h, double *xi, double *eta, int64_t *langevin_steps)
+{
+    HB_NEED(h);
+    HB_CK(cudaMemcpyAsync(h->h_tstate, h->tstate, sizeof(double) * TS_COUNT, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    if (xi) *xi = h->h_tstate[TS_XI];
+    if (eta) *eta = h->h_tstate[TS_ETA];
+    if (langevin_steps) *langevin_steps = h->lang_steps;
+    return HB_OK;
+}
+
+int hb_set_thermostat(hb_system *h, double xi, double eta, int64_t langevin_steps)
+{
+    HB_NEED(h);
+    if (langevin_steps < 0) return HB_EINVAL;
+    memset(h->h_tstate, 0, sizeof(double) * TS_COUNT);
+    h->h_tstate[TS_XI] = xi;
+    h->h_tstate[TS_ETA] = eta;
+    HB_CK(cudaMemcpyAsync(h->tstate, h->h_tstate, sizeof(double) * TS_COUNT, cudaMemcpyHostToDevice, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    h->lang_steps = langevin_steps;
     return HB_OK;
 }
 

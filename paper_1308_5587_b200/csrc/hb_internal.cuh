@@ -83,6 +83,15 @@ struct Tunables {
     int graph_steps = 100;
 };
 
+enum { TS_XI = 0, TS_ETA = 1, TS_KSUM = 2, TS_LBASE = 3, TS_COUNT = 8 };
+
+struct Ensemble {
+    int mode = 0;               // 0 NVE, 1 Nose-Hoover, 2 Langevin
+    double T = 0, par = 0;
+    unsigned long long seed = 0;
+    bool operator==(const Ensemble &o) const { return mode == o.mode && T == o.T && par == o.par && seed == o.seed; }
+};
+
 struct hb_system {
     int64_t N = 0;
     int ntypes = 1;
@@ -162,6 +171,11 @@ struct hb_system {
     bool have_state = false, cells_valid = false, nlist_valid = false, forces_valid = false, bk_valid = false;
     bool moved = true;           // positions changed since the last cell build
     int parity = 0;              // number of drifts done so far, mod 2
+    int parity0 = 0;             // its value at the start of the running chunk (0 for graph chunks)
+    Ensemble ens, graph_ens;     // the integration method of the running call, and the one the cached graphs were captured for
+    double *tstate = nullptr, *bk_tstate = nullptr;   // device [TS_COUNT]: thermostat state (NveArgs::tstate), and its chunk backup
+    double *h_tstate = nullptr;  // pinned [TS_COUNT]
+    int64_t lang_steps = 0;      // Langevin steps taken since hb_set_state (the stream of the generator)
     hb_stats_t stats{};
     int64_t since_sort = -1;     // steps since the last hb_sort inside hb_run_nve (-1 = never sorted)
 
@@ -216,7 +230,16 @@ struct NveArgs {
     int need_set, need_clear;   // flag indices
     cudaGraphConditionalHandle cond;
     int use_cond;
+    // thermostats (readings n1, n2).  ens: 0 NVE, 1 Nose-Hoover, 2 Langevin
+    int ens;
+    float T, par;               // set temperature; tau (Nose-Hoover) or gamma (Langevin)
+    double gdof;                // 3N - 3
+    unsigned long long seed;    // Langevin
+    int kick_step;              // number, inside the chunk, of the time step whose second half kick this launch makes
+    double *tstate;             // device: [0] xi, [1] eta, [2] sum of v'^2 / 2 of the running drift, [3] (as int64) Langevin steps done before the chunk
+    const uint32_t *tag;        // Langevin: the generator is indexed by the particle's identity
 };
+
 
 // ---- kernel launchers (each enqueues on h->stream and returns cudaGetLastError) ----
 // cells.cu: Algorithm 2 + reorder of the particle data into cell order

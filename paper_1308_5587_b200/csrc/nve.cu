@@ -2,6 +2,7 @@
 // that decides when the neighbor list is rebuilt (reading c3), the
 // thermodynamic reduction and the state pack/unpack kernels.
 #include "hb_internal.cuh"
+#include "integrate_dev.cuh"
 
 // The stand-alone integrator kernel (hb_step_nve, the first drift of a run, fuse_nve = 0):
 //   kick_prev  : v += (dt/2) F   -- second half of the previous step (reading c7)
@@ -16,19 +17,16 @@ nve_kernel(float4 *pos, const float4 *__restrict__ force, int N, float L, int *_
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const float hdt = 0.5f * nv.dt, hL = 0.5f * L, dt = nv.dt;
     bool exceed = false;
+    double ksum = 0.0;
+    const float xi = nv.ens == 1 ? (float)nv.tstate[TS_XI] : 0.f;     // read by every block before the last one updates it
     if (nv.kick_drift && i == 0) flags[nv.need_clear] = 0;
     if (i < N) {
         float4 v = nv.vel[i];
         const float4 f = force[i];
-        if (nv.kick_prev) {
-            v.x = __fmaf_rn(hdt, f.x, v.x);
-            v.y = __fmaf_rn(hdt, f.y, v.y);
-            v.z = __fmaf_rn(hdt, f.z, v.z);
-        }
+        if (nv.kick_prev) thermo_kick_prev(nv, xi, hdt, f.x, f.y, f.z, v, nv.ens == 2 ? nv.tag[i] : 0u);
         if (nv.kick_drift) {
-            v.x = __fmaf_rn(hdt, f.x, v.x);
-            v.y = __fmaf_rn(hdt, f.y, v.y);
-            v.z = __fmaf_rn(hdt, f.z, v.z);
+            thermo_kick_first(nv, xi, hdt, f.x, f.y, f.z, v);
+            if (nv.ens == 1) ksum = 0.5 * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
             float4 p = pos[i];
             p.x = __fmaf_rn(dt, v.x, p.x);
             p.y = __fmaf_rn(dt, v.y, p.y);
@@ -49,19 +47,7 @@ nve_kernel(float4 *pos, const float4 *__restrict__ force, int N, float L, int *_
     }
     if (nv.kick_drift) {
         if (__any_sync(0xffffffffu, exceed) && (threadIdx.x & 31) == 0) flags[nv.need_set] = 1;
-        if (nv.use_cond) {
-            __syncthreads();
-            if (threadIdx.x == 0) {
-                __threadfence();
-                const int ticket = atomicAdd(&flags[FL_DONE_CTR], 1);
-                if (ticket == (int)gridDim.x - 1) {
-                    __threadfence();
-                    const int need = *((volatile int *)&flags[nv.need_set]);
-                    cudaGraphSetConditional(nv.cond, need ? 1u : 0u);
-                    flags[FL_DONE_CTR] = 0;
-                }
-            }
-        }
+        step_epilogue(nv, flags, ksum, gridDim.x);
     }
 }
 

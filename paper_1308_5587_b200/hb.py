@@ -23,7 +23,8 @@ HB_SHIFT_NONE, HB_SHIFT_ENERGY, HB_XPLOR = 0, 1, 2
 _ERR_NAMES = {-1: "HB_EINVAL", -2: "HB_ECUDA", -3: "HB_ENOMEM", -4: "HB_EBOX", -5: "HB_ESTATE", -6: "HB_ENAN"}
 
 EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_set_ron_pair", "hb_build_cells",
-           "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_sort",
+           "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_run_nvt", "hb_run_langevin",
+           "hb_get_thermostat", "hb_set_thermostat", "hb_sort",
            "hb_thermo", "hb_get_cells", "hb_get_nlist", "hb_get_forces", "hb_stats", "hb_set_tunable",
            "hb_get_tunable", "hb_time_stage", "hb_measure_peak", "hb_last_error", "hb_version"]
 
@@ -75,6 +76,10 @@ def load():
     L.hb_compute_lj.argtypes = [vp, i32]
     L.hb_step_nve.argtypes = [vp, dbl]
     L.hb_run_nve.argtypes = [vp, dbl, i64, i64]
+    L.hb_run_nvt.argtypes = [vp, dbl, i64, i64, dbl, dbl]
+    L.hb_run_langevin.argtypes = [vp, dbl, i64, i64, dbl, dbl, C.c_uint64]
+    L.hb_get_thermostat.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
+    L.hb_set_thermostat.argtypes = [vp, dbl, dbl, i64]
     L.hb_sort.argtypes = [vp]
     L.hb_thermo.argtypes = [vp, C.POINTER(hb_thermo_t)]
     L.hb_get_cells.argtypes = [vp, vp, vp, vp, i32]
@@ -253,6 +258,20 @@ class System:
 
     def run_nve(self, dt, nsteps, sort_period=0):
         self._ck(self._lib.hb_run_nve(self._h, float(dt), int(nsteps), int(sort_period)))
+
+    def run_nvt(self, dt, nsteps, T, tau, sort_period=0):
+        self._ck(self._lib.hb_run_nvt(self._h, float(dt), int(nsteps), int(sort_period), float(T), float(tau)))
+
+    def run_langevin(self, dt, nsteps, T, gamma, seed, sort_period=0):
+        self._ck(self._lib.hb_run_langevin(self._h, float(dt), int(nsteps), int(sort_period), float(T), float(gamma), int(seed)))
+
+    def get_thermostat(self):
+        xi, eta, n = C.c_double(), C.c_double(), C.c_int64()
+        self._ck(self._lib.hb_get_thermostat(self._h, C.byref(xi), C.byref(eta), C.byref(n)))
+        return dict(xi=xi.value, eta=eta.value, langevin_steps=n.value)
+
+    def set_thermostat(self, xi=0.0, eta=0.0, langevin_steps=0):
+        self._ck(self._lib.hb_set_thermostat(self._h, float(xi), float(eta), int(langevin_steps)))
 
     def sort(self):
         self._ck(self._lib.hb_sort(self._h))

@@ -281,10 +281,74 @@ void orc_lj_pair_xplor(double r, double eps, double sigma, double r_cut, double 
     *minus_dVdr_over_r = flj * S - Vlj * dS_over_r;
 }
 
-/* one entry point for the three modes of the force sums: 0 = plain, 1 = energy shift, 2 = XPLOR */
-static inline void pair_by_mode(double r, double eps, double sigma, double r_cut, double r_on, int mode,
+/* NEXT-3: other pair potentials through the same sums.  The paper names them (Gaussian; Yukawa and
+ * Morse) and describes the mechanism -- a functor that returns V(r) and -(1/r) dV/dr --
+ * but prints no formula; [reading f1] the textbook forms, with the per-type-pair tables `eps`, `sigma` and `p2`
+ * reused as the potential's parameters:
+ *   pot 0  Lennard-Jones   V = 4 eps [(sigma/r)^12 - (sigma/r)^6]
+ *   pot 1  Gaussian        V = eps exp(-r^2 / (2 sigma^2))           -dV/dr = V r / sigma^2
+ *   pot 2  Yukawa          V = eps exp(-kappa r) / r, kappa = sigma   -dV/dr = V (kappa + 1/r)
+ *   pot 3  Morse           V = D0 [e^{-2 a (r - r0)} - 2 e^{-a (r - r0)}], D0 = eps, a = sigma, r0 = p2
+ *                          -dV/dr = 2 a D0 [e^{-2 a (r - r0)} - e^{-a (r - r0)}]
+ * Unshifted value and -(1/r) dV/dr at r (no cutoff applied here). */
+void orc_pair_bare(int pot, double r, double eps, double sigma, double p2, double *V, double *minus_dVdr_over_r)
+{
+    if (pot == 1) {
+        *V = eps * exp(-0.5 * (r / sigma) * (r / sigma));
+        *minus_dVdr_over_r = *V / (sigma * sigma);
+    } else if (pot == 2) {
+        *V = eps * exp(-sigma * r) / r;
+        *minus_dVdr_over_r = *V * (sigma + 1.0 / r) / r;
+    } else if (pot == 3) {
+        const double e1 = exp(-sigma * (r - p2));
+        *V = eps * (e1 * e1 - 2.0 * e1);
+        *minus_dVdr_over_r = 2.0 * sigma * eps * (e1 * e1 - e1) / r;
+    } else {
+        const double sr = sigma / r;
+        const double sr6 = sr * sr * sr * sr * sr * sr;
+        *V = 4.0 * eps * (sr6 * sr6 - sr6);
+        *minus_dVdr_over_r = (48.0 * eps * sr6 * sr6 - 24.0 * eps * sr6) / (r * r);
+    }
+}
+
+/* Any potential with the three cutoff treatments the paper describes for "every pair force":
+ * mode 0 truncated, 1 energy-shifted V - V(r_cut), 2 XPLOR-smoothed V S(r). */
+void orc_pair_generic(int pot, double r, double eps, double sigma, double p2, double r_cut, double r_on, int mode,
+                      double *V, double *minus_dVdr_over_r)
+{
+    if (!(r < r_cut)) { *V = 0.0; *minus_dVdr_over_r = 0.0; return; }
+    double v, f;
+    orc_pair_bare(pot, r, eps, sigma, p2, &v, &f);
+    if (mode == 1) {
+        double vc, fc;
+        orc_pair_bare(pot, r_cut, eps, sigma, p2, &vc, &fc);
+        v -= vc;
+    } else if (mode == 2 && r >= r_on && r_on < r_cut) {
+        const double rc2 = r_cut * r_cut, ron2 = r_on * r_on, r2 = r * r;
+        const double D = (rc2 - ron2) * (rc2 - ron2) * (rc2 - ron2);
+        const double S = (rc2 - r2) * (rc2 - r2) * (rc2 + 2.0 * r2 - 3.0 * ron2) / D;
+        const double dS_over_r = 12.0 * (rc2 - r2) * (ron2 - r2) / D;
+        f = f * S - v * dS_over_r;
+        v = v * S;
+    }
+    *V = v;
+    *minus_dVdr_over_r = f;
+}
+
+/* The third per-type-pair table (Morse r0) of the force sums below; [ntypes*ntypes], copied.  NULL: zeros. */
+static double g_p2[64 * 64];
+void orc_set_p2(const double *p2, int n)
+{
+    for (int k = 0; k < 64 * 64; k++) g_p2[k] = (p2 && k < n) ? p2[k] : 0.0;
+}
+
+/* one entry point for the force sums.  `shift` carries the cutoff treatment in its two low bits (0 = plain,
+ * 1 = energy shift, 2 = XPLOR) and the potential above them (shift >> 2: 0 LJ, 1 Gaussian, 2 Yukawa, 3 Morse). */
+static inline void pair_by_mode(double r, double eps, double sigma, double p2, double r_cut, double r_on, int shift,
                                 double *V, double *fdivr)
 {
+    const int mode = shift & 3, pot = shift >> 2;
+    if (pot != 0) { orc_pair_generic(pot, r, eps, sigma, p2, r_cut, r_on, mode, V, fdivr); return; }
     if (mode == 2) orc_lj_pair_xplor(r, eps, sigma, r_cut, r_on, V, fdivr);
     else orc_lj_pair(r, eps, sigma, r_cut, mode, V, fdivr);
 }
@@ -292,13 +356,13 @@ static inline void pair_by_mode(double r, double eps, double sigma, double r_cut
 /* ------------------------------------------------------------------ c6 ---- */
 /* One pair's contribution to particle i:  F_i += f, U_i += V/2,
  * W_i^{ab} += (1/2) d^a f^b  with d = minimage(R_i - R_j), f = [-(1/r)dV/dr] d. */
-static inline void add_pair(const double d[3], double r2, double eps, double sigma, double r_cut, double r_on,
+static inline void add_pair(const double d[3], double r2, double eps, double sigma, double p2, double r_cut, double r_on,
                             int shift, double *F, double *U, double *W,
                             double band, double *allow)
 {
     const double r = sqrt(r2);
     double V, fdivr;
-    pair_by_mode(r, eps, sigma, r_cut, r_on, shift, &V, &fdivr);
+    pair_by_mode(r, eps, sigma, p2, r_cut, r_on, shift, &V, &fdivr);
     const double f[3] = { fdivr * d[0], fdivr * d[1], fdivr * d[2] };
     F[0] += f[0]; F[1] += f[1]; F[2] += f[2];
     *U += 0.5 * V;
@@ -312,7 +376,7 @@ static inline void add_pair(const double d[3], double r2, double eps, double sig
     if (allow && fabs(r - r_cut) <= band) {
         const double rc = nextafter(r_cut, 0.0);
         double Vc, fc;
-        pair_by_mode(rc, eps, sigma, r_cut, r_on, shift, &Vc, &fc);
+        pair_by_mode(rc, eps, sigma, p2, r_cut, r_on, shift, &Vc, &fc);
         allow[0] += fabs(fc) * rc;
         allow[1] += 0.5 * fabs(Vc);
         allow[2] += 0.5 * fabs(fc) * rc * rc;
@@ -332,7 +396,7 @@ int orc_compute_lj_brute(const double *pos, const int32_t *type, int64_t N, doub
             double d[3];
             const double r2 = dist2(pos, i, j, L, d);
             const int p = type[i] * ntypes + type[j];
-            if (r2 < rcut[p] * rcut[p]) add_pair(d, r2, eps[p], sigma[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, 0.0, NULL);
+            if (r2 < rcut[p] * rcut[p]) add_pair(d, r2, eps[p], sigma[p], g_p2[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, 0.0, NULL);
         }
         memcpy(F + 3 * i, Fi, sizeof Fi); U[i] = Ui; memcpy(W + 6 * i, Wi, sizeof Wi);
     }
@@ -355,7 +419,7 @@ int orc_compute_lj_brute_sample(const double *pos, const int32_t *type, int64_t 
             const double r2 = dist2(pos, i, j, L, d);
             const int p = type[i] * ntypes + type[j];
             const double rc = rcut[p] + band;
-            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, band, al);
+            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], g_p2[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, band, al);
         }
         memcpy(F + 3 * k, Fi, sizeof Fi); U[k] = Ui; memcpy(W + 6 * k, Wi, sizeof Wi);
         if (allow) memcpy(allow + 3 * k, al, sizeof al);
@@ -382,7 +446,7 @@ int orc_compute_lj_nlist(const double *pos, const int32_t *type, int64_t N, doub
             /* add_pair() itself applies r < r_cut; pairs just outside are
              * visited only so that their allowance is recorded. */
             const double rc = rcut[p] + band;
-            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, band, al);
+            if (r2 < rc * rc) add_pair(d, r2, eps[p], sigma[p], g_p2[p], rcut[p], ron ? ron[p] : rcut[p], shift, Fi, &Ui, Wi, band, al);
         }
         memcpy(F + 3 * i, Fi, sizeof Fi); U[i] = Ui; memcpy(W + 6 * i, Wi, sizeof Wi);
         if (allow) memcpy(allow + 3 * i, al, sizeof al);

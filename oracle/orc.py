@@ -50,6 +50,8 @@ def lib():
         L.orc_max_disp2.argtypes = [_dp, _dp, C.c_int64, C.c_double]
         L.orc_lj_pair.argtypes = [C.c_double] * 4 + [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_lj_pair_xplor.argtypes = [C.c_double] * 5 + [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_pair_generic.argtypes = [C.c_int] + [C.c_double] * 6 + [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_set_p2.argtypes = [_vp, C.c_int]
         L.orc_compute_lj_brute.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
         L.orc_compute_lj_brute_sample.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int,
                                                   _lp, C.c_int64, C.c_double, _dp, _dp, _dp, _vp]
@@ -92,13 +94,24 @@ def _check(rc, what):
 class Params:
     """Per-type-pair tables as fp64 arrays (values already fp32-representable)."""
 
-    def __init__(self, ntypes, eps, sigma, rcut, shift, ron=None):
-        """shift: 0 plain, 1 energy shift, 2 XPLOR smoothing (needs ron per type pair)."""
+    POTS = {"lj": 0, "gauss": 1, "yukawa": 2, "morse": 3}
+
+    def __init__(self, ntypes, eps, sigma, rcut, shift, ron=None, pot="lj", p2=None):
+        """shift: 0 plain, 1 energy shift, 2 XPLOR smoothing (needs ron per type pair).  pot: the potential whose
+        parameters the eps / sigma / p2 tables hold (see orc_pair_bare)."""
         self.ntypes = int(ntypes)
         self.eps, self.sigma, self.rcut = _d(eps).ravel(), _d(sigma).ravel(), _d(rcut).ravel()
         self.ron = self.rcut.copy() if ron is None else _d(ron).ravel()
-        self.shift = int(shift)
-        assert self.eps.size == self.sigma.size == self.rcut.size == self.ron.size == self.ntypes ** 2
+        self.p2 = np.zeros_like(self.eps) if p2 is None else _d(p2).ravel()
+        self.mode, self.pot = int(shift), self.POTS[pot]
+        assert self.eps.size == self.sigma.size == self.rcut.size == self.ron.size == self.p2.size == self.ntypes ** 2
+
+    @property
+    def shift(self):
+        """What the C sums take: cutoff treatment in the low two bits, the potential above them; the p2 table goes
+        in through orc_set_p2 every time the value is read for a call."""
+        lib().orc_set_p2(_ptr(self.p2), self.p2.size)
+        return self.mode + 4 * self.pot
 
     @classmethod
     def of(cls, w):
@@ -172,6 +185,13 @@ def max_disp2(pos, pos_build, L):
 def lj_pair(r, eps, sigma, r_cut, shift):
     V, f = C.c_double(), C.c_double()
     lib().orc_lj_pair(float(r), float(eps), float(sigma), float(r_cut), int(shift), C.byref(V), C.byref(f))
+    return V.value, f.value
+
+
+def pair_generic(pot, r, eps, sigma, p2, r_cut, r_on, mode):
+    V, f = C.c_double(), C.c_double()
+    lib().orc_pair_generic(Params.POTS[pot], float(r), float(eps), float(sigma), float(p2), float(r_cut), float(r_on), int(mode),
+                           C.byref(V), C.byref(f))
     return V.value, f.value
 
 

@@ -454,6 +454,12 @@ int orc_compute_lj_nlist(const double *pos, const int32_t *type, int64_t N, doub
     return ORC_OK;
 }
 
+/* NEXT-3: per-particle mass ("HOOMD version 0.8.1 allows a mass ... to be specified for each
+ * particle"; the base path has m = 1, reading c7).  The table is test-infrastructure state: orc_set_mass(m, N)
+ * before a call, orc_set_mass(NULL, 0) for m = 1, in which case every expression below is the m = 1 one. */
+static const double *g_mass = NULL;
+void orc_set_mass(const double *mass, int64_t N) { (void)N; g_mass = mass; }
+
 /* ------------------------------------------------------------------ c7 ---- */
 /* Velocity Verlet, first half ([reading c7] m = 1):
  *   v' = v + (dt/2) F(t);  x(t+dt) = x + dt v';
@@ -461,7 +467,8 @@ int orc_compute_lj_nlist(const double *pos, const int32_t *type, int64_t N, doub
 void orc_nve_step1(double *pos, double *vel, const double *F, int32_t *image, int64_t N, double L, double dt)
 {
     for (int64_t k = 0; k < 3 * N; k++) {
-        vel[k] = vel[k] + 0.5 * dt * F[k];
+        if (g_mass) vel[k] = vel[k] + 0.5 * dt * F[k] / g_mass[k / 3];
+        else vel[k] = vel[k] + 0.5 * dt * F[k];
         double x = pos[k] + dt * vel[k];
         if (x >= 0.5 * L) { x -= L; image[k] += 1; }
         else if (x < -0.5 * L) { x += L; image[k] -= 1; }
@@ -472,6 +479,7 @@ void orc_nve_step1(double *pos, double *vel, const double *F, int32_t *image, in
 /* second half: v(t+dt) = v' + (dt/2) F(t+dt). */
 void orc_nve_step2(double *vel, const double *F, int64_t N, double dt)
 {
+    if (g_mass) { for (int64_t k = 0; k < 3 * N; k++) vel[k] = vel[k] + 0.5 * dt * F[k] / g_mass[k / 3]; return; }
     for (int64_t k = 0; k < 3 * N; k++) vel[k] = vel[k] + 0.5 * dt * F[k];
 }
 
@@ -482,9 +490,10 @@ void orc_thermo(const double *vel, const double *U, const double *W, int64_t N, 
 {
     memset(out, 0, 12 * sizeof(double));
     for (int64_t i = 0; i < N; i++) {
+        const double mi = g_mass ? g_mass[i] : 1.0;
         for (int a = 0; a < 3; a++) {
-            out[0] += 0.5 * vel[3 * i + a] * vel[3 * i + a];
-            out[9 + a] += vel[3 * i + a];
+            out[0] += 0.5 * mi * vel[3 * i + a] * vel[3 * i + a];
+            out[9 + a] += mi * vel[3 * i + a];
         }
         out[1] += U[i];
         for (int a = 0; a < 6; a++) out[2 + a] += W[6 * i + a];
@@ -622,7 +631,7 @@ int orc_run_nve(double *pos, double *vel, int32_t *image, const int32_t *type, i
         if (step > 0) orc_nve_step2(vel, F, N, dt);
         if (log_KU) {
             double K = 0.0, Ut = 0.0;
-            for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * vel[k] * vel[k];
+            for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * (g_mass ? g_mass[k / 3] : 1.0) * vel[k] * vel[k];
             for (int64_t i = 0; i < N; i++) Ut += U[i];
             log_KU[2 * step] = K; log_KU[2 * step + 1] = Ut;
         }
@@ -711,14 +720,14 @@ int orc_run_thermostat(int mode, double *pos, double *vel, int32_t *image, const
             if (mode == 1) {
                 /* [n1] first half: friction implicit, drift, wrap */
                 for (int64_t k = 0; k < 3 * N; k++) {
-                    vel[k] = (vel[k] + 0.5 * dt * F[k]) / (1.0 + 0.5 * dt * xi);
+                    vel[k] = (vel[k] + 0.5 * dt * F[k] / (g_mass ? g_mass[k / 3] : 1.0)) / (1.0 + 0.5 * dt * xi);
                     double x = pos[k] + dt * vel[k];
                     if (x >= 0.5 * L) { x -= L; image[k] += 1; }
                     else if (x < -0.5 * L) { x += L; image[k] -= 1; }
                     pos[k] = x;
                 }
                 double K = 0.0;
-                for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * vel[k] * vel[k];
+                for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * (g_mass ? g_mass[k / 3] : 1.0) * vel[k] * vel[k];
                 const double xi_new = xi + dt / (par * par) * ((2.0 * K / g) / T - 1.0);
                 eta += 0.5 * dt * (xi + xi_new);
                 xi = xi_new;
@@ -755,17 +764,22 @@ int orc_run_thermostat(int mode, double *pos, double *vel, int32_t *image, const
         }
         if (step > 0) {
             if (mode == 1) {
-                for (int64_t k = 0; k < 3 * N; k++) vel[k] = vel[k] + 0.5 * dt * (F[k] - xi * vel[k]);   /* [n1] second half */
+                for (int64_t k = 0; k < 3 * N; k++)                                                          /* [n1] second half */
+                    vel[k] = vel[k] + 0.5 * dt * (F[k] / (g_mass ? g_mass[k / 3] : 1.0) - xi * vel[k]);
             } else {
                 orc_nve_step2(vel, F, N, dt);
                 const double c = 1.0 - par * dt, sgm = sqrt(6.0 * par * T * dt);                        /* [n2] */
+                if (g_mass) {                                /* friction and noise are forces: both divided by m */
+                    for (int64_t k = 0; k < 3 * N; k++)
+                        vel[k] = vel[k] * (1.0 - par * dt / g_mass[k / 3]) + sgm / g_mass[k / 3] * orc_uniform_pm1(seed, tstep, (uint64_t)k);
+                } else
                 for (int64_t k = 0; k < 3 * N; k++) vel[k] = vel[k] * c + sgm * orc_uniform_pm1(seed, tstep, (uint64_t)k);
                 tstep++;
             }
         }
         if (log) {
             double K = 0.0, Ut = 0.0;
-            for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * vel[k] * vel[k];
+            for (int64_t k = 0; k < 3 * N; k++) K += 0.5 * (g_mass ? g_mass[k / 3] : 1.0) * vel[k] * vel[k];
             for (int64_t i = 0; i < N; i++) Ut += U[i];
             log[4 * step] = K; log[4 * step + 1] = Ut; log[4 * step + 2] = xi; log[4 * step + 3] = eta;
         }

@@ -52,6 +52,7 @@ def lib():
         L.orc_lj_pair_xplor.argtypes = [C.c_double] * 5 + [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_pair_generic.argtypes = [C.c_int] + [C.c_double] * 6 + [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_set_p2.argtypes = [_vp, C.c_int]
+        L.orc_set_mass.argtypes = [_vp, C.c_int64]
         L.orc_compute_lj_brute.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp]
         L.orc_compute_lj_brute_sample.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _dp, _dp, _dp, C.c_int,
                                                   _lp, C.c_int64, C.c_double, _dp, _dp, _dp, _vp]
@@ -233,6 +234,19 @@ def compute_lj_nlist(pos, typ, L, p: Params, count, row_start, nbr, band=0.0):
     return F, U, W, A
 
 
+class _Mass:
+    """with _Mass(mass): ... -- the per-particle masses of the integrator calls inside (None: m = 1)."""
+
+    def __init__(self, mass):
+        self.m = None if mass is None else _d(mass).copy()
+
+    def __enter__(self):
+        lib().orc_set_mass(_ptr(self.m), 0 if self.m is None else len(self.m))
+
+    def __exit__(self, *a):
+        lib().orc_set_mass(None, 0)
+
+
 def nve_step1(pos, vel, F, image, L, dt):
     """In place on float64 pos/vel and int32 image."""
     lib().orc_nve_step1(pos, vel, _d(F), image, len(pos), float(L), float(dt))
@@ -245,9 +259,10 @@ def nve_step2(vel, F, dt):
 THERMO_FIELDS = ("K", "U", "Wxx", "Wxy", "Wxz", "Wyy", "Wyz", "Wzz", "P", "px", "py", "pz")
 
 
-def thermo(vel, U, W, L):
+def thermo(vel, U, W, L, mass=None):
     out = np.empty(12)
-    lib().orc_thermo(_d(vel), _d(U), _d(W), len(vel), float(L), out)
+    with _Mass(mass):
+        lib().orc_thermo(_d(vel), _d(U), _d(W), len(vel), float(L), out)
     return dict(zip(THERMO_FIELDS, out))
 
 
@@ -269,7 +284,7 @@ def sort_perm(key, B=8):
     return perm
 
 
-def run_nve(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, forces=None, log=False):
+def run_nve(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, forces=None, log=False, mass=None):
     """Whole loop; returns dict(pos, vel, image, F, U, W, KU, builds, max_nbrs)."""
     pos, vel = _d(pos).copy(), _d(vel).copy()
     image = np.ascontiguousarray(image, dtype=np.int32).copy()
@@ -282,8 +297,9 @@ def run_nve(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, forces=None,
         have = 1
     KU = np.zeros((nsteps + 1, 2)) if log else None
     stats = np.zeros(2, dtype=np.int64)
-    _check(lib().orc_run_nve(pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
-                             float(r_buff), float(dt), int(nsteps), have, F, U, W, _ptr(KU), _ptr(stats)), "run_nve")
+    with _Mass(mass):
+        _check(lib().orc_run_nve(pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
+                                 float(r_buff), float(dt), int(nsteps), have, F, U, W, _ptr(KU), _ptr(stats)), "run_nve")
     return dict(pos=pos, vel=vel, image=image, F=F, U=U, W=W, KU=KU, builds=int(stats[0]), max_nbrs=int(stats[1]))
 
 
@@ -295,7 +311,7 @@ def uniform_pm1(seed, stream, index):
     return lib().orc_uniform_pm1(int(seed), int(stream), int(index))
 
 
-def _run_thermostat(mode, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, par, seed, state, forces, log):
+def _run_thermostat(mode, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, par, seed, state, forces, log, mass=None):
     pos, vel = _d(pos).copy(), _d(vel).copy()
     image = np.ascontiguousarray(image, dtype=np.int32).copy()
     typ = np.ascontiguousarray(typ, dtype=np.int32)
@@ -308,20 +324,21 @@ def _run_thermostat(mode, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, par
     lg = np.zeros((nsteps + 1, 4)) if log else None
     stats = np.zeros(2, dtype=np.int64)
     st = np.array(state, dtype=np.float64)
-    _check(lib().orc_run_thermostat(mode, pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
-                                    float(r_buff), float(dt), int(nsteps), float(T), float(par), int(seed), st, have,
-                                    F, U, W, _ptr(lg), _ptr(stats)), "run_thermostat")
+    with _Mass(mass):
+        _check(lib().orc_run_thermostat(mode, pos, vel, image, typ, N, float(L), p.ntypes, p.eps, p.sigma, p.rcut, p.ron, p.shift,
+                                        float(r_buff), float(dt), int(nsteps), float(T), float(par), int(seed), st, have,
+                                        F, U, W, _ptr(lg), _ptr(stats)), "run_thermostat")
     return dict(pos=pos, vel=vel, image=image, F=F, U=U, W=W, log=lg, state=st, builds=int(stats[0]))
 
 
-def run_nvt(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, T, tau, xi=0.0, eta=0.0, forces=None, log=False):
+def run_nvt(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, T, tau, xi=0.0, eta=0.0, forces=None, log=False, mass=None):
     """Nose-Hoover (reading n1); returns dict(pos, vel, image, F, U, W, log[K, U, xi, eta], state=[xi, eta])."""
-    return _run_thermostat(1, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, tau, 0, [xi, eta], forces, log)
+    return _run_thermostat(1, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, tau, 0, [xi, eta], forces, log, mass)
 
 
-def run_langevin(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, T, gamma, seed, step0=0, forces=None, log=False):
+def run_langevin(pos, vel, image, typ, L, p: Params, r_buff, dt, nsteps, T, gamma, seed, step0=0, forces=None, log=False, mass=None):
     """Langevin (reading n2); state[0] = number of the next time step."""
-    return _run_thermostat(2, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, gamma, seed, [float(step0), 0.0], forces, log)
+    return _run_thermostat(2, pos, vel, image, typ, L, p, r_buff, dt, nsteps, T, gamma, seed, [float(step0), 0.0], forces, log, mass)
 
 
 def num_threads():

@@ -61,6 +61,18 @@ extern "C" {
 #define HB_XPLOR 2        /* V = V_lj(r) S(r): XPLOR smoothing from r_on to r_cut, V and dV/dr -> 0 at r_cut
                              (PAPER.md:355-367); r_on per type pair from hb_set_ron_pair */
 
+/* Pair potentials through the same kernel (a functor that returns V(r) and -(1/r) dV/dr; the paper names
+ * Gaussian, Yukawa and Morse, and prints no formula: reading f1 of DESIGN.md, the textbook
+ * forms).  The eps / sigma tables of hb_create and the p2 table of hb_set_pair_potential hold the parameters:
+ *   HB_POT_LJ      V = 4 eps [(sigma/r)^12 - (sigma/r)^6]
+ *   HB_POT_GAUSS   V = eps exp(-r^2 / (2 sigma^2))
+ *   HB_POT_YUKAWA  V = eps exp(-kappa r) / r,                       kappa = sigma
+ *   HB_POT_MORSE   V = D0 [e^{-2 a (r - r0)} - 2 e^{-a (r - r0)}],   D0 = eps, a = sigma, r0 = p2 */
+#define HB_POT_LJ 0
+#define HB_POT_GAUSS 1
+#define HB_POT_YUKAWA 2
+#define HB_POT_MORSE 3
+
 typedef struct hb_system hb_system;
 
 /* Optional device allocator (e.g. PyTorch's caching allocator).  alloc returns
@@ -71,8 +83,8 @@ typedef struct hb_allocator {
     void *user;
 } hb_allocator;
 
-/* Thermodynamic sums: K = 1/2 sum v^2 (m = 1), U = sum U_i,
- * W = sum W_i, P = (2K + tr W) / (3 L^3), p = sum v. */
+/* Thermodynamic sums: K = 1/2 sum m v^2, U = sum U_i,
+ * W = sum W_i, P = (2K + tr W) / (3 L^3), p = sum m v  (m = 1 unless hb_set_mass was called). */
 typedef struct hb_thermo_t {
     double K, U, W[6], P, px, py, pz;
 } hb_thermo_t;
@@ -118,6 +130,17 @@ HB_API int hb_set_rcut_pair(hb_system *h, const double *rcut);
  * hb_compute_lj(HB_XPLOR).  Default: 3/2 sigma_ab, the paper's test value.  r_on,ab >= r_cut,ab
  * leaves no switching interval: that pair is plainly truncated (reading x1). */
 HB_API int hb_set_ron_pair(hb_system *h, const double *ron);
+
+/* The pair potential evaluated by hb_compute_lj and the integrators (default HB_POT_LJ), with any of the three cutoff
+ * treatments (HB_SHIFT_NONE, HB_SHIFT_ENERGY, HB_XPLOR).  p2 [ntypes*ntypes], symmetric: the third parameter table
+ * (Morse r0); NULL = zeros.  Forces become stale. */
+HB_API int hb_set_pair_potential(hb_system *h, int pot, const double *p2);
+
+/* Per-particle masses, mass [N] BY TAG, all > 0; they enter the velocity updates (v += dt/2 F/m), the
+ * thermostats (readings n1, n2: friction and noise are forces) and hb_thermo.  hb_set_state resets every mass to 1.
+ * hb_get_mass downloads them by tag. */
+HB_API int hb_set_mass(hb_system *h, const float *mass, int on_device);
+HB_API int hb_get_mass(hb_system *h, float *mass, int on_device);
 
 /* Algorithm 2: bin the particles into m^3 cells, m = floor(L / r_max), with
  * c = floor((x - b) m / L) per axis evaluated in binary32 without contraction

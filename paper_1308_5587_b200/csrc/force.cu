@@ -99,40 +99,74 @@ struct Acc {
 
 // One listed pair.  pj is already the nearest image.  The force sums are the same operations in both variants
 // (fma(f/r, d, F)), so the trajectory does not depend on whether the energy and virial terms are compiled in.
-// XPLOR: V = V_lj S(r), -(1/r) dV/dr = [-(1/r) dV_lj/dr] S - V_lj S'/r with
-//   S = (rc^2 - r^2)^2 (rc^2 + 2 r^2 - 3 ron^2) / (rc^2 - ron^2)^3,  S'/r = 12 (rc^2 - r^2)(ron^2 - r^2) / (rc^2 - ron^2)^3
-// between r_on and r_cut, S = 1 below r_on.
-template <bool THERMO, bool XPLOR>
+// FN selects the functor (V(r) and -(1/r) dV/dr):
+//   FN_LJ     Lennard-Jones, truncated or energy-shifted
+//   FN_XPLOR  Lennard-Jones with XPLOR smoothing: V = V_lj S(r),
+//             -(1/r) dV/dr = [-(1/r) dV_lj/dr] S - V_lj S'/r with
+//             S = (rc^2 - r^2)^2 (rc^2 + 2 r^2 - 3 ron^2) / (rc^2 - ron^2)^3,  S'/r = 12 (rc^2 - r^2)(ron^2 - r^2) / (rc^2 - ron^2)^3
+//             between r_on and r_cut, S = 1 below r_on
+//   FN_GEN    Gaussian, Yukawa or Morse (reading f1; `pot` is uniform over the launch) with any of the three cutoff
+//             treatments: eshift = V(r_cut) or 0, smoothing where invD != 0.
+enum { FN_LJ = 0, FN_XPLOR = 1, FN_GEN = 2 };
+
+template <bool THERMO, int FN>
 __device__ __forceinline__ void pair_term(const float4 &pi, const float4 &pj, const float lj1x12, const float lj2x6,
-                                          const float rcut2, const float lj1, const float lj2, const float eshift,
-                                          const float ron2, const float invD, Acc &a)
+                                          const PairParam &pp, const PairParamX &px, const int pot, Acc &a)
 {
     const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-    const bool in = r2 < rcut2;                        // strict <
-    const float r2inv = in ? rcp_approx(r2) : 0.0f;    // 0 switches the whole pair off: no branch (a branch per pair
-    const float r4inv = r2inv * r2inv;                 // would serialise the EPL pairs of an iteration)
-    const float r6inv = r4inv * r2inv;
-    float fdivr = (r4inv * r4inv) * __fmaf_rn(lj1x12, r6inv, -lj2x6);
-    float v = 0.f;
-    if (THERMO || XPLOR) v = r6inv * __fmaf_rn(lj1, r6inv, -lj2);
-    if (XPLOR) {
-        const float r2c = fminf(r2, rcut2);            // the dummy slot is 1e18 away: keep (rc^2 - r^2)^2 finite
-        const float d = rcut2 - r2c;
-        const bool sw = r2c > ron2;
-        const float S = sw ? d * d * __fmaf_rn(2.0f, r2c, __fmaf_rn(-3.0f, ron2, rcut2)) * invD : 1.0f;
-        const float dS = sw ? 12.0f * d * (ron2 - r2c) * invD : 0.0f;
-        fdivr = __fmaf_rn(fdivr, S, -v * dS);
-        v *= S;
+    const bool in = r2 < pp.rcut2;                     // strict <
+    float fdivr, v = 0.f;
+    if (FN == FN_GEN) {
+        const float r2s = in ? r2 : pp.rcut2;          // the dummy slot is 1e18 away: keep every intermediate finite
+        float f;
+        if (pot == HB_POT_GAUSS) {
+            v = pp.lj1 * expf(-r2s * pp.lj2);
+            f = v * (2.0f * pp.lj2);
+        } else if (pot == HB_POT_YUKAWA) {
+            const float r = sqrtf(r2s), ri = 1.0f / r;
+            v = pp.lj1 * expf(-pp.lj2 * r) * ri;
+            f = v * (pp.lj2 + ri) * ri;
+        } else {
+            const float r = sqrtf(r2s);
+            const float e1 = expf(-pp.lj2 * (r - px.p2));
+            v = pp.lj1 * (e1 * e1 - 2.0f * e1);
+            f = 2.0f * pp.lj2 * pp.lj1 * (e1 * e1 - e1) / r;
+        }
+        if (px.invD != 0.0f && r2s > px.ron2) {
+            const float d = pp.rcut2 - r2s;
+            const float S = d * d * __fmaf_rn(2.0f, r2s, __fmaf_rn(-3.0f, px.ron2, pp.rcut2)) * px.invD;
+            const float dS = 12.0f * d * (px.ron2 - r2s) * px.invD;
+            f = __fmaf_rn(f, S, -v * dS);
+            v *= S;
+        }
+        fdivr = in ? f : 0.0f;
+        v = in ? v - pp.eshift : 0.0f;
+    } else {
+        const float r2inv = in ? rcp_approx(r2) : 0.0f;    // 0 switches the whole pair off: no branch (a branch per pair
+        const float r4inv = r2inv * r2inv;                 // would serialise the EPL pairs of an iteration)
+        const float r6inv = r4inv * r2inv;
+        fdivr = (r4inv * r4inv) * __fmaf_rn(lj1x12, r6inv, -lj2x6);
+        if (THERMO || FN == FN_XPLOR) v = r6inv * __fmaf_rn(pp.lj1, r6inv, -pp.lj2);
+        if (FN == FN_XPLOR) {
+            const float r2c = fminf(r2, pp.rcut2);         // the dummy slot is 1e18 away: keep (rc^2 - r^2)^2 finite
+            const float d = pp.rcut2 - r2c;
+            const bool sw = r2c > px.ron2;
+            const float S = sw ? d * d * __fmaf_rn(2.0f, r2c, __fmaf_rn(-3.0f, px.ron2, pp.rcut2)) * px.invD : 1.0f;
+            const float dS = sw ? 12.0f * d * (px.ron2 - r2c) * px.invD : 0.0f;
+            fdivr = __fmaf_rn(fdivr, S, -v * dS);
+            v *= S;
+        }
+        if (THERMO) v -= in ? pp.eshift : 0.0f;
     }
     a.fx = __fmaf_rn(fdivr, dx, a.fx);
     a.fy = __fmaf_rn(fdivr, dy, a.fy);
     a.fz = __fmaf_rn(fdivr, dz, a.fz);
     if (THERMO) {
-        a.u += v - (in ? eshift : 0.0f);
-        const float px = fdivr * dx, py = fdivr * dy, pz = fdivr * dz;
-        a.wxx = __fmaf_rn(dx, px, a.wxx); a.wxy = __fmaf_rn(dx, py, a.wxy); a.wxz = __fmaf_rn(dx, pz, a.wxz);
-        a.wyy = __fmaf_rn(dy, py, a.wyy); a.wyz = __fmaf_rn(dy, pz, a.wyz); a.wzz = __fmaf_rn(dz, pz, a.wzz);
+        a.u += v;
+        const float px_ = fdivr * dx, py_ = fdivr * dy, pz_ = fdivr * dz;
+        a.wxx = __fmaf_rn(dx, px_, a.wxx); a.wxy = __fmaf_rn(dx, py_, a.wxy); a.wxz = __fmaf_rn(dx, pz_, a.wxz);
+        a.wyy = __fmaf_rn(dy, py_, a.wyy); a.wyz = __fmaf_rn(dy, pz_, a.wyz); a.wzz = __fmaf_rn(dz, pz_, a.wzz);
     }
 }
 
@@ -157,7 +191,7 @@ struct ForceArgs {
     const int *cell_start;
     const float4 *pos;
     const uint16_t *nlist;
-    int pitch, N, ntypes;
+    int pitch, N, ntypes, pot;
     const PairParam *params;
     const PairParamX *paramsx;
     float4 *force, *virial;
@@ -253,7 +287,7 @@ __device__ __forceinline__ bool force_tile_tables(const TileGeom &g, const int *
     return s.d.nslots <= g.cap;
 }
 
-template <int TPP, int EPL, bool ONE_TYPE, bool THERMO, bool SCALED, bool XPLOR>
+template <int TPP, int EPL, bool ONE_TYPE, bool THERMO, bool SCALED, int FN>
 __global__ void __launch_bounds__(TILE_THREADS, 4)   // <= 64 registers: 8 blocks of 128 threads per SM
 lj_tile_kernel(const ForceArgs A)
 {
@@ -271,7 +305,7 @@ lj_tile_kernel(const ForceArgs A)
     unsigned char *sp = smem_raw;
     float4 *stage = reinterpret_cast<float4 *>(sp);                      sp += (size_t)g.cap * 16;
     PairParam *s_params = reinterpret_cast<PairParam *>(sp);             sp += ONE_TYPE ? 0 : ((A.ntypes * A.ntypes * sizeof(PairParam) + 15) & ~(size_t)15);
-    PairParamX *s_paramsx = reinterpret_cast<PairParamX *>(sp);          sp += (ONE_TYPE || !XPLOR) ? 0 : ((A.ntypes * A.ntypes * sizeof(PairParamX) + 15) & ~(size_t)15);
+    PairParamX *s_paramsx = reinterpret_cast<PairParamX *>(sp);          sp += (ONE_TYPE || FN == FN_LJ) ? 0 : ((A.ntypes * A.ntypes * sizeof(PairParamX) + 15) & ~(size_t)15);
     EntryVec *ring = reinterpret_cast<EntryVec *>(sp) + threadIdx.x;     sp += (size_t)PF * sizeof(EntryVec) * nthreads;
     float4 *own = reinterpret_cast<float4 *>(sp);                        sp += (size_t)3 * PPB * 16;       // [v | x | x_build][PPB]
     TileShared &sgen = *reinterpret_cast<TileShared *>(sp);              // the general (small-box) geometry only
@@ -284,7 +318,7 @@ lj_tile_kernel(const ForceArgs A)
     if (!ONE_TYPE)
         for (int k = threadIdx.x; k < A.ntypes * A.ntypes; k += nthreads) {
             s_params[k] = A.params[k];
-            if (XPLOR) s_paramsx[k] = A.paramsx[k];
+            if (FN != FN_LJ) s_paramsx[k] = A.paramsx[k];
         }
     if (drift && block0 && threadIdx.x == 0) A.flags[nv.need_clear] = 0;
 
@@ -358,8 +392,8 @@ lj_tile_kernel(const ForceArgs A)
     }
 
     const PairParam pp1 = A.params[0];
-    PairParamX px1 = {0.f, 0.f};
-    if (XPLOR) px1 = A.paramsx[0];
+    PairParamX px1 = {0.f, 0.f, 0.f, 0.f};
+    if (FN != FN_LJ) px1 = A.paramsx[0];
     const float c12 = 12.0f * pp1.lj1, c6 = 6.0f * pp1.lj2;
     const float hdt = 0.5f * nv.dt, hL = 0.5f * g.L, L = g.L;
     const unsigned char *stage_b = reinterpret_cast<const unsigned char *>(stage);
@@ -373,7 +407,7 @@ lj_tile_kernel(const ForceArgs A)
         const float4 pi = stage[slot_n];         // slot 0 (the dummy) for idle thread groups
         const uint16_t *row = A.nlist + (int64_t)gi * A.pitch + sub * EPL;
         const PairParam *prow = ONE_TYPE ? nullptr : s_params + __float_as_int(pi.w) * A.ntypes;
-        const PairParamX *prowx = (ONE_TYPE || !XPLOR) ? nullptr : s_paramsx + __float_as_int(pi.w) * A.ntypes;
+        const PairParamX *prowx = (ONE_TYPE || FN == FN_LJ) ? nullptr : s_paramsx + __float_as_int(pi.w) * A.ntypes;
         Acc a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
         if (active) {
@@ -400,14 +434,13 @@ lj_tile_kernel(const ForceArgs A)
 #pragma unroll
                 for (int e = 0; e < EPL; e++) {
                     if (ONE_TYPE) {
-                        pair_term<THERMO, XPLOR>(pi, pj[e], c12, c6, pp1.rcut2, pp1.lj1, pp1.lj2, pp1.eshift, px1.ron2, px1.invD, a);
+                        pair_term<THERMO, FN>(pi, pj[e], c12, c6, pp1, px1, A.pot, a);
                     } else {
                         const int tj = __float_as_int(pj[e].w);
                         const PairParam pp = prow[tj];
-                        PairParamX px = {0.f, 0.f};
-                        if (XPLOR) px = prowx[tj];
-                        pair_term<THERMO, XPLOR>(pi, pj[e], 12.0f * pp.lj1, 6.0f * pp.lj2, pp.rcut2, pp.lj1, pp.lj2, pp.eshift, px.ron2,
-                                                 px.invD, a);
+                        PairParamX px = {0.f, 0.f, 0.f, 0.f};
+                        if (FN != FN_LJ) px = prowx[tj];
+                        pair_term<THERMO, FN>(pi, pj[e], 12.0f * pp.lj1, 6.0f * pp.lj2, pp, px, A.pot, a);
                     }
                 }
             }
@@ -447,7 +480,7 @@ lj_tile_kernel(const ForceArgs A)
         if (nv.kick_prev) thermo_kick_prev(nv, xi, hdt, a.fx, a.fy, a.fz, v, nv.ens == 2 ? nv.tag[gi] : 0u);
         if (nv.kick_drift) {
             thermo_kick_first(nv, xi, hdt, a.fx, a.fy, a.fz, v);
-            if (nv.ens == 1) ksum += 0.5 * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+            if (nv.ens == 1) ksum += 0.5 * (double)v.w * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
             // p is the stored position: the staged one may be another periodic image of it
             p.x = __fmaf_rn(nv.dt, v.x, p.x);
             p.y = __fmaf_rn(nv.dt, v.y, p.y);
@@ -483,7 +516,7 @@ size_t force_smem_bytes(const hb_system *h)
            (size_t)4 * 16 * force_block_of(h) + (size_t)3 * 16 * force_ppb(h) + (h->geom.fast ? 0 : sizeof(TileShared));
 }
 
-template <int TPP, int EPL, bool THERMO, bool SCALED, bool XPLOR>
+template <int TPP, int EPL, bool THERMO, bool SCALED, int FN>
 static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
 {
     const size_t smem = force_smem_bytes(h);
@@ -496,6 +529,7 @@ static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
     A.pitch = h->row_pitch;
     A.N = (int)h->N;
     A.ntypes = h->ntypes;
+    A.pot = h->pot;
     A.params = h->params;
     A.paramsx = h->paramsx;
     A.force = h->force;
@@ -505,35 +539,37 @@ static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
     if (nve) A.nv = *nve;
     cudaError_t e;
 #define LJ_LAUNCH(ONE)                                                                                                      \
-    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, XPLOR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, FN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
     if (e != cudaSuccess) return e;                                                                                         \
-    lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, XPLOR><<<grid, force_block_of(h), smem, h->stream>>>(A);
+    lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, FN><<<grid, force_block_of(h), smem, h->stream>>>(A);
     if (h->ntypes == 1) { LJ_LAUNCH(true) } else { LJ_LAUNCH(false) }
 #undef LJ_LAUNCH
     h->stats.kernel_launches++;
     return cudaGetLastError();
 }
 
-template <int TPP, int EPL, bool XPLOR>
+template <int TPP, int EPL, int FN>
 static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
 {
     // energies and virials of a step can only be read after hb_run_nve returns: with thermo_every = 0 the inner
     // steps of a chunk (both half kicks fused in) compute forces only
     const bool thermo = !(nve && nve->forces_only);
     const bool scaled = h->geom.eshift == 4;
-    if (thermo) return scaled ? launch_force_tts<TPP, EPL, true, true, XPLOR>(h, nve) : launch_force_tts<TPP, EPL, true, false, XPLOR>(h, nve);
-    return scaled ? launch_force_tts<TPP, EPL, false, true, XPLOR>(h, nve) : launch_force_tts<TPP, EPL, false, false, XPLOR>(h, nve);
+    if (thermo) return scaled ? launch_force_tts<TPP, EPL, true, true, FN>(h, nve) : launch_force_tts<TPP, EPL, true, false, FN>(h, nve);
+    return scaled ? launch_force_tts<TPP, EPL, false, true, FN>(h, nve) : launch_force_tts<TPP, EPL, false, false, FN>(h, nve);
 }
 
 cudaError_t launch_force(hb_system *h, const NveArgs *nve)
 {
-    // the smoothed functor comes in the default thread layout only (tpp 2, epl 8); the tunables apply to plain / shifted LJ
-    if (h->shift_mode == HB_XPLOR) return launch_force_t<2, 8, true>(h, nve);
+    // the smoothed and the generic functors come in the default thread layout only (tpp 2, epl 8); the tunables apply
+    // to plain / shifted LJ
+    if (h->pot != HB_POT_LJ) return launch_force_t<2, 8, FN_GEN>(h, nve);
+    if (h->shift_mode == HB_XPLOR) return launch_force_t<2, 8, FN_XPLOR>(h, nve);
     const int epl = h->tun.epl == 8 ? 8 : 4;
     switch (h->tun.tpp) {
-        case 2: return epl == 8 ? launch_force_t<2, 8, false>(h, nve) : launch_force_t<2, 4, false>(h, nve);
-        case 8: return launch_force_t<8, 4, false>(h, nve);   // 8 x 8 entries would read past the 32-entry row padding
-        default: return epl == 8 ? launch_force_t<4, 8, false>(h, nve) : launch_force_t<4, 4, false>(h, nve);
+        case 2: return epl == 8 ? launch_force_t<2, 8, FN_LJ>(h, nve) : launch_force_t<2, 4, FN_LJ>(h, nve);
+        case 8: return launch_force_t<8, 4, FN_LJ>(h, nve);   // 8 x 8 entries would read past the 32-entry row padding
+        default: return epl == 8 ? launch_force_t<4, 8, FN_LJ>(h, nve) : launch_force_t<4, 4, FN_LJ>(h, nve);
     }
 }
 

@@ -62,6 +62,17 @@ void destroy_graphs(hb_system *h)
     h->graphs.clear();
 }
 
+// Unshifted V(r) of the chosen potential in binary64 (for the energy shift V(r_cut)); reading f1.
+double pair_energy(int pot, double r, double e, double s, double p2)
+{
+    switch (pot) {
+        case HB_POT_GAUSS: return e * std::exp(-0.5 * (r / s) * (r / s));
+        case HB_POT_YUKAWA: return e * std::exp(-s * r) / r;
+        case HB_POT_MORSE: { const double e1 = std::exp(-s * (r - p2)); return e * (e1 * e1 - 2.0 * e1); }
+        default: { const double sr6 = std::pow(s / r, 6.0); return 4.0 * e * (sr6 * sr6 - sr6); }
+    }
+}
+
 // Per-type-pair device table from eps, sigma, r_cut (binary64 -> rounded once).
 int upload_params(hb_system *h)
 {
@@ -70,17 +81,26 @@ int upload_params(hb_system *h)
     h->h_paramsx.resize(nt2);
     double rc_max = 0.0;
     for (int p = 0; p < nt2; p++) {
-        const double e = h->eps[p], s = h->sigma[p], rc = h->rcut[p];
-        const double s6 = std::pow(s, 6.0);
+        const double e = h->eps[p], s = h->sigma[p], rc = h->rcut[p], p2 = h->p2[p];
         PairParam pp;
-        pp.lj1 = (float)(4.0 * e * s6 * s6);
-        pp.lj2 = (float)(4.0 * e * s6);
+        if (h->pot == HB_POT_LJ) {
+            const double s6 = std::pow(s, 6.0);
+            pp.lj1 = (float)(4.0 * e * s6 * s6);
+            pp.lj2 = (float)(4.0 * e * s6);
+        } else if (h->pot == HB_POT_GAUSS) {
+            pp.lj1 = (float)e;
+            pp.lj2 = (float)(0.5 / (s * s));
+        } else {
+            pp.lj1 = (float)e;      // Yukawa: eps, kappa; Morse: D0, a
+            pp.lj2 = (float)s;
+        }
         pp.rcut2 = (float)(rc * rc);
-        const double sr6 = s6 / std::pow(rc, 6.0);
-        pp.eshift = h->shift_mode == HB_SHIFT_ENERGY ? (float)(4.0 * e * (sr6 * sr6 - sr6)) : 0.0f;
+        pp.eshift = h->shift_mode == HB_SHIFT_ENERGY ? (float)pair_energy(h->pot, rc, e, s, p2) : 0.0f;
         h->h_params[p] = pp;
         const double ron = h->ron[p], d = rc * rc - ron * ron;
-        h->h_paramsx[p] = PairParamX{(float)(ron * ron), ron < rc ? (float)(1.0 / (d * d * d)) : 0.0f};
+        // the smoothing is on where invD != 0: in HB_XPLOR mode and only where r_on < r_cut (reading x1)
+        const bool smooth = h->shift_mode == HB_XPLOR && ron < rc;
+        h->h_paramsx[p] = PairParamX{(float)(ron * ron), smooth ? (float)(1.0 / (d * d * d)) : 0.0f, (float)p2, 0.0f};
         if (rc > rc_max) rc_max = rc;
     }
     h->r_cut_max = (float)rc_max;
@@ -761,6 +781,7 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     for (int p = 0; p < ntypes * ntypes; p++) h->rcut[p] = (double)(float)(2.5 * sigma[p]);
     h->ron.resize(ntypes * ntypes);
     for (int p = 0; p < ntypes * ntypes; p++) h->ron[p] = (double)(float)(1.5 * sigma[p]);
+    h->p2.assign((size_t)ntypes * ntypes, 0.0);
     h->stream = (cudaStream_t)cuda_stream;
     if (alloc && alloc->alloc && alloc->free) { h->alloc = *alloc; h->has_alloc = true; }
     *out = h;  // from here on the caller can read hb_last_error and must hb_destroy
@@ -929,6 +950,60 @@ int hb_set_ron_pair(hb_system *h, const double *ron)
     for (int p = 0; p < nt * nt; p++) h->ron[p] = (double)(float)ron[p];
     h->forces_valid = false;
     return upload_params(h);
+}
+
+int hb_set_pair_potential(hb_system *h, int pot, const double *p2)
+{
+    HB_NEED(h);
+    if (pot < HB_POT_LJ || pot > HB_POT_MORSE) { h->err = "unknown pair potential"; return HB_EINVAL; }
+    const int nt = h->ntypes;
+    if (p2)
+        for (int a = 0; a < nt; a++)
+            for (int b = 0; b < nt; b++)
+                if (p2[a * nt + b] != p2[b * nt + a]) { h->err = "p2 table must be symmetric"; return HB_EINVAL; }
+    for (int p = 0; p < nt * nt; p++) h->p2[p] = p2 ? (double)(float)p2[p] : 0.0;
+    h->pot = pot;
+    h->forces_valid = false;
+    destroy_graphs(h);          // the captured step kernels are instantiated for one pair functor
+    if (h->m > 0) HB_TRY(choose_tiles(h, 0));   // the functor decides the block size and with it the shared-memory budget
+    return upload_params(h);
+}
+
+int hb_set_mass(hb_system *h, const float *mass, int on_device)
+{
+    HB_NEED(h);
+    if (!mass) { h->err = "mass is NULL"; return HB_EINVAL; }
+    if (!h->have_state) { h->err = "no state: call hb_set_state first (it resets the masses to 1)"; return HB_ESTATE; }
+    const size_t N = (size_t)h->N;
+    const float *d = mass;
+    if (!on_device) {
+        HB_TRY(ensure_stage(h, N * 4));
+        HB_CK(cudaMemcpyAsync(h->acc_stage, mass, N * 4, cudaMemcpyHostToDevice, h->stream));
+        d = (const float *)h->acc_stage;
+    }
+    HB_CK(launch_mass(h, d, nullptr));
+    HB_TRY(read_flags(h));
+    if (h->h_flags[FL_BADTYPE]) {
+        HB_TRY(set_flag(h, FL_BADTYPE, 0));
+        h->err = "masses must be positive and finite (some were not; the others have been set)";
+        return HB_EINVAL;
+    }
+    h->bk_valid = false;
+    return HB_OK;
+}
+
+int hb_get_mass(hb_system *h, float *mass, int on_device)
+{
+    HB_NEED(h);
+    if (!mass) { h->err = "mass is NULL"; return HB_EINVAL; }
+    if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    const size_t N = (size_t)h->N;
+    if (on_device) { HB_CK(launch_mass(h, nullptr, mass)); return HB_OK; }
+    HB_TRY(ensure_stage(h, N * 4));
+    HB_CK(launch_mass(h, nullptr, (float *)h->acc_stage));
+    HB_CK(cudaMemcpyAsync(mass, h->acc_stage, N * 4, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    return HB_OK;
 }
 
 int hb_build_cells(hb_system *h)

@@ -31,15 +31,17 @@ enum {
 };
 
 struct PairParam {  // one per type pair, 16 B
-    float lj1;      // 4 eps sigma^12
-    float lj2;      // 4 eps sigma^6
+    float lj1;      // LJ: 4 eps sigma^12 | Gauss: eps            | Yukawa: eps   | Morse: D0
+    float lj2;      // LJ: 4 eps sigma^6  | Gauss: 1/(2 sigma^2)  | Yukawa: kappa | Morse: a
     float rcut2;    // r_cut^2
-    float eshift;   // V_lj(r_cut) if energy shift, else 0
+    float eshift;   // V(r_cut) if energy shift, else 0
 };
 
-struct PairParamX {  // XPLOR smoothing, one per type pair, 8 B
+struct PairParamX {  // XPLOR smoothing and the third parameter, one per type pair, 16 B
     float ron2;     // r_on^2
     float invD;     // 1 / (r_cut^2 - r_on^2)^3, 0 where r_on >= r_cut (no switching interval)
+    float p2;       // Morse: r0
+    float pad;
 };
 
 // A tile is a brick of tx x ty x tz cells (clipped at the upper faces of the box).  One
@@ -97,8 +99,9 @@ struct hb_system {
     int ntypes = 1;
     float L = 0, r_cut_max = 0, r_buff = 0, r_max = 0;
     int shift_mode = HB_SHIFT_ENERGY;
+    int pot = HB_POT_LJ;     // pair potential (hb_set_pair_potential)
     bool rcut_user = false;  // hb_set_rcut_pair was called
-    std::vector<double> eps, sigma, rcut, ron;
+    std::vector<double> eps, sigma, rcut, ron, p2;
     std::vector<PairParam> h_params;
     std::vector<PairParamX> h_paramsx;
     cudaStream_t stream = nullptr;
@@ -110,7 +113,7 @@ struct hb_system {
     // particle data (storage order), SoA of 16 B vectors
     float4 *posbuf[2] = {nullptr, nullptr};  // x, y, z, type bits; posbuf[cur] is current (the fused step ping-pongs)
     int cur = 0;
-    float4 *vel = nullptr;      // vx, vy, vz, unused
+    float4 *vel = nullptr;      // vx, vy, vz, mass (1 unless hb_set_mass)
     float4 *force = nullptr;    // Fx, Fy, Fz, U_i
     float4 *virial = nullptr;   // [2N]: (xx, xy, xz, yy), (yz, zz, 0, 0)
     int *image = nullptr;       // [3][N]
@@ -210,7 +213,7 @@ struct hb_system {
 static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // threads per particle of the step kernel actually launched (the smoothed functor exists in the default layout only)
-static inline int force_tpp(const hb_system *h) { return h->shift_mode == HB_XPLOR ? 2 : h->tun.tpp; }
+static inline int force_tpp(const hb_system *h) { return (h->shift_mode == HB_XPLOR || h->pot != HB_POT_LJ) ? 2 : h->tun.tpp; }
 
 static inline int force_block_of(const hb_system *h)
 {
@@ -271,6 +274,7 @@ int measure_peak(hb_system *h, const char *which, double *value);
 cudaError_t launch_pack_state(hb_system *h, const float *pos_xyz, const int32_t *type, const float *vel_xyz, const int32_t *image);
 cudaError_t launch_unpack_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image);
 cudaError_t launch_unpack_forces(hb_system *h, float *f4, float *vir6);
+cudaError_t launch_mass(hb_system *h, const float *mass_in, float *mass_out);   // by tag: set (mass_in) or get (mass_out)
 cudaError_t launch_nlist_counts_by_tag(hb_system *h, int *counts);
 cudaError_t launch_nlist_fill_by_tag(hb_system *h, const int64_t *row_start, uint32_t *out);
 cudaError_t launch_nlist_rows_by_tag(hb_system *h, const int *counts, int64_t *rows);   // exclusive scan, rows[N] = total

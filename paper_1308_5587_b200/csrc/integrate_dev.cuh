@@ -1,11 +1,13 @@
 // The per-particle velocity updates of the three integration methods and the end-of-drift bookkeeping, shared by
 // the stand-alone integrator kernel (nve.cu) and the fused step kernel (force.cu).
-//   NVE          v += (dt/2) F                                                   (reading c7)
-//   Nose-Hoover  first half  v' = (v + (dt/2) F) / (1 + (dt/2) xi)
-//                second half v  = v' + (dt/2) (F - xi v')                         (reading n1)
-//                after every drift the LAST block to finish advances xi and eta from sum v'^2
-//   Langevin     NVE, and after the second half kick v = v (1 - gamma dt) + sqrt(6 gamma T dt) u,
+//   NVE          v += (dt/2) F / m                                               (reading c7)
+//   Nose-Hoover  first half  v' = (v + (dt/2) F / m) / (1 + (dt/2) xi)
+//                second half v  = v' + (dt/2) (F / m - xi v')                     (reading n1)
+//                after every drift the LAST block to finish advances xi and eta from sum m v'^2
+//   Langevin     NVE, and after the second half kick v = v (1 - gamma dt / m) + sqrt(6 gamma T dt) / m u,
 //                u = counter-based uniform in (-1, 1) of (seed, time step, 3 tag + component)   (reading n2)
+// The mass is v.w (1 unless hb_set_mass was called); F / m is formed as F * (1 / m) with 1 / m = __frcp_rn(m), which
+// leaves every operation of the m = 1 path bit for bit what it was (F * 1 = F).
 #pragma once
 #include "hb_internal.cuh"
 
@@ -35,6 +37,8 @@ __device__ __forceinline__ unsigned long long hb_seed_stream(unsigned long long 
 // second half kick of a step (v is v'), with what the method adds to it
 __device__ __forceinline__ void thermo_kick_prev(const NveArgs &nv, float xi, float hdt, float fx, float fy, float fz, float4 &v, unsigned tag)
 {
+    const float im = __frcp_rn(v.w);
+    fx *= im; fy *= im; fz *= im;
     if (nv.ens == 1) {
         v.x = __fmaf_rn(hdt, __fmaf_rn(-xi, v.x, fx), v.x);
         v.y = __fmaf_rn(hdt, __fmaf_rn(-xi, v.y, fy), v.y);
@@ -45,7 +49,7 @@ __device__ __forceinline__ void thermo_kick_prev(const NveArgs &nv, float xi, fl
     v.y = __fmaf_rn(hdt, fy, v.y);
     v.z = __fmaf_rn(hdt, fz, v.z);
     if (nv.ens == 2) {
-        const float c = 1.0f - nv.par * nv.dt, sg = sqrtf(6.0f * nv.par * nv.T * nv.dt);
+        const float c = 1.0f - (nv.par * nv.dt) * im, sg = sqrtf(6.0f * nv.par * nv.T * nv.dt) * im;
         const unsigned long long step = (unsigned long long)(*reinterpret_cast<const long long *>(nv.tstate + TS_LBASE)) + (unsigned long long)nv.kick_step;
         const unsigned long long ss = hb_seed_stream(nv.seed, step);
         v.x = __fmaf_rn(sg, hb_uniform_pm1(ss, 3ULL * tag + 0ULL), v.x * c);
@@ -57,9 +61,10 @@ __device__ __forceinline__ void thermo_kick_prev(const NveArgs &nv, float xi, fl
 // first half kick of a step
 __device__ __forceinline__ void thermo_kick_first(const NveArgs &nv, float xi, float hdt, float fx, float fy, float fz, float4 &v)
 {
-    v.x = __fmaf_rn(hdt, fx, v.x);
-    v.y = __fmaf_rn(hdt, fy, v.y);
-    v.z = __fmaf_rn(hdt, fz, v.z);
+    const float im = __frcp_rn(v.w);
+    v.x = __fmaf_rn(hdt, fx * im, v.x);
+    v.y = __fmaf_rn(hdt, fy * im, v.y);
+    v.z = __fmaf_rn(hdt, fz * im, v.z);
     if (nv.ens == 1) {
         const float den = __fmaf_rn(hdt, xi, 1.0f);
         v.x = __fdiv_rn(v.x, den); v.y = __fdiv_rn(v.y, den); v.z = __fdiv_rn(v.z, den);
@@ -68,7 +73,7 @@ __device__ __forceinline__ void thermo_kick_first(const NveArgs &nv, float xi, f
 
 // After a drift: Nose-Hoover's kinetic-energy sum, and the work of the last block to finish: advance the thermostat
 // (every block read xi when it started, so nobody sees the new value before the next kernel) and hand the rebuild
-// decision to a conditional graph node if there is one.  ksum: this thread's v'^2 / 2.
+// decision to a conditional graph node if there is one.  ksum: this thread's m v'^2 / 2.
 __device__ __forceinline__ void step_epilogue(const NveArgs &nv, int *__restrict__ flags, double ksum, unsigned nblocks)
 {
     if (nv.ens == 1) {

@@ -26,7 +26,7 @@ nve_kernel(float4 *pos, const float4 *__restrict__ force, int N, float L, int *_
         if (nv.kick_prev) thermo_kick_prev(nv, xi, hdt, f.x, f.y, f.z, v, nv.ens == 2 ? nv.tag[i] : 0u);
         if (nv.kick_drift) {
             thermo_kick_first(nv, xi, hdt, f.x, f.y, f.z, v);
-            if (nv.ens == 1) ksum = 0.5 * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+            if (nv.ens == 1) ksum = 0.5 * (double)v.w * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
             float4 p = pos[i];
             p.x = __fmaf_rn(dt, v.x, p.x);
             p.y = __fmaf_rn(dt, v.y, p.y);
@@ -100,10 +100,11 @@ thermo_partial_kernel(const float4 *__restrict__ vel, const float4 *__restrict__
         const float4 v = vel[i];
         const float4 f = force[i];
         const float4 w0 = virial[2 * (int64_t)i], w1 = virial[2 * (int64_t)i + 1];
-        a[0] += 0.5 * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+        const double m = (double)v.w;
+        a[0] += 0.5 * m * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
         a[1] += f.w;
         a[2] += w0.x; a[3] += w0.y; a[4] += w0.z; a[5] += w0.w; a[6] += w1.x; a[7] += w1.y;
-        a[8] += v.x; a[9] += v.y; a[10] += v.z;
+        a[8] += m * v.x; a[9] += m * v.y; a[10] += m * v.z;
     }
     __shared__ double sm[TH_THREADS / 32][TH_VALS];
 #pragma unroll
@@ -150,7 +151,7 @@ __global__ void pack_state_kernel(const float *__restrict__ pos_xyz, const int32
     if (t < 0 || t >= ntypes) { flags[FL_BADTYPE] = 1; t = 0; }   // the force kernel indexes its pair table with it
     pos[i] = make_float4(pos_xyz[3 * (int64_t)i], pos_xyz[3 * (int64_t)i + 1], pos_xyz[3 * (int64_t)i + 2],
                          __int_as_float(t));
-    vel[i] = make_float4(vel_xyz[3 * (int64_t)i], vel_xyz[3 * (int64_t)i + 1], vel_xyz[3 * (int64_t)i + 2], 0.f);
+    vel[i] = make_float4(vel_xyz[3 * (int64_t)i], vel_xyz[3 * (int64_t)i + 1], vel_xyz[3 * (int64_t)i + 2], 1.0f);   // .w = mass
     for (int a = 0; a < 3; a++) image[(int64_t)a * N + i] = image_in ? image_in[3 * (int64_t)i + a] : 0;
     tag[i] = i;
     rtag[i] = i;
@@ -183,5 +184,26 @@ cudaError_t launch_unpack_state(hb_system *h, float *pos_xyz, int32_t *type, flo
 {
     unpack_state_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->pos(), h->vel, h->image, h->tag, (int)h->N, pos_xyz,
                                                                           type, vel_xyz, image);
+    return cudaGetLastError();
+}
+
+// per-particle mass lives in vel.w; the accessors go by tag
+__global__ void mass_kernel(float4 *__restrict__ vel, const uint32_t *__restrict__ tag, int N, const float *__restrict__ mass_in,
+                            float *__restrict__ mass_out, int *__restrict__ flags)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const uint32_t t = tag[i];
+    if (mass_in) {
+        const float m = mass_in[t];
+        if (!(m > 0.f) || !(m < 3.0e38f)) flags[FL_BADTYPE] = 1;
+        else vel[i].w = m;
+    }
+    if (mass_out) mass_out[t] = vel[i].w;
+}
+
+cudaError_t launch_mass(hb_system *h, const float *mass_in, float *mass_out)
+{
+    mass_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->vel, h->tag, (int)h->N, mass_in, mass_out, h->flags);
     return cudaGetLastError();
 }

@@ -20,9 +20,12 @@ LIB_PATH = os.path.join(_HERE, "libhb.so")
 
 HB_OK, HB_EINVAL, HB_ECUDA, HB_ENOMEM, HB_EBOX, HB_ESTATE, HB_ENAN = 0, -1, -2, -3, -4, -5, -6
 HB_SHIFT_NONE, HB_SHIFT_ENERGY, HB_XPLOR = 0, 1, 2
+HB_POT_LJ, HB_POT_GAUSS, HB_POT_YUKAWA, HB_POT_MORSE = 0, 1, 2, 3
+POTS = {"lj": HB_POT_LJ, "gauss": HB_POT_GAUSS, "yukawa": HB_POT_YUKAWA, "morse": HB_POT_MORSE}
 _ERR_NAMES = {-1: "HB_EINVAL", -2: "HB_ECUDA", -3: "HB_ENOMEM", -4: "HB_EBOX", -5: "HB_ESTATE", -6: "HB_ENAN"}
 
-EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_set_ron_pair", "hb_build_cells",
+EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_set_ron_pair",
+           "hb_set_pair_potential", "hb_set_mass", "hb_get_mass", "hb_build_cells",
            "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_run_nvt", "hb_run_langevin",
            "hb_get_thermostat", "hb_set_thermostat", "hb_sort",
            "hb_thermo", "hb_get_cells", "hb_get_nlist", "hb_get_forces", "hb_stats", "hb_set_tunable",
@@ -70,6 +73,9 @@ def load():
     L.hb_get_state.argtypes = [vp, vp, vp, vp, vp, vp, i32]
     L.hb_set_rcut_pair.argtypes = [vp, vp]
     L.hb_set_ron_pair.argtypes = [vp, vp]
+    L.hb_set_pair_potential.argtypes = [vp, i32, vp]
+    L.hb_set_mass.argtypes = [vp, vp, i32]
+    L.hb_get_mass.argtypes = [vp, vp, i32]
     L.hb_build_cells.argtypes = [vp]
     L.hb_build_nlist.argtypes = [vp, dbl, dbl]
     L.hb_needs_rebuild.argtypes = [vp, C.POINTER(i32)]
@@ -238,6 +244,26 @@ class System:
         if ron.size != self.ntypes ** 2:
             raise ValueError("ron must have ntypes*ntypes entries")
         self._ck(self._lib.hb_set_ron_pair(self._h, ron.ctypes.data_as(C.c_void_p)))
+
+    def set_pair_potential(self, pot, p2=None):
+        """pot: HB_POT_* or one of "lj", "gauss", "yukawa", "morse"; p2: third parameter table (Morse r0)."""
+        pot = POTS[pot] if isinstance(pot, str) else int(pot)
+        ptr = None
+        if p2 is not None:
+            p2 = np.ascontiguousarray(p2, dtype=np.float64).ravel()
+            if p2.size != self.ntypes ** 2:
+                raise ValueError("p2 must have ntypes*ntypes entries")
+            ptr = p2.ctypes.data_as(C.c_void_p)
+        self._ck(self._lib.hb_set_pair_potential(self._h, pot, ptr))
+
+    def set_mass(self, mass):
+        m, d = _ptr(mass, np.float32)
+        self._ck(self._lib.hb_set_mass(self._h, m, d))
+
+    def get_mass(self):
+        m = np.empty(self.N, np.float32)
+        self._ck(self._lib.hb_get_mass(self._h, m.ctypes.data_as(C.c_void_p), 0))
+        return m
 
     def build_cells(self):
         self._ck(self._lib.hb_build_cells(self._h))

@@ -174,15 +174,15 @@ template <int EPL> struct Entries;
 template <> struct Entries<4> { uint2 v; };
 template <> struct Entries<8> { uint4 v; };
 
-// byte offsets of the EPL gathers of one iteration (entries are (slot << 2) | two membership bits, tile.cuh)
-template <int EPL>
+// byte offsets of the EPL gathers of one iteration
+template <int EPL, bool SCALED>
 __device__ __forceinline__ void unpack_entries(const Entries<EPL> &e, unsigned (&off)[EPL])
 {
     const unsigned w[4] = {e.v.x, e.v.y, EPL == 8 ? ((const unsigned *)&e.v)[2] : 0u, EPL == 8 ? ((const unsigned *)&e.v)[3] : 0u};
 #pragma unroll
     for (int k = 0; k < EPL / 2; k++) {
-        off[2 * k] = (w[k] & 0xfffcu) << 2;
-        off[2 * k + 1] = (w[k] >> 14) & 0x3fff0u;
+        if (SCALED) { off[2 * k] = w[k] & 0xffffu; off[2 * k + 1] = w[k] >> 16; }
+        else { off[2 * k] = (w[k] & 0xffffu) << 4; off[2 * k + 1] = (w[k] >> 16) << 4; }
     }
 }
 
@@ -191,7 +191,7 @@ struct ForceArgs {
     const int *cell_start;
     const float4 *pos;
     const uint16_t *nlist;
-    int pitch, N, ntypes, pot, dbg;
+    int pitch, N, ntypes, pot;
     const PairParam *params;
     const PairParamX *paramsx;
     float4 *force, *virial;
@@ -267,15 +267,10 @@ __device__ __forceinline__ bool force_tile_tables(const TileGeom &g, const int *
         s.d.own_slot[tid] += s.piece_slot[2 * ((lz + 1) * t.hy + (ly + 1))];
     }
     if (tid == 0) {
-        int run = 0, prun = 0;
+        int run = 0;
         const int nrows = t.ey * t.ez;
         s.d.own_off[0] = 0;
-        s.d.pair_off[0] = 0;
-        for (int r = 0; r < nrows; r++) {
-            const int n = s.d.own_off[r + 1];
-            s.d.own_off[r + 1] = run + n; run += n;
-            prun += (n + 1) >> 1; s.d.pair_off[r + 1] = prun;
-        }
+        for (int r = 0; r < nrows; r++) { const int n = s.d.own_off[r + 1]; s.d.own_off[r + 1] = run + n; run += n; }
         const float wcell = g.L / (float)m, hL = 0.5f * g.L;
         s.d.nslots = s.piece_slot[np];
         s.d.nown = run;
@@ -292,33 +287,32 @@ __device__ __forceinline__ bool force_tile_tables(const TileGeom &g, const int *
     return s.d.nslots <= g.cap;
 }
 
-template <int TPP, int EPL, bool ONE_TYPE, bool THERMO, int FN>
-__global__ void __launch_bounds__(TILE_THREADS, THERMO ? 3 : 4)   // forces only: <= 64 registers, 8 blocks of 128 threads per SM; with U_i, W_i: 80
+template <int TPP, int EPL, bool ONE_TYPE, bool THERMO, bool SCALED, int FN>
+__global__ void __launch_bounds__(TILE_THREADS, 4)   // <= 64 registers: 8 blocks of 128 threads per SM
 lj_tile_kernel(const ForceArgs A)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ ForceTile s;
     const TileGeom &g = A.g;
     const int nthreads = blockDim.x;
-    const int PPB = nthreads / TPP;              // PAIRS of particles per block per pass (one thread group each)
-    constexpr int G = TPP * EPL;                 // entries per pair row per iteration
+    const int PPB = nthreads / TPP;              // particles per block per pass
+    constexpr int G = TPP * EPL;                 // entries per particle per iteration
     constexpr int PF = 4;                        // depth of the ring of list copies
     using EntryVec = decltype(Entries<EPL>::v);
 
-    // dynamic shared memory: staging area | pair table | ring | own data of a pass (v, x, x_build of 2 PPB particles;
-    // one buffer: a thread reads its particle's data into registers before it starts the copies of the next pass)
+    // dynamic shared memory: staging area | pair table | ring | own data of a pass (v, x, x_build; one buffer: a
+    // thread group reads its particle's data into registers before it starts the copies of the next pass)
     unsigned char *sp = smem_raw;
     float4 *stage = reinterpret_cast<float4 *>(sp);                      sp += (size_t)g.cap * 16;
     PairParam *s_params = reinterpret_cast<PairParam *>(sp);             sp += ONE_TYPE ? 0 : ((A.ntypes * A.ntypes * sizeof(PairParam) + 15) & ~(size_t)15);
     PairParamX *s_paramsx = reinterpret_cast<PairParamX *>(sp);          sp += (ONE_TYPE || FN == FN_LJ) ? 0 : ((A.ntypes * A.ntypes * sizeof(PairParamX) + 15) & ~(size_t)15);
     EntryVec *ring = reinterpret_cast<EntryVec *>(sp) + threadIdx.x;     sp += (size_t)PF * sizeof(EntryVec) * nthreads;
-    float4 *own = reinterpret_cast<float4 *>(sp);                        sp += (size_t)3 * 2 * PPB * 16;   // [v | x | x_build][2 PPB]
+    float4 *own = reinterpret_cast<float4 *>(sp);                        sp += (size_t)3 * PPB * 16;       // [v | x | x_build][PPB]
     TileShared &sgen = *reinterpret_cast<TileShared *>(sp);              // the general (small-box) geometry only
     const int ring_stride = nthreads;
     const NveArgs &nv = A.nv;
     const bool nve = A.do_nve != 0, drift = nve && nv.kick_drift;
     const bool block0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
-    if (A.dbg & 4) return;
 
     if (threadIdx.x == 0 && g.fast) mbar_init(&s.mbar, 1);
     if (!ONE_TYPE)
@@ -349,31 +343,32 @@ lj_tile_kernel(const ForceArgs A)
         TileCtx t;
         tile_decode_xyz(g, blockIdx.x, blockIdx.y, blockIdx.z, t);
         fits = tile_tables(g, A.cell_start, t, sgen, A.flags);
-        for (int k = threadIdx.x; k < (int)(sizeof(TileDesc) / 4); k += nthreads) reinterpret_cast<int *>(&s.d)[k] = reinterpret_cast<const int *>(&sgen.d)[k];
+        if (threadIdx.x < sizeof(TileDesc) / 4) reinterpret_cast<int *>(&s.d)[threadIdx.x] = reinterpret_cast<const int *>(&sgen.d)[threadIdx.x];
         __syncthreads();
         if (fits) tile_stage_positions(g, t, sgen, A.pos, stage, nullptr);
     }
-    const int npairs = fits ? s.d.pair_off[s.d.nrows] : 0;
-    if (A.dbg & 2) return;
+    const int nown = fits ? s.d.nown : 0;
 
     const int sub = threadIdx.x % TPP;
-    const int ql = threadIdx.x / TPP;            // pair of the pass this thread group works for
-    int gi_n = 0, slot_n = 0, np_n = 0;
-    // start of a pass: the pair of this thread group, the first PF copies of its row, and (lanes 0 and 1 of the
-    // group, one particle each) what the integration will need
+    const int ql = threadIdx.x / TPP;            // particle of the pass this thread group works for
+    int gi_n = 0, slot_n = 0;
+    bool active_n = false;
+    // start of a pass: the particle of this thread group, the first PF copies of its row, and (lanes 0 and 1 of the
+    // group) what the integration of the particle will need
     auto prep = [&](int q0) {
-        const int P = q0 + ql;
-        gi_n = 0; slot_n = 0; np_n = 0;
-        if (P < npairs) tile_pair(s.d, P, gi_n, slot_n, np_n);
+        const int q = q0 + ql;
+        active_n = q < nown;
+        gi_n = 0; slot_n = 0;
+        if (active_n) tile_own(s.d, q, gi_n, slot_n);
         const uint16_t *row = A.nlist + (int64_t)gi_n * A.pitch + sub * EPL;
-        if (nve && sub < np_n) {
-            float4 *o = own + 2 * ql + sub;
-            cp_async_cg16(o, nv.vel + gi_n + sub);
-            if (nv.kick_drift) { cp_async_cg16(o + 2 * PPB, A.pos + gi_n + sub); cp_async_cg16(o + 4 * PPB, nv.pos_build + gi_n + sub); }
+        if (nve && active_n) {
+            float4 *o = own + ql;
+            if (sub == 0) { cp_async_cg16(o, nv.vel + gi_n); if (nv.kick_drift) cp_async_cg16(o + PPB, A.pos + gi_n); }
+            if (sub == 1 && nv.kick_drift) cp_async_cg16(o + 2 * PPB, nv.pos_build + gi_n);
         }
 #pragma unroll
         for (int u = 0; u < PF; u++) {
-            if (np_n) cp_async<EPL * 2>(ring + u * ring_stride, row + u * G);
+            if (active_n) cp_async<EPL * 2>(ring + u * ring_stride, row + u * G);
             cp_async_commit();
         }
     };
@@ -406,101 +401,80 @@ lj_tile_kernel(const ForceArgs A)
     double ksum = 0.0;
     const float xi = (nve && nv.ens == 1) ? (float)nv.tstate[TS_XI] : 0.f;   // read by every block before the last one updates it
 
-    for (int q0 = 0; q0 < npairs; q0 += PPB) {   // block-uniform trip count: the shuffles need whole warps
-        const int np = np_n;                     // particles of this group's pair: 2, 1 (last of a row) or 0 (idle group)
-        const int gi0 = gi_n;
-        const float4 pi0 = stage[slot_n];        // slot 0 (the dummy) for idle thread groups
-        const float4 pi1 = stage[np == 2 ? slot_n + 1 : 0];
-        const uint16_t *row = A.nlist + (int64_t)gi0 * A.pitch + sub * EPL;
-        const PairParam *prow0 = ONE_TYPE ? nullptr : s_params + __float_as_int(pi0.w) * A.ntypes;
-        const PairParam *prow1 = ONE_TYPE ? nullptr : s_params + __float_as_int(pi1.w) * A.ntypes;
-        const PairParamX *prowx0 = (ONE_TYPE || FN == FN_LJ) ? nullptr : s_paramsx + __float_as_int(pi0.w) * A.ntypes;
-        const PairParamX *prowx1 = (ONE_TYPE || FN == FN_LJ) ? nullptr : s_paramsx + __float_as_int(pi1.w) * A.ntypes;
-        Acc a0 = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, a1 = a0;
+    for (int q0 = 0; q0 < nown; q0 += PPB) {     // block-uniform trip count: the shuffles need whole warps
+        const bool active = active_n;
+        const int gi = gi_n;
+        const float4 pi = stage[slot_n];         // slot 0 (the dummy) for idle thread groups
+        const uint16_t *row = A.nlist + (int64_t)gi * A.pitch + sub * EPL;
+        const PairParam *prow = ONE_TYPE ? nullptr : s_params + __float_as_int(pi.w) * A.ntypes;
+        const PairParamX *prowx = (ONE_TYPE || FN == FN_LJ) ? nullptr : s_paramsx + __float_as_int(pi.w) * A.ntypes;
+        Acc a = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 
-        // one listed (or partner) particle against both particles of the pair
-        auto both = [&](const float4 &pj) {
-            if (ONE_TYPE) {
-                pair_term<THERMO, FN>(pi0, pj, c12, c6, pp1, px1, A.pot, a0);
-                pair_term<THERMO, FN>(pi1, pj, c12, c6, pp1, px1, A.pot, a1);
-            } else {
-                const int tj = __float_as_int(pj.w);
-                const PairParam p0 = prow0[tj], p1 = prow1[tj];
-                PairParamX x0 = {0.f, 0.f, 0.f, 0.f}, x1 = x0;
-                if (FN != FN_LJ) { x0 = prowx0[tj]; x1 = prowx1[tj]; }
-                pair_term<THERMO, FN>(pi0, pj, 12.0f * p0.lj1, 6.0f * p0.lj2, p0, x0, A.pot, a0);
-                pair_term<THERMO, FN>(pi1, pj, 12.0f * p1.lj1, 6.0f * p1.lj2, p1, x1, A.pot, a1);
-            }
-        };
-
-        if (np) {
+        if (active) {
             int c = 0;
-            const int kmax = (A.dbg & 1) ? 0 : np * A.pitch;       // a pair's row is the two rows of its particles
             cp_async_wait<PF - 1>();
             Entries<EPL> ent;
             ent.v = ring[0];
-            for (int k = 0; k < kmax; k += G) {
+            for (int k = 0; k < A.pitch; k += G) {
                 if ((ent.v.x & 0xffffu) == 0u) break;                    // padding: the row is over for this thread
                 cp_async<EPL * 2>(ring + c * ring_stride, row + k + PF * G);   // refill PF iterations ahead (reads past the
                 cp_async_commit();                                       // row's end are harmless: the array has slack)
                 c = (c + 1 == PF) ? 0 : c + 1;
                 unsigned off[EPL];
-                unpack_entries<EPL>(ent, off);
+                unpack_entries<EPL, SCALED>(ent, off);
+#ifdef HB_EXPERIMENT_BANKS   // timing experiment only (wrong physics): force the bank group of every gather to the conflict-free pattern
+#pragma unroll
+                for (int e = 0; e < EPL; e++) off[e] = (off[e] & ~0x70u) | ((unsigned)((ql + sub * EPL + e) & 7) << 4);
+#endif
                 float4 pj[EPL];
 #pragma unroll
                 for (int e = 0; e < EPL; e++) pj[e] = *reinterpret_cast<const float4 *>(stage_b + off[e]);
                 cp_async_wait<PF - 1>();                                 // the next group of entries, read before the
                 ent.v = ring[c * ring_stride];                           // arithmetic so that its latency hides behind it
 #pragma unroll
-                for (int e = 0; e < EPL; e++) both(pj[e]);
-            }
-            // the pair's own interaction (its particles are not entries of their row): once per pair.  For a single
-            // particle pi1 is the dummy: nothing.
-            if (sub == 0) {
-                if (ONE_TYPE) {
-                    pair_term<THERMO, FN>(pi0, pi1, c12, c6, pp1, px1, A.pot, a0);
-                    pair_term<THERMO, FN>(pi1, pi0, c12, c6, pp1, px1, A.pot, a1);
-                } else {
-                    const PairParam p01 = prow0[__float_as_int(pi1.w)];
-                    PairParamX x01 = {0.f, 0.f, 0.f, 0.f};
-                    if (FN != FN_LJ) x01 = prowx0[__float_as_int(pi1.w)];
-                    pair_term<THERMO, FN>(pi0, pi1, 12.0f * p01.lj1, 6.0f * p01.lj2, p01, x01, A.pot, a0);
-                    pair_term<THERMO, FN>(pi1, pi0, 12.0f * p01.lj1, 6.0f * p01.lj2, p01, x01, A.pot, a1);
+                for (int e = 0; e < EPL; e++) {
+                    if (ONE_TYPE) {
+                        pair_term<THERMO, FN>(pi, pj[e], c12, c6, pp1, px1, A.pot, a);
+                    } else {
+                        const int tj = __float_as_int(pj[e].w);
+                        const PairParam pp = prow[tj];
+                        PairParamX px = {0.f, 0.f, 0.f, 0.f};
+                        if (FN != FN_LJ) px = prowx[tj];
+                        pair_term<THERMO, FN>(pi, pj[e], 12.0f * pp.lj1, 6.0f * pp.lj2, pp, px, A.pot, a);
+                    }
                 }
             }
         }
         cp_async_wait<0>();                          // the own data of this pass has landed; nothing of this pass may land
-        __syncwarp();                                //   after the next pass's copies start
-        const float4 *o = own + 2 * ql + sub;
-        float4 v = make_float4(0.f, 0.f, 0.f, 1.f), p = v, pb = v;
-        const bool mine = sub < np;                  // lane sub finishes particle gi0 + sub
-        if (nve && mine) { v = o[0]; if (nv.kick_drift) { p = o[2 * PPB]; pb = o[4 * PPB]; } }
-        if (q0 + PPB < npairs) prep(q0 + PPB);       // the next pass's copies fly during the reduction and the integration
+        __syncwarp();                                //   after the next pass's copies start; lane 1's copy visible to lane 0
+        const float4 *o = own + ql;
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f), p = v, pb = v;
+        if (nve && active && sub == 0) { v = o[0]; if (nv.kick_drift) { p = o[PPB]; pb = o[2 * PPB]; } }
+        if (q0 + PPB < nown) prep(q0 + PPB);             // the next pass's copies fly during the reduction and the integration
 
 #pragma unroll
         for (int o2 = TPP >> 1; o2 > 0; o2 >>= 1) {
-            a0.fx += __shfl_xor_sync(0xffffffffu, a0.fx, o2); a1.fx += __shfl_xor_sync(0xffffffffu, a1.fx, o2);
-            a0.fy += __shfl_xor_sync(0xffffffffu, a0.fy, o2); a1.fy += __shfl_xor_sync(0xffffffffu, a1.fy, o2);
-            a0.fz += __shfl_xor_sync(0xffffffffu, a0.fz, o2); a1.fz += __shfl_xor_sync(0xffffffffu, a1.fz, o2);
+            a.fx += __shfl_xor_sync(0xffffffffu, a.fx, o2);
+            a.fy += __shfl_xor_sync(0xffffffffu, a.fy, o2);
+            a.fz += __shfl_xor_sync(0xffffffffu, a.fz, o2);
             if (THERMO) {
-                a0.u += __shfl_xor_sync(0xffffffffu, a0.u, o2);     a1.u += __shfl_xor_sync(0xffffffffu, a1.u, o2);
-                a0.wxx += __shfl_xor_sync(0xffffffffu, a0.wxx, o2); a1.wxx += __shfl_xor_sync(0xffffffffu, a1.wxx, o2);
-                a0.wxy += __shfl_xor_sync(0xffffffffu, a0.wxy, o2); a1.wxy += __shfl_xor_sync(0xffffffffu, a1.wxy, o2);
-                a0.wxz += __shfl_xor_sync(0xffffffffu, a0.wxz, o2); a1.wxz += __shfl_xor_sync(0xffffffffu, a1.wxz, o2);
-                a0.wyy += __shfl_xor_sync(0xffffffffu, a0.wyy, o2); a1.wyy += __shfl_xor_sync(0xffffffffu, a1.wyy, o2);
-                a0.wyz += __shfl_xor_sync(0xffffffffu, a0.wyz, o2); a1.wyz += __shfl_xor_sync(0xffffffffu, a1.wyz, o2);
-                a0.wzz += __shfl_xor_sync(0xffffffffu, a0.wzz, o2); a1.wzz += __shfl_xor_sync(0xffffffffu, a1.wzz, o2);
+                a.u += __shfl_xor_sync(0xffffffffu, a.u, o2);
+                a.wxx += __shfl_xor_sync(0xffffffffu, a.wxx, o2);
+                a.wxy += __shfl_xor_sync(0xffffffffu, a.wxy, o2);
+                a.wxz += __shfl_xor_sync(0xffffffffu, a.wxz, o2);
+                a.wyy += __shfl_xor_sync(0xffffffffu, a.wyy, o2);
+                a.wyz += __shfl_xor_sync(0xffffffffu, a.wyz, o2);
+                a.wzz += __shfl_xor_sync(0xffffffffu, a.wzz, o2);
             }
         }
-        if (!mine) continue;
-        const Acc &a = sub ? a1 : a0;
-        const int gi = gi0 + sub;
+        if (!active) continue;
         // U_i = 1/2 sum V, W_i = 1/2 sum d f (reading c6.i)
-        if (THERMO) {
-            A.force[gi] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
+        if (THERMO && sub == TPP - 1) {
             A.virial[2 * (int64_t)gi] = make_float4(0.5f * a.wxx, 0.5f * a.wxy, 0.5f * a.wxz, 0.5f * a.wyy);
             A.virial[2 * (int64_t)gi + 1] = make_float4(0.5f * a.wyz, 0.5f * a.wzz, 0.f, 0.f);
         }
+        if (sub != 0) continue;
+        if (THERMO) A.force[gi] = make_float4(a.fx, a.fy, a.fz, 0.5f * a.u);
         if (!nve) continue;
         // reading c7 (and n1, n2), operation by operation as nve_kernel does it
         if (nv.kick_prev) thermo_kick_prev(nv, xi, hdt, a.fx, a.fy, a.fz, v, nv.ens == 2 ? nv.tag[gi] : 0u);
@@ -539,10 +513,10 @@ size_t force_smem_bytes(const hb_system *h)
     // and forces of a pass
     return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? ((sizeof(PairParam) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
            (h->ntypes > 1 ? ((sizeof(PairParamX) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
-           (size_t)4 * 16 * force_block_of(h) + (size_t)3 * 2 * 16 * force_ppb(h) + (h->geom.fast ? 0 : sizeof(TileShared));
+           (size_t)4 * 16 * force_block_of(h) + (size_t)3 * 16 * force_ppb(h) + (h->geom.fast ? 0 : sizeof(TileShared));
 }
 
-template <int TPP, int EPL, bool THERMO, int FN>
+template <int TPP, int EPL, bool THERMO, bool SCALED, int FN>
 static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
 {
     const size_t smem = force_smem_bytes(h);
@@ -556,7 +530,6 @@ static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
     A.N = (int)h->N;
     A.ntypes = h->ntypes;
     A.pot = h->pot;
-    A.dbg = h->tun.dbg;
     A.params = h->params;
     A.paramsx = h->paramsx;
     A.force = h->force;
@@ -566,9 +539,9 @@ static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
     if (nve) A.nv = *nve;
     cudaError_t e;
 #define LJ_LAUNCH(ONE)                                                                                                      \
-    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO, FN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, FN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
     if (e != cudaSuccess) return e;                                                                                         \
-    lj_tile_kernel<TPP, EPL, ONE, THERMO, FN><<<grid, force_block_of(h), smem, h->stream>>>(A);
+    lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, FN><<<grid, force_block_of(h), smem, h->stream>>>(A);
     if (h->ntypes == 1) { LJ_LAUNCH(true) } else { LJ_LAUNCH(false) }
 #undef LJ_LAUNCH
     h->stats.kernel_launches++;
@@ -581,7 +554,9 @@ static cudaError_t launch_force_t(hb_system *h, const NveArgs *nve)
     // energies and virials of a step can only be read after hb_run_nve returns: with thermo_every = 0 the inner
     // steps of a chunk (both half kicks fused in) compute forces only
     const bool thermo = !(nve && nve->forces_only);
-    return thermo ? launch_force_tts<TPP, EPL, true, FN>(h, nve) : launch_force_tts<TPP, EPL, false, FN>(h, nve);
+    const bool scaled = h->geom.eshift == 4;
+    if (thermo) return scaled ? launch_force_tts<TPP, EPL, true, true, FN>(h, nve) : launch_force_tts<TPP, EPL, true, false, FN>(h, nve);
+    return scaled ? launch_force_tts<TPP, EPL, false, true, FN>(h, nve) : launch_force_tts<TPP, EPL, false, false, FN>(h, nve);
 }
 
 cudaError_t launch_force(hb_system *h, const NveArgs *nve)
@@ -591,7 +566,7 @@ cudaError_t launch_force(hb_system *h, const NveArgs *nve)
     if (h->pot != HB_POT_LJ) return launch_force_t<2, 8, FN_GEN>(h, nve);
     if (h->shift_mode == HB_XPLOR) return launch_force_t<2, 8, FN_XPLOR>(h, nve);
     const int epl = h->tun.epl == 8 ? 8 : 4;
-    switch (force_tpp(h)) {
+    switch (h->tun.tpp) {
         case 2: return epl == 8 ? launch_force_t<2, 8, FN_LJ>(h, nve) : launch_force_t<2, 4, FN_LJ>(h, nve);
         case 8: return launch_force_t<8, 4, FN_LJ>(h, nve);   // 8 x 8 entries would read past the 32-entry row padding
         default: return epl == 8 ? launch_force_t<4, 8, FN_LJ>(h, nve) : launch_force_t<4, 4, FN_LJ>(h, nve);

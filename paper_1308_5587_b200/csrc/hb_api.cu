@@ -110,20 +110,13 @@ int upload_params(hb_system *h)
     return HB_OK;
 }
 
-// candidate-list entries of the list build per staged slot: every halo row serves up to nine own rows (nlist.cu)
-double clist_per_slot(int ty, int tz) { return 9.0 * ty * tz / ((ty + 2.0) * (tz + 2.0)); }
-
-int clist_cap_of(int cap, int ty, int tz) { return ((int)(cap * clist_per_slot(ty, tz)) + 64 + 63) / 64 * 64; }
-
-int stage_cap_max(const hb_system *h, int ty, int tz)
+int stage_cap_max(const hb_system *h)
 {
-    // what is left of the opt-in shared memory after the static tables (ListShared, the scan scratch: < 8 KB), for the
-    // list build (16 bytes per slot + its candidate lists) and for the step kernel (16 bytes per slot + its extras)
-    const int64_t left = (int64_t)h->smem_max - 8192;
-    const int64_t force_extra = (int64_t)force_smem_bytes(h) - (int64_t)h->geom.cap * 16;
-    const int64_t by_force = (left - force_extra) / 16;
-    const int64_t by_list = (int64_t)((left - 256) / (16.0 + 2.0 * clist_per_slot(ty, tz)));
-    return (int)std::max<int64_t>(64, std::min<int64_t>(16383, std::min(by_force, by_list)));   // 14-bit slots (tile.cuh)
+    // what is left of the opt-in shared memory after the static tables (TileShared and the scan scratch, < 4 KB) and
+    // the larger of the two kernels' extras beside the staging area itself (both functions count cap * 16 bytes)
+    const size_t extra = std::max(nlist_smem_bytes(h), force_smem_bytes(h)) - (size_t)h->geom.cap * 16;
+    const int64_t left = (int64_t)h->smem_max - 4096 - (int64_t)extra;
+    return (int)std::max<int64_t>(64, std::min<int64_t>(65535, left / 16));
 }
 
 // Tile dimensions and staging capacity (tile.cuh).  Tunables override the choice.
@@ -167,23 +160,21 @@ int choose_tiles(hb_system *h, int min_cap)
     }
     cap = std::max(cap, min_cap);
     cap = round_up(std::max(cap, 64), 32);
-    const int cap_max = stage_cap_max(h, ty, tz);
-    if (cap > cap_max) {
-        if (min_cap > cap_max && tx * ty * tz > 1) {
+    if (cap > stage_cap_max(h)) {
+        if (min_cap > stage_cap_max(h) && tx * ty * tz > 1) {
             // shrink to one cell per tile (27 staged cells) and scale the requirement with the halo volume
             const int nh = (tx + 2) * (ty + 2) * (tz + 2);
             h->tun.tile_x = h->tun.tile_y = h->tun.tile_z = 1;
             return choose_tiles(h, (int)((int64_t)min_cap * 27 / nh));
         }
-        if (min_cap > cap_max) {
+        if (min_cap > stage_cap_max(h)) {
             h->err = "a tile of cells with its halo holds " + std::to_string(min_cap) +
                      " particles: more than fit in shared memory; use smaller tiles (tile_x/y/z = 1)";
             return HB_ENOMEM;
         }
-        cap = cap_max;
+        cap = stage_cap_max(h);
     }
     g.cap = cap;
-    g.ccap = clist_cap_of(cap, ty, tz);
     h->own_est = (double)h->N / (double)h->ncells * tx * ty * tz;
     // fast geometry: tile + halo + what a particle can drift between builds is narrower than L/2 on every axis,
     // so the periodic image nearest to the tile centre is the right one for every staged particle
@@ -192,6 +183,7 @@ int choose_tiles(hb_system *h, int min_cap)
         const int tmax = std::max(tx, std::max(ty, tz));
         g.fast = ((0.5 * tmax + 1.0) * w + 2.0 * (double)h->r_buff + 0.05 * w < 0.5 * (double)h->L) ? 1 : 0;
     }
+    g.eshift = g.cap <= 4096 ? 4 : 0;
     if (memcmp(&g, &h->geom, sizeof g) != 0) {
         destroy_graphs(h);
         h->nlist_valid = false;
@@ -235,12 +227,6 @@ int configure_geometry(hb_system *h)
     }
     HB_TRY(choose_tiles(h, 0));
     h->stats.cells_per_axis = m;
-    {   // per-type-pair list cutoffs (tunable nlist_pair_rcut): (r_cut,ab + r_buff)^2, each operation in binary32
-        std::vector<float> t2((size_t)h->ntypes * h->ntypes);
-        for (size_t p = 0; p < t2.size(); p++) { const float r = (float)h->rcut[p] + h->r_buff; t2[p] = r * r; }
-        HB_CK(cudaMemcpyAsync(h->rmax2_pair, t2.data(), t2.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
-        HB_CK(cudaStreamSynchronize(h->stream));
-    }
     return HB_OK;
 }
 
@@ -342,15 +328,14 @@ int build_nlist_sync(hb_system *h)
             continue;
         }
         h->stats.max_nbrs = h->h_flags[FL_MAX_NBRS];
-        const int rows_needed = h->h_flags[FL_OVERFLOWED];      // 0, or the pitch the longest row of this build needs
-        if (!rows_needed) {
+        if (h->h_flags[FL_MAX_NBRS] <= h->row_pitch) {
+            HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
             HB_TRY(clear_need_flags(h));
             h->cells_valid = h->nlist_valid = true;
             return HB_OK;
         }
         h->stats.overflow_retries++;
-        HB_TRY(set_flag(h, FL_OVERFLOWED, 0));
-        HB_TRY(ensure_rows(h, (int)(rows_needed * (1.0 + 0.01 * h->tun.grow_pct)) + 8));
+        HB_TRY(ensure_rows(h, (int)(h->h_flags[FL_MAX_NBRS] * (1.0 + 0.01 * h->tun.grow_pct)) + 8));
     }
     h->err = "neighbor-list rows keep overflowing";
     return HB_ENOMEM;
@@ -820,7 +805,6 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     HB_TRY(dev_alloc_t(h, &h->nlistn, n));
     HB_TRY(dev_alloc_t(h, &h->params, (size_t)ntypes * ntypes));
     HB_TRY(dev_alloc_t(h, &h->paramsx, (size_t)ntypes * ntypes));
-    HB_TRY(dev_alloc_t(h, &h->rmax2_pair, (size_t)ntypes * ntypes));
     HB_TRY(dev_alloc_t(h, &h->flags, (size_t)FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_flags, sizeof(int) * FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_thermo, sizeof(double) * 16));
@@ -863,7 +847,7 @@ int hb_destroy(hb_system *h)
     dev_free(h, h->bk_tstate);
     void *ptrs[] = {h->posbuf[0], h->posbuf[1], h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->vel2,
                     h->force2, h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_image,
-                    h->bk_tag, h->params, h->paramsx, h->rmax2_pair, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
+                    h->bk_tag, h->params, h->paramsx, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
                     h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
                     h->flags, h->thermo_part};
     for (void *p : ptrs) dev_free(h, p);
@@ -1386,7 +1370,6 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "force_block")) return &h->tun.force_block;
     if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
     if (!strcmp(name, "nlist_block")) return &h->tun.nlist_block;
-    if (!strcmp(name, "nlist_pair_rcut")) return &h->tun.nlist_pair_rcut;
     if (!strcmp(name, "tile_x")) return &h->tun.tile_x;
     if (!strcmp(name, "tile_y")) return &h->tun.tile_y;
     if (!strcmp(name, "tile_z")) return &h->tun.tile_z;
@@ -1400,7 +1383,6 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "coop_blocks")) return &h->tun.coop_blocks;
     if (!strcmp(name, "graph_mode")) return &h->tun.graph_mode;
     if (!strcmp(name, "graph_steps")) return &h->tun.graph_steps;
-    if (!strcmp(name, "dbg")) return &h->tun.dbg;
     return nullptr;
 }
 
@@ -1410,15 +1392,15 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     int *slot = tunable_slot(h, name);
     if (!slot) { h->err = std::string("unknown tunable ") + (name ? name : "(null)"); return HB_EINVAL; }
     bool ok = true;
-    if (slot == &h->tun.tpp) ok = value == 0 || value == 2 || value == 4 || value == 8;
+    if (slot == &h->tun.tpp) ok = value == 2 || value == 4 || value == 8;
     else if (slot == &h->tun.epl) ok = value == 4 || value == 8;
-    else if (slot == &h->tun.force_block) ok = value == 0 || value == 64 || value == 128 || value == 256;
+    else if (slot == &h->tun.force_block) ok = value == 0 || value == 128 || value == 256;
     else if (slot == &h->tun.nlist_block) ok = value == 128 || value == 256;
     else if (slot == &h->tun.nlist_ppi) ok = value == 1 || value == 2 || value == 4;
     else if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z) ok = value >= 0 && value <= 16;
     else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;
     else if (slot == &h->tun.row_pitch) ok = value >= 0 && value <= 4096;
-    else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve || slot == &h->tun.thermo_every || slot == &h->tun.nlist_pair_rcut) ok = value == 0 || value == 1;
+    else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve || slot == &h->tun.thermo_every) ok = value == 0 || value == 1;
     else if (slot == &h->tun.coop_rebuild) ok = value >= -1 && value <= 2;
     else if (slot == &h->tun.coop_blocks) ok = value >= 1 && value <= 8;
     else if (slot == &h->tun.grow_pct) ok = value >= 0 && value <= 400;
@@ -1428,9 +1410,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     *slot = value;
     destroy_graphs(h);
     if (slot == &h->tun.row_pitch && value > 0) HB_TRY(ensure_rows(h, value));
-    if (slot == &h->tun.nlist_pair_rcut) h->nlist_valid = false;
-    if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z || slot == &h->tun.stage_cap ||
-        slot == &h->tun.force_block || slot == &h->tun.tpp) {      // the block size decides the step kernel's shared-memory budget
+    if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z || slot == &h->tun.stage_cap) {
         h->nlist_valid = false;
         if (h->m > 0) HB_TRY(choose_tiles(h, 0));
     }

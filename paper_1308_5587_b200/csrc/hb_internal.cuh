@@ -55,7 +55,7 @@ struct TileGeom {
     int ntiles;
     int cap;            // shared-memory slots (slot 0 is the far-away dummy)
     int fast;           // 1: tile + halo narrower than L/2 on every axis (image by tile centre, halo rows staged as contiguous pieces)
-    int ccap;           // entries of the list build's candidate lists (shared memory, 16 bit each), sized with cap
+    int eshift;         // list entries are slot << eshift: 4 (the byte offset of the staged position) when cap <= 4096, else 0
     float L;
 };
 
@@ -66,11 +66,10 @@ constexpr int TILE_PROWS_MAX = 86;    // halo (y, z) rows per tile, at most: TIL
 constexpr int ROW_PAD = 32;           // list rows are padded with dummy entries to a multiple of this
 
 struct Tunables {
-    int tpp = 0;           // threads per PAIR of particles in the step kernel (0 = 4 below 200,000 particles, else 2: measured)
+    int tpp = 2;           // threads per particle in the force kernel
     int epl = 8;           // list entries per thread per iteration (4 or 8)
-    int force_block = 0;   // threads per block of the force kernel (64, 128 or 256; 0 = one pass over the tile's particles if possible)
-    int nlist_ppi = 4;     // (kept for compatibility: the pair-row build always tests four particles per candidate load)
-    int nlist_pair_rcut = 0;   // 1: the list keeps pair (i, j) iff d < r_cut(type i, type j) + r_buff; 0: one r_max
+    int force_block = 0;   // threads per block of the force kernel (128 or 256; 0 = one pass over the tile's particles if possible)
+    int nlist_ppi = 4;     // particles tested per candidate load
     int nlist_block = 256; // threads per block of the stand-alone list kernel (128 or 256)
     int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
     int stage_cap = 0;     // 0 = estimated from the density
@@ -84,7 +83,6 @@ struct Tunables {
     int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 100;
-    int dbg = 0;           // timing experiments only (wrong physics): 1 skip the pair loop, 2 stop after the tile tables, 4 empty kernel
 };
 
 enum { TS_XI = 0, TS_ETA = 1, TS_KSUM = 2, TS_LBASE = 3, TS_COUNT = 8 };
@@ -133,7 +131,6 @@ struct hb_system {
     int bk_cur = 0, bk_parity = 0;
     PairParam *params = nullptr;
     PairParamX *paramsx = nullptr;
-    float *rmax2_pair = nullptr;   // [ntypes^2] (r_cut,ab + r_buff)^2 for the typed list build
 
     float4 *pos() const { return posbuf[cur]; }
 
@@ -216,17 +213,12 @@ struct hb_system {
 static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // threads per particle of the step kernel actually launched (the smoothed functor exists in the default layout only)
-static inline int force_tpp(const hb_system *h)
-{
-    if (h->shift_mode == HB_XPLOR || h->pot != HB_POT_LJ) return 2;
-    return h->tun.tpp > 0 ? h->tun.tpp : (h->N < 200000 ? 4 : 2);
-}
+static inline int force_tpp(const hb_system *h) { return (h->shift_mode == HB_XPLOR || h->pot != HB_POT_LJ) ? 2 : h->tun.tpp; }
 
 static inline int force_block_of(const hb_system *h)
 {
     if (h->tun.force_block > 0) return h->tun.force_block;
-    const double threads = 0.5 * h->own_est * force_tpp(h);   // one pass over the tile: a thread group per PAIR of particles
-    return threads > 320.0 ? 256 : (threads > 80.0 ? 128 : 64);
+    return h->own_est * force_tpp(h) > 160.0 ? 256 : 128;
 }
 
 // What the drift part of a step kernel needs (nve_kernel and the fused force kernel).

@@ -4,38 +4,34 @@
 // unsynchronised row writes "a big bottleneck" that "GF100 does not have enough
 // shared memory to regularize".  Here ONE BLOCK OWNS ONE TILE of
 // cells (tile.cuh): the tile plus its one-cell halo is staged once in shared
-// memory (one warp per halo cell), already moved to the periodic image the tile sees.
-//
-// PAIR ROWS.  ncu on the round-1 step kernel showed the shared-memory pipe as its limit: every listed pair costs one
-// random 16-byte gather (profiles/r2a_kernels.md).  So two consecutive particles (a, a + 1) of an own (y, z) row of
-// the tile share ONE list row, the UNION of their neighbor sets (they are about one sigma apart, the union is about
-// 1.3 times one set): one gather in the step kernel then serves two pair evaluations.  Each 16-bit entry carries, beside
-// the slot, two bits that say whose neighbor it is (bit 0: of a, bit 1: of a + 1), so the row still states N(a) and
-// N(a + 1) exactly (hb_get_nlist reads them back); the two particles of a pair are never entries of their own row
-// (the step kernel evaluates that one interaction directly; nlistn carries a flag if they are within r_max).
-//
-//   1. candidates: for every own row of the tile the block writes ONE list of candidate slots, column by column in x
-//      (a column = the 3 x 3 cells around the row at one x), so that the 27 cells around any run of own cells are ONE
-//      contiguous range of it (Alg. 3 l.11; no celladj table: PAPER.md:187 stored it to save registers);
-//   2. a warp takes four consecutive particles of a row (two pairs): lane l tests candidates l, l + 32, ... of the
-//      range that belongs to the cells of those four against all four (one candidate load serves four tests, Alg. 3
-//      l.16-17) and records the hits as bits of four registers;
-//   3. per pair the union mask is compacted with one warp prefix sum of popcounts (both pairs in one scan) and the
-//      lanes write their entries straight into the row-major, 128-byte aligned list; the row ends with at least 32
-//      entries of 0 (the step kernel reads no row length).
-// List entries are slots of the tile's staging layout, not particle indices: the step kernel stages the same tile
-// the same way and gathers from shared memory (hb_get_nlist translates back to tags).
-// The kernel also finishes the reorder of the particle data: it copies the tile's own particles from the scratch set
-// (cell order) back into the live arrays.
+// memory (one warp per halo cell), already moved to the periodic image the tile sees,
+// and then ONE WARP OWNS ONE CELL of the tile (several warps split a cell's particles
+// when the tile has fewer cells than the block has warps):
+//   1. lanes 0..8 look up the nine x-rows of three adjacent cells (on the fly, no
+//      celladj table: PAPER.md:187 stored it to save registers) -- in the staged
+//      layout each row is one contiguous run of slots -- and the warp flattens the
+//      nine runs into one list of candidate slots (16-bit), padded with the
+//      far-away dummy slot 0 to whole groups of 32;
+//   2. for every particle i of the cell (PPI at a time, so each candidate load
+//      serves PPI distance tests) lane l tests candidates l, l+32, ... and records
+//      the hits as bits of a register; one warp prefix sum of the per-lane __popc
+//      counts gives every lane its positions in the row and the lanes write their
+//      hits' SLOT NUMBERS (16 bit) straight into the row-major, 128-byte aligned
+//      list; the row ends with at least 32 entries of slot 0 (the force kernel reads no row length).
+// List entries are slots of the tile's staging layout, not particle indices: the
+// force kernel stages the same tile the same way and gathers from shared memory
+// (hb_get_nlist translates back to tags).  Half the bytes of a 32-bit index list.
+// The kernel also finishes the reorder of the particle data: it copies the tile's
+// own particles from the scratch set (cell order) back into the live arrays.
 #include "cells_dev.cuh"
 #include "tile.cuh"
 
-constexpr int NL_PPI = 4;        // particles tested per candidate load = two pairs
-constexpr int NL_CHUNK = 1024;   // candidates per pass over a group = 32 groups of 32 = one bit mask per particle
+constexpr int NL_CLIST = 1024;   // candidate slots per warp per chunk = 32 groups of 32 = one bit mask
+constexpr int NL_WARPS = TILE_THREADS / 32;
 
 size_t nlist_smem_bytes(const hb_system *h)
 {
-    return (size_t)h->geom.cap * 16 + (size_t)h->geom.ccap * 2;   // staged positions | candidate lists
+    return (size_t)h->geom.cap * 16 + (size_t)NL_WARPS * NL_CLIST * 2;   // sized for the largest block (8 warps)
 }
 
 struct CopyBack {   // scratch set -> live arrays; pos == nullptr: skip
@@ -53,23 +49,14 @@ struct ListArgs {
     const int *cell_start;
     const float4 *pos_build;
     float rmax2;
-    const float *rmax2_pair;   // TYPED: [ntypes * ntypes] squared list cutoffs (r_cut,ab + r_buff)^2
-    int ntypes;
     int pitch;
     uint16_t *nlist;
     int *nlistn, *flags;
     CopyBack cb;
 };
 
-struct ListShared {
-    TileShared t;
-    int colabs[TILE_HMAX + 1];       // start of column (own row, jx) in the candidate array, index row * hx + jx; [nrows * hx] = total
-    int colmid[TILE_HMAX];           // where the centre cell of that column (the own row's cell at jx) starts
-    int grp_off[TILE_ROWS_MAX + 1];  // groups of NL_PPI particles per own row, prefix
-};
-
-// Algorithm 3 for one tile, by one block
-template <bool TYPED>
+// Algorithm 3 for one tile, by one block of TILE_THREADS threads
+template <int PPI>
 __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int tile, unsigned char *smem_raw)
 {
     const TileGeom &g = la.g;
@@ -81,25 +68,22 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
     int *__restrict__ nlistn = la.nlistn;
     int *__restrict__ flags = la.flags;
     const CopyBack &cb = la.cb;
-    __shared__ ListShared s;
-    __shared__ float s_rm2[TYPED ? 64 : 1];     // TYPED needs ntypes <= 8 (the host falls back to the single cutoff otherwise)
+    const int eshift = g.eshift;
+    __shared__ TileShared s;
     float4 *stage = reinterpret_cast<float4 *>(smem_raw);
-    uint16_t *clist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)g.cap * 16);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-    constexpr unsigned FULL = 0xffffffffu;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    uint16_t *clist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)g.cap * 16) + warp * NL_CLIST;
 
     if (tile == 0 && threadIdx.x == 0) flags[FL_BUILDS] += 1;
-    if (TYPED)
-        for (int k = threadIdx.x; k < la.ntypes * la.ntypes; k += blockDim.x) s_rm2[k] = la.rmax2_pair[k];
     TileCtx t;
     tile_decode(g, tile, t);
-    const bool fits = tile_tables(g, cell_start, t, s.t, flags);
+    const bool fits = tile_tables(g, cell_start, t, s, flags);
 
     // the reorder's last leg: own particles, scratch set -> live arrays (always, so the state stays whole)
     if (cb.pos) {
         for (int q = threadIdx.x; q < t.nown; q += blockDim.x) {
             int gi, slot;
-            tile_own(s.t.d, q, gi, slot);
+            tile_own(s.d, q, gi, slot);
             cb.pos[gi] = pos_build[gi];
             cb.vel[gi] = cb.vel2[gi];
             cb.image[gi] = cb.image2[gi];
@@ -111,212 +95,147 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
         }
     }
     if (!fits) return;
-    tile_stage_positions_by_cell(g, t, s.t, pos_build, stage, nullptr);
-
-    // ---- 1. candidate columns: lengths, prefix, fill ----
-    const int ncol = t.nrows * t.hx;
-    for (int c = threadIdx.x; c < ncol; c += blockDim.x) {
-        const int orow = c / t.hx, jx = c - orow * t.hx;
-        const int ly = orow % t.ey, lz = orow / t.ey;
-        int n = 0;
-#pragma unroll
-        for (int k = 0; k < 9; k++) {
-            const int h = jx + t.hx * ((ly + k % 3) + t.hy * (lz + k / 3));   // (ly + 1 + dy, lz + 1 + dz), dy, dz = -1, 0, 1
-            n += s.t.hslot[h + 1] - s.t.hslot[h];
-        }
-        s.colabs[c] = n;
-    }
-    if (threadIdx.x == 0) {
-        int run = 0;
-        s.grp_off[0] = 0;
-        for (int r = 0; r < t.nrows; r++) { run += (s.t.d.own_off[r + 1] - s.t.d.own_off[r] + NL_PPI - 1) / NL_PPI; s.grp_off[r + 1] = run; }
-    }
-    __syncthreads();
-    if (threadIdx.x < 32) {   // exclusive scan of up to TILE_HMAX column lengths: 8 per lane
-        const int base = lane * 8;
-        int v[8], tsum = 0;
-#pragma unroll
-        for (int q = 0; q < 8; q++) { v[q] = base + q < ncol ? s.colabs[base + q] : 0; tsum += v[q]; }
-        int incl = tsum;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULL, incl, o); if (lane >= o) incl += y; }
-        int run = incl - tsum;
-#pragma unroll
-        for (int q = 0; q < 8; q++) { if (base + q < ncol) s.colabs[base + q] = run; run += v[q]; }
-        if (lane == 31) s.colabs[ncol] = run;
-    }
-    __syncthreads();
-    const int ctotal = s.colabs[ncol];
-    if (ctotal > g.ccap) {    // the candidate lists need more room than the staging capacity was sized for: same repair
-        if (threadIdx.x == 0) atomicMax(&flags[FL_STAGE_OVER], max(t.nslots + 1, (int)((int64_t)ctotal * g.cap / g.ccap) + 1));
-        return;
-    }
-    for (int c = warp; c < ncol; c += nwarps) {
-        const int orow = c / t.hx, jx = c - orow * t.hx;
-        const int ly = orow % t.ey, lz = orow / t.ey;
-        int at = s.colabs[c];
-#pragma unroll
-        for (int k = 0; k < 9; k++) {
-            const int h = jx + t.hx * ((ly + k % 3) + t.hy * (lz + k / 3));
-            const int s0 = s.t.hslot[h], n = s.t.hslot[h + 1] - s0;
-            if (k == 4 && lane == 0) s.colmid[c] = at;
-            for (int v = lane; v < n; v += 32) clist[at + v] = (uint16_t)(s0 + v);
-            at += n;
-        }
-    }
+    tile_stage_positions_by_cell(g, t, s, pos_build, stage, nullptr);
     __syncthreads();
 
-    // ---- 2., 3. groups of four particles (two pairs) ----
-    int wmax_len = 0, wmax_need = 0;
-    const int ngrp = s.grp_off[t.nrows];
-    for (int grp = warp; grp < ngrp; grp += nwarps) {
-        int orow = 0;
-        while (orow + 1 < t.nrows && s.grp_off[orow + 1] <= grp) orow++;
-        const int q0 = NL_PPI * (grp - s.grp_off[orow]);
-        const int nvalid = min(NL_PPI, s.t.d.own_off[orow + 1] - s.t.d.own_off[orow] - q0);
-        const int slot_f = s.t.d.own_slot[orow] + q0;
-        const int gi_f = s.t.d.own_start[orow] + q0;
-        const int ly = orow % t.ey, lz = orow / t.ey;
-        const int hrow = ((lz + 1) * t.hy + (ly + 1)) * t.hx;     // halo cell (jx = 0) of the own row
-        // own cell lx of a slot of this row: how many own cells start at or before it, minus one
-        const int cell_first = lane < t.ex ? s.t.hslot[hrow + 1 + lane] : 0x7fffffff;
-        float px[NL_PPI], py[NL_PPI], pz[NL_PPI];
-        int self[NL_PPI], cnt[NL_PPI];
-        const float *rmrow[NL_PPI];
-        int lxa = 0, lxb = 0;
-#pragma unroll
-        for (int p = 0; p < NL_PPI; p++) {
-            px[p] = py[p] = pz[p] = -1e18f;
-            self[p] = -1;
-            cnt[p] = 0;
-            rmrow[p] = s_rm2;
-            if (p < nvalid) {     // warp-uniform
-                const int sp = slot_f + p;
-                const float4 q = stage[sp];                      // same address in all lanes: one broadcast
-                px[p] = q.x; py[p] = q.y; pz[p] = q.z;
-                if (TYPED) rmrow[p] = s_rm2 + __float_as_int(q.w) * la.ntypes;
-                const int lx = __popc(__ballot_sync(FULL, cell_first <= sp)) - 1;
-                if (p == 0) lxa = lx;
-                lxb = lx;
-                self[p] = s.colmid[orow * t.hx + lx + 1] + (sp - s.t.hslot[hrow + 1 + lx]);
-            }
-        }
-        const int c0 = s.colabs[orow * t.hx + lxa], c1 = s.colabs[orow * t.hx + lxb + 3];
-        uint16_t *const rowA = nlist + (int64_t)gi_f * pitch, *const rowB = nlist + (int64_t)(gi_f + 2) * pitch;
-        const int capA = nvalid >= 2 ? 2 * pitch : pitch, capB = nvalid >= 4 ? 2 * pitch : pitch;
-        int totA = 0, totB = 0;
-        bool abA = false, abB = false;
+    int wmax = 0;
+    const int ncell_own = t.ex * t.ey * t.ez;
+    // a tile with fewer cells than the block has warps gives every cell several warps: they share the cell's
+    // candidates and split its particles
+    const int nwarps = blockDim.x >> 5;
+    const int wpc = max(1, nwarps / max(1, ncell_own));
+    for (int item = warp; item < ncell_own * wpc; item += nwarps) {
+        const int oc = item / wpc, part = item % wpc;
+        const int lx = oc % t.ex, ly = (oc / t.ex) % t.ey, lz = oc / (t.ex * t.ey);
+        const int hc = ((lz + 1) * t.hy + (ly + 1)) * t.hx + (lx + 1);
+        const int cslot0 = s.hslot[hc];
+        const int n_c = s.hslot[hc + 1] - cslot0;
+        if (n_c == 0) continue;
+        const int cg0 = s.hg[hc];
 
-        for (int k0 = c0; k0 < c1; k0 += NL_CHUNK) {
-            const int Tc = min(NL_CHUNK, c1 - k0);
+        // ---- 1. nine runs of candidates (Alg. 3 l.11: the 27 adjacent cells) ----
+        int rs = 0, rl = 0;
+        if (lane < 9) {
+            const int dy = lane % 3 - 1, dz = lane / 3 - 1;
+            const int hrow = ((lz + 1 + dz) * t.hy + (ly + 1 + dy)) * t.hx + lx;
+            rs = s.hslot[hrow];
+            rl = s.hslot[hrow + 3] - rs;
+        }
+        int incl = rl;
+#pragma unroll
+        for (int o = 1; o < 16; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += y;
+        }
+        const int roff = incl - rl;
+        const int T = __shfl_sync(0xffffffffu, incl, 8);
+        // candidate number of the own cell's first member (run 4 = the own row)
+        const int self0 = __shfl_sync(0xffffffffu, roff, 4) + (cslot0 - __shfl_sync(0xffffffffu, rs, 4));
+
+        for (int k0 = 0; k0 < T; k0 += NL_CLIST) {
+            const int Tc = min(NL_CLIST, T - k0);
             const int ngroups = (Tc + 31) >> 5;
-            unsigned hits[NL_PPI] = {0u, 0u, 0u, 0u};
-            // lane l tests candidates l, l+32, ...; bit gq of hits[p] records candidate 32 gq + l (Alg. 3 l.16-17)
-#pragma unroll 2
-            for (int gq = 0; gq < ngroups; gq++) {
-                const int ci = k0 + (gq << 5) + lane;
-                const float4 e = stage[ci < c1 ? clist[ci] : 0];      // slot 0 = the far-away dummy: never a hit
-                const unsigned bit = 1u << gq;
+            __syncwarp();
 #pragma unroll
-                for (int p = 0; p < NL_PPI; p++) {
-                    const float dx = e.x - px[p], dy = e.y - py[p], dz = e.z - pz[p];
-                    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                    const float rm = TYPED ? rmrow[p][__float_as_int(e.w)] : rmax2;
-                    if (d2 < rm) hits[p] |= bit;   // strict <
-                }
+            for (int r = 0; r < 9; r++) {
+                const int rs_r = __shfl_sync(0xffffffffu, rs, r), rl_r = __shfl_sync(0xffffffffu, rl, r);
+                const int ro_r = __shfl_sync(0xffffffffu, roff, r);
+                const int lo = max(ro_r, k0), hi = min(ro_r + rl_r, k0 + Tc);
+                for (int v = lo + lane; v < hi; v += 32) clist[v - k0] = (uint16_t)(rs_r + (v - ro_r));
             }
-            // the particles of a pair are not entries of their own row; whether they are within r_max of each other
-            // (the test is symmetric bit for bit: dx and -dx square to the same number) goes into nlistn
-#pragma unroll
-            for (int p = 0; p < NL_PPI; p++) {
-                const int rel = self[p] - k0;
-                if (self[p] >= 0 && rel >= 0 && rel < Tc) {      // warp-uniform
-                    const unsigned b = 1u << (rel >> 5);
-                    const bool mine = (rel & 31) == lane;
-                    if (p & 1) {   // second particle of its pair: is it a neighbor of the first?
-                        const bool ab = __any_sync(FULL, mine && (hits[p - 1] & b));
-                        if (p == 1) abA = abA || ab; else abB = abB || ab;
-                    }
-                    if (mine) { hits[p & ~1] &= ~b; hits[p | 1] &= ~b; }
-                }
-            }
-#pragma unroll
-            for (int p = 0; p < NL_PPI; p++) cnt[p] += __reduce_add_sync(FULL, __popc(hits[p]));
-            // compact: one warp scan of the per-lane union counts of both pairs gives every lane its positions (l.18-19)
-            unsigned UA = hits[0] | hits[1], UB = hits[2] | hits[3];
-            const int x = __popc(UA) | (__popc(UB) << 16);
-            int inc = x;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int y = __shfl_up_sync(FULL, inc, o);
-                if (lane >= o) inc += y;
-            }
-            const int tot = __shfl_sync(FULL, inc, 31);
-            int atA = totA + ((inc - x) & 0xffff), atB = totB + ((inc - x) >> 16);
-            while (UA) {
-                const int gq = __ffs(UA) - 1;
-                UA &= UA - 1;
-                const unsigned e = ((unsigned)clist[k0 + (gq << 5) + lane] << 2) | ((hits[0] >> gq) & 1u) | (((hits[1] >> gq) & 1u) << 1);
-                if (atA < capA) rowA[atA] = (uint16_t)e;
-                atA++;
-            }
-            while (UB) {
-                const int gq = __ffs(UB) - 1;
-                UB &= UB - 1;
-                const unsigned e = ((unsigned)clist[k0 + (gq << 5) + lane] << 2) | ((hits[2] >> gq) & 1u) | (((hits[3] >> gq) & 1u) << 1);
-                if (atB < capB) rowB[atB] = (uint16_t)e;
-                atB++;
-            }
-            totA += tot & 0xffff;
-            totB += tot >> 16;
-        }
+            for (int v = Tc + lane; v < (ngroups << 5); v += 32) clist[v] = 0;   // dummy: never a hit
+            __syncwarp();
 
+            // ---- 2. every particle of the cell against every candidate ----
+            for (int i0 = part * PPI; i0 < n_c; i0 += wpc * PPI) {
+                float px[PPI], py[PPI], pz[PPI];
+                int gidx[PPI], cnt0[PPI];
+                unsigned hits[PPI];
 #pragma unroll
-        for (int pr = 0; pr < 2; pr++) {
-            if (2 * pr >= nvalid) break;      // warp-uniform
-            const bool two = 2 * pr + 1 < nvalid;
-            uint16_t *row = pr ? rowB : rowA;
-            const int cap = pr ? capB : capA, tot = pr ? totB : totA;
-            const int ab = (pr ? abB : abA) ? 1 : 0;
-            const int ca = cnt[2 * pr] + ab, cbn = cnt[2 * pr + 1] + ab;
-            const int nw = min(tot, cap);
-            // at least 32 entries of 0 end the row: the step kernel stops at the first one it meets
-            // (pad_end is even and the row is 128-byte aligned: one 16-bit store if nw is odd, then 32-bit words)
-            const int pad_end = min(cap, (nw & ~(ROW_PAD - 1)) + 2 * ROW_PAD);
-            const int e0 = (nw + 1) & ~1;
-            if (lane == 0 && e0 != nw && nw < pad_end) row[nw] = 0;
-            if (e0 + 2 * lane < pad_end) reinterpret_cast<uint32_t *>(row)[(e0 >> 1) + lane] = 0u;
-            if (lane == 0) {                                     // l.22
-                const int gi0 = gi_f + 2 * pr;
-                nlistn[gi0] = ca | (ab << 30);                   // bit 30: the two particles of the pair are neighbors
-                if (two) nlistn[gi0 + 1] = cbn;
+                for (int p = 0; p < PPI; p++) {
+                    gidx[p] = -1;
+                    px[p] = py[p] = pz[p] = -1e18f;
+                    cnt0[p] = 0;
+                    hits[p] = 0u;
+                    if (i0 + p < n_c) {
+                        const float4 q = stage[cslot0 + i0 + p];  // same address in all lanes: one broadcast
+                        px[p] = q.x; py[p] = q.y; pz[p] = q.z;
+                        gidx[p] = cg0 + i0 + p;
+                        if (k0 > 0) cnt0[p] = __ldcg(&nlistn[gidx[p]]);
+                    }
+                }
+                // lane l tests candidates l, l+32, ...; bit gq of hits[p] records candidate 32 gq + l (Alg. 3 l.16-17)
+#pragma unroll 2
+                for (int gq = 0; gq < ngroups; gq++) {
+                    const float4 e = stage[clist[(gq << 5) + lane]];
+                    const unsigned bit = 1u << gq;
+#pragma unroll
+                    for (int p = 0; p < PPI; p++) {
+                        const float dx = e.x - px[p], dy = e.y - py[p], dz = e.z - pz[p];
+                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+                        if (d2 < rmax2) hits[p] |= bit;   // strict <
+                    }
+                }
+                // i != j: particle i0+p is candidate self0 + i0 + p; drop that one bit
+#pragma unroll
+                for (int p = 0; p < PPI; p++) {
+                    const int ks = self0 + i0 + p - k0;
+                    if (ks >= 0 && ks < Tc && (ks & 31) == lane) hits[p] &= ~(1u << (ks >> 5));
+                }
+                // compact: warp scan of the per-lane hit counts gives every lane its positions (l.18-19)
+#pragma unroll
+                for (int p = 0; p < PPI; p++) {
+                    if (gidx[p] < 0) continue;   // warp-uniform
+                    const int cn = __popc(hits[p]);
+                    int inc = cn;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int y = __shfl_up_sync(0xffffffffu, inc, o);
+                        if (lane >= o) inc += y;
+                    }
+                    const int total = cnt0[p] + __shfl_sync(0xffffffffu, inc, 31);
+                    int at = cnt0[p] + inc - cn;
+                    uint16_t *row = nlist + (int64_t)gidx[p] * pitch;
+                    unsigned hm = hits[p];
+                    while (hm) {
+                        const int gq = __ffs(hm) - 1;
+                        hm &= hm - 1;
+                        if (at < pitch) row[at] = (uint16_t)(clist[(gq << 5) + lane] << eshift);
+                        at++;
+                    }
+                    const int nw = min(total, pitch);
+                    // at least 32 dummy entries end the row: the force kernel stops at the first one it meets
+                    // (pad_end is even and the row is 128-byte aligned: one 16-bit store if nw is odd, then 32-bit words)
+                    const int pad_end = min(pitch, (nw & ~(ROW_PAD - 1)) + 2 * ROW_PAD);
+                    const int e0 = (nw + 1) & ~1;
+                    if (lane == 0 && e0 != nw && nw < pad_end) row[nw] = 0;
+                    if (e0 + 2 * lane < pad_end) reinterpret_cast<uint32_t *>(row)[(e0 >> 1) + lane] = 0u;
+                    if (lane == 0) nlistn[gidx[p]] = nw;                      // l.22
+                    wmax = max(wmax, total);
+                }
             }
-            wmax_len = max(wmax_len, two ? max(ca, cbn) : ca);
-            // a pair's row is the two rows of its particles: the union must fit in 2 pitch, and (so that row_pitch
-            // >= the longest neighbor set stays true) each set in one pitch
-            wmax_need = max(wmax_need, two ? max(max(ca, cbn), (tot + 1) >> 1) : tot);
         }
     }
-    // longest neighbor set and longest row needed by this build (may exceed the pitch: overflow)
-    if (lane == 0) {
-        if (wmax_len > __ldcg(&flags[FL_MAX_NBRS])) atomicMax(&flags[FL_MAX_NBRS], wmax_len);
-        if (wmax_need > pitch) atomicMax(&flags[FL_OVERFLOWED], wmax_need);
+    // longest row needed by this build (may exceed the pitch: overflow)
+    if (lane == 0 && wmax > __ldcg(&flags[FL_MAX_NBRS])) {
+        atomicMax(&flags[FL_MAX_NBRS], wmax);
+        if (wmax > pitch) atomicMax(&flags[FL_OVERFLOWED], wmax);
     }
 }
 
-template <bool TYPED>
+template <int PPI>
 __global__ void __launch_bounds__(TILE_THREADS) nlist_tile_kernel(ListArgs la, const int *__restrict__ pred)
 {
     if (pred && *pred == 0) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    nlist_tile_body<TYPED>(la, blockIdx.x, smem_raw);
+    nlist_tile_body<PPI>(la, blockIdx.x, smem_raw);
 }
 
 // The whole rebuild in ONE cooperative launch: Algorithm 2 (count, scan, scatter), the reorder into cell
 // order (gather) and Algorithm 3, with grid-wide barriers between the phases.  Inside hb_run_nve's graphs
 // every step carries the rebuild's kernels as early-exit launches; one launch instead of five takes
 // about 4 us off every step (N = 64,000, measured), and the phases lose their launch gaps.
-template <bool TYPED, bool WITH_LIST>
+template <int PPI, bool WITH_LIST>
 __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs ca, GatherArgs ga, int do_sort, ListArgs la,
                                                                     const int *__restrict__ pred)
 {
@@ -374,7 +293,7 @@ __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs 
             __syncthreads();
             const int tile = next_tile;
             if (tile >= la.g.ntiles) break;
-            nlist_tile_body<TYPED>(la, tile, smem_raw);
+            nlist_tile_body<PPI>(la, tile, smem_raw);
             __syncthreads();              // the next tile reuses the staging area (and next_tile)
         }
     }
@@ -387,8 +306,6 @@ static ListArgs make_list_args(hb_system *h, bool copyback)
     la.cell_start = h->cell_start;
     la.pos_build = h->pos_build;
     la.rmax2 = h->r_max * h->r_max;
-    la.rmax2_pair = h->rmax2_pair;
-    la.ntypes = h->ntypes;
     la.pitch = h->row_pitch;
     la.nlist = h->nlist;
     la.nlistn = h->nlistn;
@@ -397,34 +314,35 @@ static ListArgs make_list_args(hb_system *h, bool copyback)
     return la;
 }
 
-// per-type-pair list cutoffs (tunable nlist_pair_rcut) need the table in shared memory
-static bool list_typed(const hb_system *h) { return h->tun.nlist_pair_rcut != 0 && h->ntypes > 1 && h->ntypes <= 8; }
-
 cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback)
 {
     const size_t smem = nlist_smem_bytes(h);
     const unsigned grid = (unsigned)h->geom.ntiles;
     const ListArgs la = make_list_args(h, copyback);
     cudaError_t e;
-#define NL_LAUNCH(TYPED)                                                                                                \
-    e = cudaFuncSetAttribute(nlist_tile_kernel<TYPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);         \
+#define NL_LAUNCH(PPI)                                                                                                  \
+    e = cudaFuncSetAttribute(nlist_tile_kernel<PPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
     if (e != cudaSuccess) return e;                                                                                     \
-    nlist_tile_kernel<TYPED><<<grid, h->tun.nlist_block, smem, h->stream>>>(la, pred);
-    if (list_typed(h)) { NL_LAUNCH(true) } else { NL_LAUNCH(false) }
+    nlist_tile_kernel<PPI><<<grid, h->tun.nlist_block, smem, h->stream>>>(la, pred);
+    switch (h->tun.nlist_ppi) {
+        case 1: NL_LAUNCH(1) break;
+        case 2: NL_LAUNCH(2) break;
+        default: NL_LAUNCH(4) break;
+    }
 #undef NL_LAUNCH
     h->stats.kernel_launches++;
     return cudaGetLastError();
 }
 
 // count + scan + scatter + gather (+ list) in one cooperative launch (see rebuild_coop_kernel)
-template <bool TYPED, bool WITH_LIST>
+template <int PPI, bool WITH_LIST>
 static cudaError_t launch_rebuild_coop_t(hb_system *h, const int *pred)
 {
     const size_t smem = WITH_LIST ? nlist_smem_bytes(h) : 0;
-    cudaError_t e = cudaFuncSetAttribute(rebuild_coop_kernel<TYPED, WITH_LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(rebuild_coop_kernel<PPI, WITH_LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rebuild_coop_kernel<TYPED, WITH_LIST>, TILE_THREADS, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rebuild_coop_kernel<PPI, WITH_LIST>, TILE_THREADS, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorCooperativeLaunchTooLarge;
     // every phase strides over the grid; no more blocks than there is work for or than fit on the device at once
@@ -437,7 +355,7 @@ static cudaError_t launch_rebuild_coop_t(hb_system *h, const int *pred)
     int do_sort = h->tun.cell_sort;
     ListArgs la = make_list_args(h, true);
     void *args[] = {&ca, &ga, &do_sort, &la, (void *)&pred};
-    e = cudaLaunchCooperativeKernel((const void *)rebuild_coop_kernel<TYPED, WITH_LIST>, dim3(grid), dim3(TILE_THREADS), args, smem,
+    e = cudaLaunchCooperativeKernel((const void *)rebuild_coop_kernel<PPI, WITH_LIST>, dim3(grid), dim3(TILE_THREADS), args, smem,
                                     h->stream);
     h->stats.kernel_launches++;
     return e != cudaSuccess ? e : cudaGetLastError();
@@ -445,8 +363,12 @@ static cudaError_t launch_rebuild_coop_t(hb_system *h, const int *pred)
 
 cudaError_t launch_rebuild_coop(hb_system *h, const int *pred, bool with_list)
 {
-    if (!with_list) return launch_rebuild_coop_t<false, false>(h, pred);
-    return list_typed(h) ? launch_rebuild_coop_t<true, true>(h, pred) : launch_rebuild_coop_t<false, true>(h, pred);
+    if (!with_list) return launch_rebuild_coop_t<4, false>(h, pred);
+    switch (h->tun.nlist_ppi) {
+        case 1: return launch_rebuild_coop_t<1, true>(h, pred);
+        case 2: return launch_rebuild_coop_t<2, true>(h, pred);
+        default: return launch_rebuild_coop_t<4, true>(h, pred);
+    }
 }
 
 // ---- accessors: the list BY TAG as CSR ----
@@ -454,11 +376,10 @@ __global__ void nlist_counts_by_tag_kernel(const int *__restrict__ nlistn, const
                                            int *__restrict__ counts)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < N) counts[tag[i]] = nlistn[i] & 0x3fffffff;
+    if (i < N) counts[tag[i]] = nlistn[i];
 }
 
-// One block per tile: slot -> storage index through the same tables, then the pair rows -> tags.  A warp reads the row
-// of a pair 32 entries at a time; an entry goes to the first / second particle's output row if its bit 0 / 1 is set.
+// One block per tile: slot -> storage index through the same tables, then rows -> tags.
 __global__ void __launch_bounds__(TILE_THREADS)
 nlist_fill_by_tag_kernel(TileGeom g, const int *__restrict__ cell_start, const uint16_t *__restrict__ nlist,
                          const int *__restrict__ nlistn, int pitch, const uint32_t *__restrict__ tag,
@@ -476,28 +397,13 @@ nlist_fill_by_tag_kernel(TileGeom g, const int *__restrict__ cell_start, const u
     }
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const unsigned lt = (1u << lane) - 1u;
-    const int npairs = s.d.pair_off[s.d.nrows];
-    for (int P = warp; P < npairs; P += TILE_THREADS / 32) {
-        int gi0, slot0, np;
-        tile_pair(s.d, P, gi0, slot0, np);
-        const uint32_t ta = tag[gi0], tb = np == 2 ? tag[gi0 + 1] : 0u;
-        int64_t oa = row_start[ta], ob = np == 2 ? row_start[tb] : 0;
-        if (np == 2 && (nlistn[gi0] >> 30) & 1) {   // the two particles of the pair are neighbors of each other
-            if (lane == 0) { out[oa] = tb; out[ob] = ta; }
-            oa++; ob++;
-        }
-        const uint16_t *row = nlist + (int64_t)gi0 * pitch;
-        const int cap = np == 2 ? 2 * pitch : pitch;
-        for (int k0 = 0; k0 < cap; k0 += 32) {
-            const unsigned e = k0 + lane < cap ? row[k0 + lane] : 0u;
-            const unsigned ma = __ballot_sync(0xffffffffu, e & 1u), mb = __ballot_sync(0xffffffffu, e & 2u);
-            const uint32_t tj = e ? tag[gidx[e >> 2]] : 0u;
-            if (e & 1u) out[oa + __popc(ma & lt)] = tj;
-            if (e & 2u) out[ob + __popc(mb & lt)] = tj;
-            oa += __popc(ma); ob += __popc(mb);
-            if (__any_sync(0xffffffffu, e == 0u)) break;      // padding: the row is over
-        }
+    for (int q = warp; q < t.nown; q += TILE_THREADS / 32) {
+        int gi, slot;
+        tile_own(s.d, q, gi, slot);
+        const int n = nlistn[gi];
+        const int64_t o = row_start[tag[gi]];
+        const uint16_t *row = nlist + (int64_t)gi * pitch;
+        for (int k = lane; k < n; k += 32) out[o + k] = tag[gidx[row[k] >> g.eshift]];
     }
 }
 

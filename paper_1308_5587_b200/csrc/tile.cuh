@@ -29,10 +29,9 @@ struct TileCtx {
     int nrows;        // own (y, z) rows = ey * ez
 };
 
-// What the kernels need to know about the own particles of a tile (shared memory, rebuilt from cell_start by every
-// block).  PAIR ROWS: the own particles of an own (y, z) row are one contiguous storage range; consecutive particles
-// (2k, 2k + 1) of it form a pair that shares ONE list row (the union of both neighbor sets, see nlist.cu); an odd
-// count leaves the last particle single.
+// What the force kernel needs to know about a tile.  It depends on cell_start only, so the list
+// build writes it once per build (one per tile, in global memory) and the force kernel, which
+// runs every step, just loads it.
 struct TileDesc {
     int nslots;       // 1 + staged particles (1 = nothing staged: the build found the tile too big)
     int nown;         // own particles
@@ -41,9 +40,9 @@ struct TileDesc {
     int own_start[TILE_ROWS_MAX];    // storage index of the first own particle of row r
     int own_off[TILE_ROWS_MAX + 1];  // tile-local number of the first own particle of row r
     int own_slot[TILE_ROWS_MAX];     // its slot
-    int pair_off[TILE_ROWS_MAX + 1]; // tile-local number of the first pair of row r; [nrows] = pairs of the tile
     int pad;
 };
+static_assert(sizeof(TileDesc) == 416, "hb_api.cu sizes the descriptor array with this number");
 
 struct TileShared {
     int hslot[TILE_HMAX + 1];   // first slot of halo cell h
@@ -132,14 +131,9 @@ __device__ __forceinline__ bool tile_tables(const TileGeom &g, const int *__rest
     }
     __syncthreads();
     if (tid == 0) {
-        int run = 0, prun = 0;
+        int run = 0;
         s.d.own_off[0] = 0;
-        s.d.pair_off[0] = 0;
-        for (int r = 0; r < t.nrows; r++) {
-            const int n = s.d.own_off[r + 1];
-            s.d.own_off[r + 1] = run + n; run += n;
-            prun += (n + 1) >> 1; s.d.pair_off[r + 1] = prun;
-        }
+        for (int r = 0; r < t.nrows; r++) { const int n = s.d.own_off[r + 1]; s.d.own_off[r + 1] = run + n; run += n; }
         const float wcell = g.L / (float)g.m, hL = 0.5f * g.L;
         s.d.nslots = t.nslots;
         s.d.nown = run;
@@ -318,19 +312,3 @@ __device__ __forceinline__ void tile_own(const TileDesc &d, int q, int &gi, int 
     gi = d.own_start[r] + off;
     slot = d.own_slot[r] + off;
 }
-
-// pair P of the tile: storage index and slot of its first particle, and how many particles it has (2, or 1 for the
-// last particle of a row with an odd count)
-__device__ __forceinline__ void tile_pair(const TileDesc &d, int P, int &gi0, int &slot0, int &np)
-{
-    int r = 0;
-    while (r + 1 < d.nrows && d.pair_off[r + 1] <= P) r++;
-    const int k = 2 * (P - d.pair_off[r]);
-    gi0 = d.own_start[r] + k;
-    slot0 = d.own_slot[r] + k;
-    np = min(2, d.own_off[r + 1] - d.own_off[r] - k);
-}
-
-// List entries (16 bit): (slot << 2) | m1 << 1 | m0, m0 / m1 = "within r_max of the first / second particle of the
-// pair" at build time; 0 = padding (ends the row).  slot * 16 is the byte offset of the staged position.
-__device__ __forceinline__ unsigned entry_offset(unsigned e) { return (e & 0xfffcu) << 2; }

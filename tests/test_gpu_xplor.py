@@ -63,7 +63,6 @@ def test_xplor_ron_beyond_rcut_is_the_plain_truncated_potential(hb, orc):
     w = CASES["lj_20k"]
     s = wl.make_state(w)
     with hb.System.from_workload(w) as g:
-        g.set_tunable("tpp", 2)          # the thread layout of the smoothed functor: same order of summation in both
         g.set_state(s.pos, s.type, s.vel, s.image)
         g.set_ron_pair([3.0])
         g.build_nlist(0.0, w.r_buff)

@@ -213,6 +213,67 @@ int orc_nlist_cells(const double *pos, int64_t N, double L, double r_max, int m,
     return ORC_OK;
 }
 
+/* NEXT-3: per-type-pair cutoff in the LIST.  The paper gives every pair of types its own r_cut and
+ * builds the list with r_cut + r_buff; the base path uses the single largest cutoff for the list
+ * [reading c2.iii].  [reading t1] With per-pair list cutoffs the definition becomes
+ *   N(i) = { j != i : |minimage(Ri - Rj)| < r_list(type_i, type_j) },  r_list,ab = r_cut,ab + r_buff  (strict <),
+ * rlist[ntypes*ntypes] symmetric.  Definition by testing every pair, ascending j. */
+int orc_nlist_brute_typed(const double *pos, const int32_t *type, int64_t N, double L, int ntypes, const double *rlist,
+                          int32_t *count, const int64_t *row_start, int32_t *nbr)
+{
+    for (int p = 0; p < ntypes * ntypes; p++) if (L < 2.0 * rlist[p]) return ORC_EBOX;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < N; i++) {
+        int32_t n = 0;
+        double d[3];
+        for (int64_t j = 0; j < N; j++) {
+            if (j == i) continue;
+            const double rl = rlist[type[i] * ntypes + type[j]];
+            if (dist2(pos, i, j, L, d) < rl * rl) {
+                if (nbr) nbr[row_start[i] + n] = (int32_t)j;
+                n++;
+            }
+        }
+        count[i] = n;
+    }
+    return ORC_OK;
+}
+
+/* The method's way: Algorithm 3 over the cells of the LARGEST list cutoff (r_max = max rlist: the 27 cells hold every
+ * candidate), line 17 tested against the pair's own r_list. */
+int orc_nlist_cells_typed(const double *pos, const int32_t *type, int64_t N, double L, int ntypes, const double *rlist, int m,
+                          const int32_t *cell, const int64_t *cell_start, const int32_t *cell_members,
+                          int32_t *count, const int64_t *row_start, int32_t *nbr)
+{
+    double r_max = 0.0;
+    for (int p = 0; p < ntypes * ntypes; p++) if (rlist[p] > r_max) r_max = rlist[p];
+    if (m < 3 || L < 2.0 * r_max || L / m < r_max) return ORC_EBOX;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < N; i++) {
+        const int cx = cell[i] % m, cy = (cell[i] / m) % m, cz = cell[i] / (m * m);
+        int32_t n_neigh = 0;
+        for (int a = 0; a < 27; a++) {
+            const int dx = (cx + (a % 3) - 1 + m) % m;
+            const int dy = (cy + ((a / 3) % 3) - 1 + m) % m;
+            const int dz = (cz + (a / 9) - 1 + m) % m;
+            const int64_t dcell = dx + (int64_t)m * (dy + (int64_t)m * dz);
+            const int64_t n_d = cell_start[dcell + 1] - cell_start[dcell];
+            for (int64_t o = 0; o < n_d; o++) {
+                const int64_t j = cell_members[cell_start[dcell] + o];
+                double r[3];
+                const double r2 = dist2(pos, i, j, L, r);
+                const double rl = rlist[type[i] * ntypes + type[j]];
+                if (r2 < rl * rl && i != j) {
+                    if (nbr) nbr[row_start[i] + n_neigh] = (int32_t)j;
+                    n_neigh++;
+                }
+            }
+        }
+        count[i] = n_neigh;
+    }
+    return ORC_OK;
+}
+
 /* ------------------------------------------------------------------ c3 ---- */
 /* [reading c3] Rebuild rule: the list built at R^build stays valid while no
  * particle has moved more than r_buff/2 (PAPER.md:167 only says r_buff exists).

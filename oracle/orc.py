@@ -46,6 +46,8 @@ def lib():
         L.orc_nlist_brute.argtypes = [_dp, C.c_int64, C.c_double, C.c_double, _ip, _vp, _vp]
         L.orc_nlist_brute_sample.argtypes = [_dp, C.c_int64, C.c_double, C.c_double, _lp, C.c_int64, _ip, _vp, _vp]
         L.orc_nlist_cells.argtypes = [_dp, C.c_int64, C.c_double, C.c_double, C.c_int, _ip, _lp, _ip, _ip, _vp, _vp]
+        L.orc_nlist_brute_typed.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, _ip, _vp, _vp]
+        L.orc_nlist_cells_typed.argtypes = [_dp, _ip, C.c_int64, C.c_double, C.c_int, _dp, C.c_int, _ip, _lp, _ip, _ip, _vp, _vp]
         L.orc_max_disp2.restype = C.c_double
         L.orc_max_disp2.argtypes = [_dp, _dp, C.c_int64, C.c_double]
         L.orc_lj_pair.argtypes = [C.c_double] * 4 + [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -177,6 +179,24 @@ def nlist_cells(pos, L, r_max, m=None, cell=None):
     start, members = build_cells(cell, m)
     return _two_pass(lambda c, r, n: lib().orc_nlist_cells(pos, len(pos), float(L), float(r_max), int(m), cell,
                                                            start, members, c, r, n), len(pos))
+
+
+def nlist_brute_typed(pos, typ, L, ntypes, rlist):
+    """Definition of the list with per-type-pair list cutoffs rlist[ntypes*ntypes] (reading t1)."""
+    pos, rlist = _d(pos), _d(rlist).ravel()
+    typ = np.ascontiguousarray(typ, dtype=np.int32)
+    return _two_pass(lambda c, r, n: lib().orc_nlist_brute_typed(pos, typ, len(pos), float(L), int(ntypes), rlist, c, r, n), len(pos))
+
+
+def nlist_cells_typed(pos, typ, L, ntypes, rlist):
+    """Algorithm 2 + 3 over the cells of the largest list cutoff, each pair tested against its own."""
+    pos, rlist = _d(pos), _d(rlist).ravel()
+    typ = np.ascontiguousarray(typ, dtype=np.int32)
+    m = cell_dim(L, float(rlist.max()))
+    cell, _ = cell_index_f64(pos, L, m)
+    start, members = build_cells(cell, m)
+    return _two_pass(lambda c, r, n: lib().orc_nlist_cells_typed(pos, typ, len(pos), float(L), int(ntypes), rlist, int(m), cell,
+                                                                 start, members, c, r, n), len(pos))
 
 
 def max_disp2(pos, pos_build, L):

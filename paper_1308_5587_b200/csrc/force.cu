@@ -191,7 +191,7 @@ struct ForceArgs {
     const int *cell_start;
     const float4 *pos;
     const uint16_t *nlist;
-    int pitch, N, ntypes, pot;
+    int pitch, N, ntypes, pot, dbg;
     const PairParam *params;
     const PairParamX *paramsx;
     float4 *force, *virial;
@@ -313,6 +313,7 @@ lj_tile_kernel(const ForceArgs A)
     const NveArgs &nv = A.nv;
     const bool nve = A.do_nve != 0, drift = nve && nv.kick_drift;
     const bool block0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
+    if (A.dbg & 4) return;
 
     if (threadIdx.x == 0 && g.fast) mbar_init(&s.mbar, 1);
     if (!ONE_TYPE)
@@ -326,7 +327,7 @@ lj_tile_kernel(const ForceArgs A)
     bool fits;
     if (g.fast) {
         fits = force_tile_tables(g, A.cell_start, s);
-        if (fits && threadIdx.x < 32) {
+        if (fits && !(A.dbg & 2) && threadIdx.x < 32) {
             // warp 0 hands the pieces to the TMA unit: one bulk copy per contiguous run of positions
             const int lane = threadIdx.x;
             if (lane == 0) {
@@ -347,7 +348,8 @@ lj_tile_kernel(const ForceArgs A)
         __syncthreads();
         if (fits) tile_stage_positions(g, t, sgen, A.pos, stage, nullptr);
     }
-    const int nown = fits ? s.d.nown : 0;
+    const int nown = (fits && !(A.dbg & 2)) ? s.d.nown : 0;
+    if (A.dbg & 2) return;
 
     const int sub = threadIdx.x % TPP;
     const int ql = threadIdx.x / TPP;            // particle of the pass this thread group works for
@@ -415,7 +417,7 @@ lj_tile_kernel(const ForceArgs A)
             cp_async_wait<PF - 1>();
             Entries<EPL> ent;
             ent.v = ring[0];
-            for (int k = 0; k < A.pitch; k += G) {
+            for (int k = 0; k < ((A.dbg & 1) ? 0 : A.pitch); k += G) {
                 if ((ent.v.x & 0xffffu) == 0u) break;                    // padding: the row is over for this thread
                 cp_async<EPL * 2>(ring + c * ring_stride, row + k + PF * G);   // refill PF iterations ahead (reads past the
                 cp_async_commit();                                       // row's end are harmless: the array has slack)
@@ -530,6 +532,7 @@ static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
     A.N = (int)h->N;
     A.ntypes = h->ntypes;
     A.pot = h->pot;
+    A.dbg = h->tun.dbg;
     A.params = h->params;
     A.paramsx = h->paramsx;
     A.force = h->force;

@@ -227,6 +227,12 @@ int configure_geometry(hb_system *h)
     }
     HB_TRY(choose_tiles(h, 0));
     h->stats.cells_per_axis = m;
+    {   // per-type-pair list cutoffs (tunable nlist_pair_rcut): (r_cut,ab + r_buff)^2, each operation in binary32
+        std::vector<float> t2((size_t)h->ntypes * h->ntypes);
+        for (size_t p = 0; p < t2.size(); p++) { const float r = (float)h->rcut[p] + h->r_buff; t2[p] = r * r; }
+        HB_CK(cudaMemcpyAsync(h->rmax2_pair, t2.data(), t2.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        HB_CK(cudaStreamSynchronize(h->stream));
+    }
     return HB_OK;
 }
 
@@ -805,6 +811,7 @@ int hb_create(hb_system **out, int64_t N, double L, int ntypes, const double *ep
     HB_TRY(dev_alloc_t(h, &h->nlistn, n));
     HB_TRY(dev_alloc_t(h, &h->params, (size_t)ntypes * ntypes));
     HB_TRY(dev_alloc_t(h, &h->paramsx, (size_t)ntypes * ntypes));
+    HB_TRY(dev_alloc_t(h, &h->rmax2_pair, (size_t)ntypes * ntypes));
     HB_TRY(dev_alloc_t(h, &h->flags, (size_t)FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_flags, sizeof(int) * FL_COUNT));
     HB_CK(cudaMallocHost((void **)&h->h_thermo, sizeof(double) * 16));
@@ -847,7 +854,7 @@ int hb_destroy(hb_system *h)
     dev_free(h, h->bk_tstate);
     void *ptrs[] = {h->posbuf[0], h->posbuf[1], h->vel, h->force, h->virial, h->image, h->tag, h->rtag, h->pos_build, h->vel2,
                     h->force2, h->virial2, h->image2, h->tag2, h->bk_pos, h->bk_vel, h->bk_force, h->bk_virial, h->bk_image,
-                    h->bk_tag, h->params, h->paramsx, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
+                    h->bk_tag, h->params, h->paramsx, h->rmax2_pair, h->cell_count, h->cell_local, h->cell_start, h->cell_id, h->cell_rank, h->perm,
                     h->scan_sums, h->scan_tmp, h->nlist, h->nlistn, h->keys, h->keys2, h->sperm, h->sperm2, h->radix_counts,
                     h->flags, h->thermo_part};
     for (void *p : ptrs) dev_free(h, p);
@@ -1370,6 +1377,8 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "force_block")) return &h->tun.force_block;
     if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
     if (!strcmp(name, "nlist_block")) return &h->tun.nlist_block;
+    if (!strcmp(name, "nlist_pair_rcut")) return &h->tun.nlist_pair_rcut;
+    if (!strcmp(name, "dbg")) return &h->tun.dbg;
     if (!strcmp(name, "tile_x")) return &h->tun.tile_x;
     if (!strcmp(name, "tile_y")) return &h->tun.tile_y;
     if (!strcmp(name, "tile_z")) return &h->tun.tile_z;
@@ -1400,7 +1409,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     else if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z) ok = value >= 0 && value <= 16;
     else if (slot == &h->tun.stage_cap) ok = value >= 0 && value <= 65535;
     else if (slot == &h->tun.row_pitch) ok = value >= 0 && value <= 4096;
-    else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve || slot == &h->tun.thermo_every) ok = value == 0 || value == 1;
+    else if (slot == &h->tun.cell_sort || slot == &h->tun.fuse_nve || slot == &h->tun.thermo_every || slot == &h->tun.nlist_pair_rcut) ok = value == 0 || value == 1;
     else if (slot == &h->tun.coop_rebuild) ok = value >= -1 && value <= 2;
     else if (slot == &h->tun.coop_blocks) ok = value >= 1 && value <= 8;
     else if (slot == &h->tun.grow_pct) ok = value >= 0 && value <= 400;
@@ -1410,6 +1419,7 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     *slot = value;
     destroy_graphs(h);
     if (slot == &h->tun.row_pitch && value > 0) HB_TRY(ensure_rows(h, value));
+    if (slot == &h->tun.nlist_pair_rcut) h->nlist_valid = false;
     if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z || slot == &h->tun.stage_cap) {
         h->nlist_valid = false;
         if (h->m > 0) HB_TRY(choose_tiles(h, 0));

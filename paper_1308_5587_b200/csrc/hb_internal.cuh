@@ -71,6 +71,7 @@ struct Tunables {
     int force_block = 0;   // threads per block of the force kernel (128 or 256; 0 = one pass over the tile's particles if possible)
     int nlist_ppi = 4;     // particles tested per candidate load
     int nlist_block = 256; // threads per block of the stand-alone list kernel (128 or 256)
+    int nlist_pair_rcut = 0;   // 1: the list keeps pair (i, j) iff d < r_cut(type i, type j) + r_buff (reading t1); 0: one r_max (reading c2.iii)
     int tile_x = 0, tile_y = 0, tile_z = 0;   // 0 = chosen from m and the SM count
     int stage_cap = 0;     // 0 = estimated from the density
     int row_pitch = 0;
@@ -83,6 +84,7 @@ struct Tunables {
     int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 100;
+    int dbg = 0;           // timing experiments only (wrong physics): 1 skip the pair loop, 2 stop after the tile tables, 4 empty kernel
 };
 
 enum { TS_XI = 0, TS_ETA = 1, TS_KSUM = 2, TS_LBASE = 3, TS_COUNT = 8 };
@@ -131,6 +133,7 @@ struct hb_system {
     int bk_cur = 0, bk_parity = 0;
     PairParam *params = nullptr;
     PairParamX *paramsx = nullptr;
+    float *rmax2_pair = nullptr;   // [ntypes^2] (r_cut,ab + r_buff)^2 for the typed list build
 
     float4 *pos() const { return posbuf[cur]; }
 

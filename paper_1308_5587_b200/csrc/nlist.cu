@@ -49,6 +49,8 @@ struct ListArgs {
     const int *cell_start;
     const float4 *pos_build;
     float rmax2;
+    const float *rmax2_pair;   // TYPED: [ntypes * ntypes] squared list cutoffs (r_cut,ab + r_buff)^2 (tunable nlist_pair_rcut)
+    int ntypes;
     int pitch;
     uint16_t *nlist;
     int *nlistn, *flags;
@@ -56,7 +58,7 @@ struct ListArgs {
 };
 
 // Algorithm 3 for one tile, by one block of TILE_THREADS threads
-template <int PPI>
+template <int PPI, bool TYPED>
 __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int tile, unsigned char *smem_raw)
 {
     const TileGeom &g = la.g;
@@ -70,11 +72,14 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
     const CopyBack &cb = la.cb;
     const int eshift = g.eshift;
     __shared__ TileShared s;
+    __shared__ float s_rm2[TYPED ? 64 : 1];     // per-type-pair list cutoffs (reading t1): ntypes <= 8, else the single cutoff
     float4 *stage = reinterpret_cast<float4 *>(smem_raw);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint16_t *clist = reinterpret_cast<uint16_t *>(smem_raw + (size_t)g.cap * 16) + warp * NL_CLIST;
 
     if (tile == 0 && threadIdx.x == 0) flags[FL_BUILDS] += 1;
+    if (TYPED)
+        for (int k = threadIdx.x; k < la.ntypes * la.ntypes; k += blockDim.x) s_rm2[k] = la.rmax2_pair[k];
     TileCtx t;
     tile_decode(g, tile, t);
     const bool fits = tile_tables(g, cell_start, t, s, flags);
@@ -151,15 +156,18 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                 float px[PPI], py[PPI], pz[PPI];
                 int gidx[PPI], cnt0[PPI];
                 unsigned hits[PPI];
+                const float *rmrow[PPI];
 #pragma unroll
                 for (int p = 0; p < PPI; p++) {
                     gidx[p] = -1;
                     px[p] = py[p] = pz[p] = -1e18f;
                     cnt0[p] = 0;
                     hits[p] = 0u;
+                    rmrow[p] = s_rm2;
                     if (i0 + p < n_c) {
                         const float4 q = stage[cslot0 + i0 + p];  // same address in all lanes: one broadcast
                         px[p] = q.x; py[p] = q.y; pz[p] = q.z;
+                        if (TYPED) rmrow[p] = s_rm2 + __float_as_int(q.w) * la.ntypes;
                         gidx[p] = cg0 + i0 + p;
                         if (k0 > 0) cnt0[p] = __ldcg(&nlistn[gidx[p]]);
                     }
@@ -173,7 +181,8 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                     for (int p = 0; p < PPI; p++) {
                         const float dx = e.x - px[p], dy = e.y - py[p], dz = e.z - pz[p];
                         const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                        if (d2 < rmax2) hits[p] |= bit;   // strict <
+                        const float rm = TYPED ? rmrow[p][__float_as_int(e.w)] : rmax2;
+                        if (d2 < rm) hits[p] |= bit;   // strict <
                     }
                 }
                 // i != j: particle i0+p is candidate self0 + i0 + p; drop that one bit
@@ -223,19 +232,19 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
     }
 }
 
-template <int PPI>
+template <int PPI, bool TYPED>
 __global__ void __launch_bounds__(TILE_THREADS) nlist_tile_kernel(ListArgs la, const int *__restrict__ pred)
 {
     if (pred && *pred == 0) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    nlist_tile_body<PPI>(la, blockIdx.x, smem_raw);
+    nlist_tile_body<PPI, TYPED>(la, blockIdx.x, smem_raw);
 }
 
 // The whole rebuild in ONE cooperative launch: Algorithm 2 (count, scan, scatter), the reorder into cell
 // order (gather) and Algorithm 3, with grid-wide barriers between the phases.  Inside hb_run_nve's graphs
 // every step carries the rebuild's kernels as early-exit launches; one launch instead of five takes
 // about 4 us off every step (N = 64,000, measured), and the phases lose their launch gaps.
-template <int PPI, bool WITH_LIST>
+template <int PPI, bool WITH_LIST, bool TYPED>
 __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs ca, GatherArgs ga, int do_sort, ListArgs la,
                                                                     const int *__restrict__ pred)
 {
@@ -293,11 +302,14 @@ __global__ void __launch_bounds__(TILE_THREADS, 4) rebuild_coop_kernel(CellArgs 
             __syncthreads();
             const int tile = next_tile;
             if (tile >= la.g.ntiles) break;
-            nlist_tile_body<PPI>(la, tile, smem_raw);
+            nlist_tile_body<PPI, TYPED>(la, tile, smem_raw);
             __syncthreads();              // the next tile reuses the staging area (and next_tile)
         }
     }
 }
+
+// per-type-pair list cutoffs (tunable nlist_pair_rcut): the table must fit the kernel's shared array
+static bool list_typed(const hb_system *h) { return h->tun.nlist_pair_rcut != 0 && h->ntypes > 1 && h->ntypes <= 8; }
 
 static ListArgs make_list_args(hb_system *h, bool copyback)
 {
@@ -306,6 +318,8 @@ static ListArgs make_list_args(hb_system *h, bool copyback)
     la.cell_start = h->cell_start;
     la.pos_build = h->pos_build;
     la.rmax2 = h->r_max * h->r_max;
+    la.rmax2_pair = h->rmax2_pair;
+    la.ntypes = h->ntypes;
     la.pitch = h->row_pitch;
     la.nlist = h->nlist;
     la.nlistn = h->nlistn;
@@ -320,14 +334,15 @@ cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback)
     const unsigned grid = (unsigned)h->geom.ntiles;
     const ListArgs la = make_list_args(h, copyback);
     cudaError_t e;
-#define NL_LAUNCH(PPI)                                                                                                  \
-    e = cudaFuncSetAttribute(nlist_tile_kernel<PPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);           \
+#define NL_LAUNCH(PPI, TYPED)                                                                                           \
+    e = cudaFuncSetAttribute(nlist_tile_kernel<PPI, TYPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
     if (e != cudaSuccess) return e;                                                                                     \
-    nlist_tile_kernel<PPI><<<grid, h->tun.nlist_block, smem, h->stream>>>(la, pred);
-    switch (h->tun.nlist_ppi) {
-        case 1: NL_LAUNCH(1) break;
-        case 2: NL_LAUNCH(2) break;
-        default: NL_LAUNCH(4) break;
+    nlist_tile_kernel<PPI, TYPED><<<grid, h->tun.nlist_block, smem, h->stream>>>(la, pred);
+    if (list_typed(h)) { NL_LAUNCH(4, true) }      // the typed build comes with four particles per candidate load only
+    else switch (h->tun.nlist_ppi) {
+        case 1: NL_LAUNCH(1, false) break;
+        case 2: NL_LAUNCH(2, false) break;
+        default: NL_LAUNCH(4, false) break;
     }
 #undef NL_LAUNCH
     h->stats.kernel_launches++;
@@ -335,14 +350,14 @@ cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback)
 }
 
 // count + scan + scatter + gather (+ list) in one cooperative launch (see rebuild_coop_kernel)
-template <int PPI, bool WITH_LIST>
+template <int PPI, bool WITH_LIST, bool TYPED>
 static cudaError_t launch_rebuild_coop_t(hb_system *h, const int *pred)
 {
     const size_t smem = WITH_LIST ? nlist_smem_bytes(h) : 0;
-    cudaError_t e = cudaFuncSetAttribute(rebuild_coop_kernel<PPI, WITH_LIST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(rebuild_coop_kernel<PPI, WITH_LIST, TYPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rebuild_coop_kernel<PPI, WITH_LIST>, TILE_THREADS, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rebuild_coop_kernel<PPI, WITH_LIST, TYPED>, TILE_THREADS, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorCooperativeLaunchTooLarge;
     // every phase strides over the grid; no more blocks than there is work for or than fit on the device at once
@@ -355,7 +370,7 @@ static cudaError_t launch_rebuild_coop_t(hb_system *h, const int *pred)
     int do_sort = h->tun.cell_sort;
     ListArgs la = make_list_args(h, true);
     void *args[] = {&ca, &ga, &do_sort, &la, (void *)&pred};
-    e = cudaLaunchCooperativeKernel((const void *)rebuild_coop_kernel<PPI, WITH_LIST>, dim3(grid), dim3(TILE_THREADS), args, smem,
+    e = cudaLaunchCooperativeKernel((const void *)rebuild_coop_kernel<PPI, WITH_LIST, TYPED>, dim3(grid), dim3(TILE_THREADS), args, smem,
                                     h->stream);
     h->stats.kernel_launches++;
     return e != cudaSuccess ? e : cudaGetLastError();
@@ -363,11 +378,12 @@ static cudaError_t launch_rebuild_coop_t(hb_system *h, const int *pred)
 
 cudaError_t launch_rebuild_coop(hb_system *h, const int *pred, bool with_list)
 {
-    if (!with_list) return launch_rebuild_coop_t<4, false>(h, pred);
+    if (!with_list) return launch_rebuild_coop_t<4, false, false>(h, pred);
+    if (list_typed(h)) return launch_rebuild_coop_t<4, true, true>(h, pred);
     switch (h->tun.nlist_ppi) {
-        case 1: return launch_rebuild_coop_t<1, true>(h, pred);
-        case 2: return launch_rebuild_coop_t<2, true>(h, pred);
-        default: return launch_rebuild_coop_t<4, true>(h, pred);
+        case 1: return launch_rebuild_coop_t<1, true, false>(h, pred);
+        case 2: return launch_rebuild_coop_t<2, true, false>(h, pred);
+        default: return launch_rebuild_coop_t<4, true, false>(h, pred);
     }
 }
 

@@ -41,7 +41,8 @@ def pair_dist(pos, L, keys):
 
 
 def assert_nlist_equal(pos64, L, r_max, rs_ref, nbr_ref, rs_gpu, nbr_gpu):
-    """Set equality of (i, j) entries except pairs within BAND of r_max; no duplicates, no self.
+    """Set equality of (i, j) entries except pairs within BAND of r_max (a number, or a function of the int64 keys
+    i * 2^32 + j that returns each pair's own list cutoff); no duplicates, no self.
     Exact at any size: rows whose (length, sum j, sum j^2) differ are compared entry by entry as sets,
     all the others must make identical sorted key arrays."""
     kr = np.sort(rows_as_keys(rs_ref, nbr_ref))
@@ -65,8 +66,9 @@ def assert_nlist_equal(pos64, L, r_max, rs_ref, nbr_ref, rs_gpu, nbr_gpu):
     for name, ks in (("missing from GPU list", only_ref), ("extra in GPU list", only_gpu)):
         if len(ks):
             d = pair_dist(pos64, L, ks)
-            bad = np.abs(d - r_max) > BAND
-            assert not bad.any(), f"{bad.sum()} pairs {name}, e.g. d = {d[bad][:3]} vs r_max = {r_max}"
+            rm = r_max(ks) if callable(r_max) else r_max       # per-type-pair list cutoffs: a function of the (i, j) keys
+            bad = np.abs(d - rm) > BAND
+            assert not bad.any(), f"{bad.sum()} pairs {name}, e.g. d = {d[bad][:3]} vs r_max = {rm if np.isscalar(rm) else rm[bad][:3]}"
     return len(only_ref) + len(only_gpu)
 
 

@@ -122,6 +122,17 @@ HB_API int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type,
 HB_API int hb_get_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, int32_t *image,
                  uint32_t *order, int on_device);
 
+/* The same in binary64 (the double-precision build).  With the tunable
+ * "precision" = 64 the force sums and the integration run in binary64 on these arrays (kept by tag); the cell list and
+ * the neighbor list are still built from the positions rounded to binary32.  With "precision" = 32 hb_set_state_f64
+ * rounds its input and hb_get_state_f64 widens the binary32 state.  pos_xyz, vel_xyz [N][3], image [N][3] (nullable),
+ * BY TAG.  hb_get_forces_f64: f_xyz_u [N][4], virial6 [N][6] (nullable) of the binary64 sums; HB_ESTATE unless
+ * "precision" = 64. */
+HB_API int hb_set_state_f64(hb_system *h, const double *pos_xyz, const int32_t *type, const double *vel_xyz,
+                     const int32_t *image, int on_device);
+HB_API int hb_get_state_f64(hb_system *h, double *pos_xyz, double *vel_xyz, int32_t *image, int on_device);
+HB_API int hb_get_forces_f64(hb_system *h, double *f_xyz_u, double *virial6, int on_device);
+
 /* Per-type-pair cutoffs r_cut,ab [ntypes*ntypes].  The list is
  * built with the largest of them (reading c2.iii); the force applies each. */
 HB_API int hb_set_rcut_pair(hb_system *h, const double *rcut);
@@ -242,6 +253,12 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *                    2 = graphs with a conditional IF node around the rebuild
  *                    3 = the launches of mode 1 issued one by one, no graph (for profilers)
  *   "graph_steps"    steps per graph launch
+ *   "nlist_pair_rcut" 1 = the list keeps pair (i, j) iff d < r_cut(type i, type j) + r_buff (reading t1; up to 8 types);
+ *                    0 = (default) one list cutoff, the largest (reading c2.iii)
+ *   "precision"      32 = (default) binary32 arithmetic (the paper's GPU precision);
+ *                    64 = force sums and velocity Verlet in binary64 (NVE, hb_step_nve / hb_run_nve one step per host
+ *                         iteration; hb_run_nvt / hb_run_langevin return HB_EINVAL): what the arithmetic conserves
+ *                         (Table 2), not a fast path
  */
 HB_API int hb_set_tunable(hb_system *h, const char *name, int value);
 HB_API int hb_get_tunable(hb_system *h, const char *name, int *value);

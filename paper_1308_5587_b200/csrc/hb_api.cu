@@ -741,6 +741,34 @@ int run_chunk(hb_system *h, float dt, int n)
     return HB_ENOMEM;
 }
 
+// The binary64 variant (tunable precision = 64, dp.cu): one velocity-Verlet step per host iteration.
+int dp_run(hb_system *h, double dt, int64_t nsteps, int64_t sort_period)
+{
+    if (h->ens.mode != 0) { h->err = "the binary64 variant integrates NVE only"; return HB_EINVAL; }
+    if (!h->dp.have) HB_TRY(dp_from_f32(h));
+    for (int64_t s = 0; s < nsteps; s++) {
+        if (sort_period > 0 && (h->since_sort < 0 || h->since_sort >= sort_period)) {
+            if (!h->nlist_valid) HB_TRY(build_nlist_sync(h));
+            HB_TRY(sort_internal(h));
+            h->since_sort = 0;
+        }
+        if (!h->nlist_valid) { HB_TRY(build_nlist_sync(h)); h->dp.forces_valid = false; }
+        if (!h->dp.forces_valid) HB_TRY(dp_force(h));
+        HB_TRY(dp_nve(h, dt, 1));
+        h->moved = true;
+        h->forces_valid = false;          // the binary32 force arrays are not kept up in this mode
+        HB_TRY(set_flag(h, FL_CHECK, 0));
+        HB_CK(launch_disp_check(h));      // reading c3 on the binary32 mirror
+        HB_TRY(read_flags(h));
+        if (h->h_flags[FL_CHECK]) HB_TRY(build_nlist_sync(h));
+        HB_TRY(dp_force(h));
+        HB_TRY(dp_nve(h, dt, 2));
+        h->stats.steps++;
+        if (h->since_sort >= 0) h->since_sort++;
+    }
+    return HB_OK;
+}
+
 // accessor staging area, owned by the handle (grows, never shrinks)
 int ensure_stage(hb_system *h, size_t bytes)
 {
@@ -845,6 +873,7 @@ int hb_destroy(hb_system *h)
     if (!h) return HB_EINVAL;
     cudaStreamSynchronize(h->stream);
     destroy_graphs(h);
+    dp_release(h);
     dev_free(h, h->acc_stage);
     dev_free(h, h->acc_counts);
     dev_free(h, h->acc_rows);
@@ -901,6 +930,80 @@ int hb_set_state(hb_system *h, const float *pos_xyz, const int32_t *type, const 
         h->err = "a particle type is outside 0 .. ntypes-1";
         return HB_EINVAL;
     }
+    h->dp.have = h->dp.forces_valid = false;
+    if (h->tun.precision == 64) HB_TRY(dp_from_f32(h));
+    return HB_OK;
+}
+
+int hb_set_state_f64(hb_system *h, const double *pos_xyz, const int32_t *type, const double *vel_xyz, const int32_t *image, int on_device)
+{
+    HB_NEED(h);
+    if (!pos_xyz || !vel_xyz) { h->err = "pos_xyz and vel_xyz are required"; return HB_EINVAL; }
+    const size_t N = (size_t)h->N;
+    // staging: [pos f64 | vel f64 | type | image | pos f32 | vel f32]
+    HB_TRY(ensure_stage(h, N * (24 + 24 + 4 + 12 + 12 + 12)));
+    char *base = (char *)h->acc_stage;
+    double *dpos = (double *)base, *dvel = (double *)(base + N * 24);
+    int32_t *dtype = (int32_t *)(base + N * 48), *dimg = (int32_t *)(base + N * 52);
+    float *fpos = (float *)(base + N * 64), *fvel = (float *)(base + N * 76);
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    HB_CK(cudaMemcpyAsync(dpos, pos_xyz, N * 24, kind, h->stream));
+    HB_CK(cudaMemcpyAsync(dvel, vel_xyz, N * 24, kind, h->stream));
+    if (type) HB_CK(cudaMemcpyAsync(dtype, type, N * 4, kind, h->stream));
+    if (image) HB_CK(cudaMemcpyAsync(dimg, image, N * 12, kind, h->stream));
+    HB_TRY(dp_set_state(h, dpos, dvel, image ? dimg : nullptr, fpos, fvel));
+    HB_CK(launch_pack_state(h, fpos, type ? dtype : nullptr, fvel, image ? dimg : nullptr));
+    HB_TRY(read_flags(h));
+    h->have_state = true;
+    h->cells_valid = h->nlist_valid = h->forces_valid = h->bk_valid = false;
+    h->moved = true;
+    h->since_sort = -1;
+    h->lang_steps = 0;
+    HB_CK(cudaMemsetAsync(h->tstate, 0, sizeof(double) * TS_COUNT, h->stream));
+    if (h->h_flags[FL_BADTYPE] || h->h_flags[FL_BAD]) {
+        const bool badtype = h->h_flags[FL_BADTYPE] != 0;
+        HB_TRY(set_flag(h, FL_BADTYPE, 0));
+        HB_TRY(set_flag(h, FL_BAD, 0));
+        h->have_state = false;
+        h->dp.have = false;
+        h->err = badtype ? "a particle type is outside 0 .. ntypes-1" : "a position is outside [-L/2, L/2) or not finite";
+        return badtype ? HB_EINVAL : HB_ENAN;
+    }
+    return HB_OK;
+}
+
+int hb_get_state_f64(hb_system *h, double *pos_xyz, double *vel_xyz, int32_t *image, int on_device)
+{
+    HB_NEED(h);
+    if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    if (!h->dp.have || h->tun.precision != 64) HB_TRY(dp_from_f32(h));     // binary32 mode: the binary32 state, widened
+    const size_t N = (size_t)h->N;
+    if (on_device) return dp_get(h, pos_xyz, vel_xyz, image, nullptr, nullptr, nullptr, nullptr);
+    HB_TRY(ensure_stage(h, N * 60));
+    char *base = (char *)h->acc_stage;
+    double *dpos = (double *)base, *dvel = (double *)(base + N * 24);
+    int32_t *dimg = (int32_t *)(base + N * 48);
+    HB_TRY(dp_get(h, pos_xyz ? dpos : nullptr, vel_xyz ? dvel : nullptr, image ? dimg : nullptr, nullptr, nullptr, nullptr, nullptr));
+    if (pos_xyz) HB_CK(cudaMemcpyAsync(pos_xyz, dpos, N * 24, cudaMemcpyDeviceToHost, h->stream));
+    if (vel_xyz) HB_CK(cudaMemcpyAsync(vel_xyz, dvel, N * 24, cudaMemcpyDeviceToHost, h->stream));
+    if (image) HB_CK(cudaMemcpyAsync(image, dimg, N * 12, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
+    return HB_OK;
+}
+
+int hb_get_forces_f64(hb_system *h, double *f_xyz_u, double *virial6, int on_device)
+{
+    HB_NEED(h);
+    if (h->tun.precision != 64) { h->err = "hb_get_forces_f64 needs the binary64 variant (tunable precision = 64)"; return HB_ESTATE; }
+    if (!h->dp.forces_valid) { h->err = "forces are stale: call hb_compute_lj first"; return HB_ESTATE; }
+    const size_t N = (size_t)h->N;
+    if (on_device) return dp_get(h, nullptr, nullptr, nullptr, f_xyz_u, virial6, nullptr, nullptr);
+    HB_TRY(ensure_stage(h, N * 80));
+    double *sf = (double *)h->acc_stage, *sv = (double *)((char *)h->acc_stage + N * 32);
+    HB_TRY(dp_get(h, nullptr, nullptr, nullptr, f_xyz_u ? sf : nullptr, virial6 ? sv : nullptr, nullptr, nullptr));
+    if (f_xyz_u) HB_CK(cudaMemcpyAsync(f_xyz_u, sf, N * 32, cudaMemcpyDeviceToHost, h->stream));
+    if (virial6) HB_CK(cudaMemcpyAsync(virial6, sv, N * 48, cudaMemcpyDeviceToHost, h->stream));
+    HB_CK(cudaStreamSynchronize(h->stream));
     return HB_OK;
 }
 
@@ -909,8 +1012,10 @@ int hb_get_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, in
     HB_NEED(h);
     if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
     const size_t N = (size_t)h->N;
+    const bool dp = h->tun.precision == 64 && h->dp.have;     // the image flags of this mode live with the binary64 arrays
     if (on_device) {
-        HB_CK(launch_unpack_state(h, pos_xyz, type, vel_xyz, image));
+        HB_CK(launch_unpack_state(h, pos_xyz, type, vel_xyz, dp ? nullptr : image));
+        if (dp && image) HB_TRY(dp_get(h, nullptr, nullptr, image, nullptr, nullptr, nullptr, nullptr));
         if (order) HB_CK(cudaMemcpyAsync(order, h->tag, N * 4, cudaMemcpyDeviceToDevice, h->stream));
         return HB_OK;
     }
@@ -921,7 +1026,8 @@ int hb_get_state(hb_system *h, float *pos_xyz, int32_t *type, float *vel_xyz, in
     int32_t *stype = (int32_t *)(base + N * 24);
     int32_t *simg = (int32_t *)(base + N * 28);
     HB_CK(launch_unpack_state(h, pos_xyz ? spos : nullptr, type ? stype : nullptr, vel_xyz ? svel : nullptr,
-                              image ? simg : nullptr));
+                              (image && !dp) ? simg : nullptr));
+    if (dp && image) HB_TRY(dp_get(h, nullptr, nullptr, simg, nullptr, nullptr, nullptr, nullptr));
     if (pos_xyz) HB_CK(cudaMemcpyAsync(pos_xyz, spos, N * 12, cudaMemcpyDeviceToHost, h->stream));
     if (vel_xyz) HB_CK(cudaMemcpyAsync(vel_xyz, svel, N * 12, cudaMemcpyDeviceToHost, h->stream));
     if (type) HB_CK(cudaMemcpyAsync(type, stype, N * 4, cudaMemcpyDeviceToHost, h->stream));
@@ -996,7 +1102,7 @@ int hb_set_mass(hb_system *h, const float *mass, int on_device)
         return HB_EINVAL;
     }
     h->bk_valid = false;
-    return HB_OK;
+    return dp_sync_mass(h);
 }
 
 int hb_get_mass(hb_system *h, float *mass, int on_device)
@@ -1075,6 +1181,10 @@ int hb_compute_lj(hb_system *h, int shift_mode)
         destroy_graphs(h);     // the captured step kernels are instantiated for one pair functor
         HB_TRY(upload_params(h));
     }
+    if (h->tun.precision == 64) {
+        if (!h->dp.have) HB_TRY(dp_from_f32(h));
+        return dp_force(h);
+    }
     HB_CK(launch_force(h, nullptr));
     h->forces_valid = true;
     return HB_OK;
@@ -1086,6 +1196,7 @@ int hb_step_nve(hb_system *h, double dt)
     Range nvtx_range("hb_step_nve");
     if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
     if (h->m == 0) HB_TRY(configure_geometry(h));
+    if (h->tun.precision == 64) return dp_run(h, (double)(float)dt, 1, 0);
     return step_sync(h, (float)dt);
 }
 
@@ -1095,6 +1206,11 @@ static int run_md(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, 
     if (nsteps < 0 || sort_period < 0) return HB_EINVAL;
     if (h->m == 0) HB_TRY(configure_geometry(h));
     h->ens = ens;
+    if (h->tun.precision == 64) {
+        const int rcd = dp_run(h, (double)(float)dt, nsteps, sort_period);
+        h->ens = Ensemble{};
+        return rcd;
+    }
     int64_t done = 0;
     int rc = HB_OK;
     while (done < nsteps && rc == HB_OK) {
@@ -1183,6 +1299,21 @@ int hb_thermo(hb_system *h, hb_thermo_t *out)
     Range nvtx_range("hb_thermo");
     if (!out) return HB_EINVAL;
     if (!h->have_state) { h->err = "no state"; return HB_ESTATE; }
+    if (h->tun.precision == 64) {
+        if (h->m == 0) HB_TRY(configure_geometry(h));
+        if (!h->dp.have) HB_TRY(dp_from_f32(h));
+        if (!h->nlist_valid) { HB_TRY(build_nlist_sync(h)); h->dp.forces_valid = false; }
+        if (!h->dp.forces_valid) HB_TRY(dp_force(h));
+        double t[11];
+        HB_TRY(dp_thermo(h, t));
+        out->K = t[0];
+        out->U = t[1];
+        for (int a = 0; a < 6; a++) out->W[a] = t[2 + a];
+        out->px = t[8]; out->py = t[9]; out->pz = t[10];
+        const double V = (double)h->L * (double)h->L * (double)h->L;
+        out->P = (2.0 * out->K + out->W[0] + out->W[3] + out->W[5]) / (3.0 * V);
+        return HB_OK;
+    }
     if (!h->forces_valid) {       // U, W and P come from the per-particle arrays of the last force evaluation
         if (h->m == 0) HB_TRY(configure_geometry(h));
         HB_TRY(ensure_forces(h));
@@ -1247,8 +1378,19 @@ int hb_get_nlist(hb_system *h, int64_t *row_start, uint32_t *nbr_tags, int on_de
 int hb_get_forces(hb_system *h, float *f_xyz_u, float *virial6, int on_device)
 {
     HB_NEED(h);
-    if (!h->forces_valid) { h->err = "forces are stale: call hb_compute_lj first"; return HB_ESTATE; }
     const size_t N = (size_t)h->N;
+    if (h->tun.precision == 64) {      // the binary64 sums, rounded
+        if (!h->dp.forces_valid) { h->err = "forces are stale: call hb_compute_lj first"; return HB_ESTATE; }
+        if (on_device) return dp_get(h, nullptr, nullptr, nullptr, nullptr, nullptr, f_xyz_u, virial6);
+        HB_TRY(ensure_stage(h, N * 40));
+        float *sf = (float *)h->acc_stage, *sv = (float *)((char *)h->acc_stage + N * 16);
+        HB_TRY(dp_get(h, nullptr, nullptr, nullptr, nullptr, nullptr, f_xyz_u ? sf : nullptr, virial6 ? sv : nullptr));
+        if (f_xyz_u) HB_CK(cudaMemcpyAsync(f_xyz_u, sf, N * 16, cudaMemcpyDeviceToHost, h->stream));
+        if (virial6) HB_CK(cudaMemcpyAsync(virial6, sv, N * 24, cudaMemcpyDeviceToHost, h->stream));
+        HB_CK(cudaStreamSynchronize(h->stream));
+        return HB_OK;
+    }
+    if (!h->forces_valid) { h->err = "forces are stale: call hb_compute_lj first"; return HB_ESTATE; }
     if (on_device) {
         HB_CK(launch_unpack_forces(h, f_xyz_u, virial6));
         return HB_OK;
@@ -1379,6 +1521,7 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "nlist_block")) return &h->tun.nlist_block;
     if (!strcmp(name, "nlist_pair_rcut")) return &h->tun.nlist_pair_rcut;
     if (!strcmp(name, "dbg")) return &h->tun.dbg;
+    if (!strcmp(name, "precision")) return &h->tun.precision;
     if (!strcmp(name, "tile_x")) return &h->tun.tile_x;
     if (!strcmp(name, "tile_y")) return &h->tun.tile_y;
     if (!strcmp(name, "tile_z")) return &h->tun.tile_z;
@@ -1415,11 +1558,17 @@ int hb_set_tunable(hb_system *h, const char *name, int value)
     else if (slot == &h->tun.grow_pct) ok = value >= 0 && value <= 400;
     else if (slot == &h->tun.graph_mode) ok = value >= 0 && value <= 3;
     else if (slot == &h->tun.graph_steps) ok = value >= 1 && value <= 2000;
+    else if (slot == &h->tun.precision) ok = value == 32 || value == 64;
     if (!ok) { h->err = std::string("value out of range for tunable ") + name; return HB_EINVAL; }
     *slot = value;
     destroy_graphs(h);
     if (slot == &h->tun.row_pitch && value > 0) HB_TRY(ensure_rows(h, value));
     if (slot == &h->tun.nlist_pair_rcut) h->nlist_valid = false;
+    if (slot == &h->tun.precision) {
+        h->dp.have = h->dp.forces_valid = false;
+        h->forces_valid = false;
+        if (value == 64 && h->have_state) HB_TRY(dp_from_f32(h));
+    }
     if (slot == &h->tun.tile_x || slot == &h->tun.tile_y || slot == &h->tun.tile_z || slot == &h->tun.stage_cap) {
         h->nlist_valid = false;
         if (h->m > 0) HB_TRY(choose_tiles(h, 0));

@@ -84,6 +84,7 @@ struct Tunables {
     int coop_rebuild = -1; // -1: 2 below 200,000 particles, else 1 (measured on B200); 1: Algorithm 2 + reorder as ONE cooperative kernel, then the list kernel; 2: the list too; 0: five launches
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 100;
+    int precision = 32;    // 64: the binary64 variant of the force sums and the integration (dp.cu)
     int dbg = 0;           // timing experiments only (wrong physics): 1 skip the pair loop, 2 stop after the tile tables, 4 empty kernel
 };
 
@@ -190,6 +191,14 @@ struct hb_system {
     std::map<int64_t, GraphEntry> graphs;
     float graph_dt = 0;
 
+    // binary64 variant (tunable precision = 64): arrays BY TAG
+    struct Dp {
+        void *x = nullptr, *v = nullptr, *f = nullptr, *pairs = nullptr;   // double4 [N]: (x, y, z, -), (vx, vy, vz, m), (Fx, Fy, Fz, U_i); pair table
+        double *vir = nullptr, *out = nullptr;                             // [N][6]; reduction result
+        int *img = nullptr;                                                // [3][N]
+        bool have = false, forces_valid = false;
+    } dp;
+
     // accessor scratch (host <-> device staging of hb_set_state / hb_get_state / hb_get_forces / hb_get_nlist)
     void *acc_stage = nullptr;
     size_t acc_cap = 0;
@@ -271,6 +280,16 @@ cudaError_t launch_sfc_keys(hb_system *h);
 cudaError_t launch_radix_sort(hb_system *h, int key_bits);  // keys/sperm -> sorted in keys/sperm
 cudaError_t launch_gather_state(hb_system *h);              // by sperm into the scratch set (positions into pos_build)
 cudaError_t launch_rtag(hb_system *h);
+// dp.cu: the binary64 variant
+int dp_ensure(hb_system *h);
+void dp_release(hb_system *h);
+int dp_from_f32(hb_system *h);
+int dp_sync_mass(hb_system *h);
+int dp_force(hb_system *h);
+int dp_nve(hb_system *h, double dt, int what /* 1: half kick + drift, 2: half kick */);
+int dp_set_state(hb_system *h, const double *pos, const double *vel, const int32_t *image, float *pos_f, float *vel_f);
+int dp_get(hb_system *h, double *pos, double *vel, int32_t *image, double *f4, double *vir6, float *f4_f, float *vir6_f);
+int dp_thermo(hb_system *h, double *out11);
 // peaks.cu
 int measure_peak(hb_system *h, const char *which, double *value);
 // accessors

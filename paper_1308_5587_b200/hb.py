@@ -24,7 +24,7 @@ HB_POT_LJ, HB_POT_GAUSS, HB_POT_YUKAWA, HB_POT_MORSE = 0, 1, 2, 3
 POTS = {"lj": HB_POT_LJ, "gauss": HB_POT_GAUSS, "yukawa": HB_POT_YUKAWA, "morse": HB_POT_MORSE}
 _ERR_NAMES = {-1: "HB_EINVAL", -2: "HB_ECUDA", -3: "HB_ENOMEM", -4: "HB_EBOX", -5: "HB_ESTATE", -6: "HB_ENAN"}
 
-EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_rcut_pair", "hb_set_ron_pair",
+EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_state_f64", "hb_get_state_f64", "hb_get_forces_f64", "hb_set_rcut_pair", "hb_set_ron_pair",
            "hb_set_pair_potential", "hb_set_mass", "hb_get_mass", "hb_build_cells",
            "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_run_nvt", "hb_run_langevin",
            "hb_get_thermostat", "hb_set_thermostat", "hb_sort",
@@ -71,6 +71,9 @@ def load():
     L.hb_destroy.argtypes = [vp]
     L.hb_set_state.argtypes = [vp, vp, vp, vp, vp, i32]
     L.hb_get_state.argtypes = [vp, vp, vp, vp, vp, vp, i32]
+    L.hb_set_state_f64.argtypes = [vp, vp, vp, vp, vp, i32]
+    L.hb_get_state_f64.argtypes = [vp, vp, vp, vp, i32]
+    L.hb_get_forces_f64.argtypes = [vp, vp, vp, i32]
     L.hb_set_rcut_pair.argtypes = [vp, vp]
     L.hb_set_ron_pair.argtypes = [vp, vp]
     L.hb_set_pair_potential.argtypes = [vp, i32, vp]
@@ -116,7 +119,7 @@ def _ptr(a, dtype):
         return None, None
     if _is_torch(a):
         import torch
-        want = {np.float32: torch.float32, np.int32: torch.int32, np.uint32: torch.int32, np.int64: torch.int64}[dtype]
+        want = {np.float32: torch.float32, np.float64: torch.float64, np.int32: torch.int32, np.uint32: torch.int32, np.int64: torch.int64}[dtype]
         if a.dtype != want or not a.is_contiguous() or not a.is_cuda:
             raise TypeError(f"torch argument must be a contiguous CUDA tensor of {want}")
         return C.c_void_p(a.data_ptr()), 1
@@ -231,6 +234,29 @@ class System:
         im, d4 = _ptr(image, np.int32)
         o, d5 = _ptr(order, np.uint32)
         self._ck(self._lib.hb_get_state(self._h, p, t, v, im, o, _where(d1, d2, d3, d4, d5)))
+
+    # ---- the binary64 variant (tunable precision = 64) ----
+    def set_state_f64(self, pos, type=None, vel=None, image=None):
+        if vel is None:
+            vel = np.zeros((self.N, 3), dtype=np.float64)
+        p, d1 = _ptr(pos, np.float64)
+        t, d2 = _ptr(type, np.int32)
+        v, d3 = _ptr(vel, np.float64)
+        im, d4 = _ptr(image, np.int32)
+        self._ck(self._lib.hb_set_state_f64(self._h, p, t, v, im, _where(d1, d2, d3, d4)))
+
+    def get_state_f64(self):
+        """dict(pos, vel float64 [N][3], image int32 [N][3]) BY TAG."""
+        o = dict(pos=np.empty((self.N, 3), np.float64), vel=np.empty((self.N, 3), np.float64), image=np.empty((self.N, 3), np.int32))
+        self._ck(self._lib.hb_get_state_f64(self._h, *(o[k].ctypes.data_as(C.c_void_p) for k in ("pos", "vel", "image")), 0))
+        return o
+
+    def get_forces_f64(self, virial=True):
+        """(F_xyz_U float64[N][4], W float64[N][6] or None) BY TAG, of the binary64 sums."""
+        f = np.empty((self.N, 4), np.float64)
+        w = np.empty((self.N, 6), np.float64) if virial else None
+        self._ck(self._lib.hb_get_forces_f64(self._h, f.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p) if virial else None, 0))
+        return f, w
 
     # ---- the hot path ----
     def set_rcut_pair(self, rcut):

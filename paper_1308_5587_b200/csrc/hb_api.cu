@@ -587,11 +587,7 @@ int backup_state(hb_system *h)
         HB_TRY(dev_alloc_t(h, &h->bk_image, 3 * N));
         HB_TRY(dev_alloc_t(h, &h->bk_tag, N));
     }
-    HB_CK(cudaMemcpyAsync(h->bk_pos, h->pos(), N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->bk_vel, h->vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->bk_image, h->image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->bk_tag, h->tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->bk_tstate, h->tstate, sizeof(double) * TS_COUNT, cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(launch_state_copy(h, false));
     h->bk_cur = h->cur;
     h->bk_parity = h->parity;
     h->bk_valid = true;
@@ -600,14 +596,9 @@ int backup_state(hb_system *h)
 
 int restore_state(hb_system *h)
 {
-    const size_t N = (size_t)h->N;
     h->cur = h->bk_cur;
     h->parity = h->bk_parity;
-    HB_CK(cudaMemcpyAsync(h->pos(), h->bk_pos, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->vel, h->bk_vel, N * sizeof(float4), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->image, h->bk_image, 3 * N * sizeof(int), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->tag, h->bk_tag, N * sizeof(uint32_t), cudaMemcpyDeviceToDevice, h->stream));
-    HB_CK(cudaMemcpyAsync(h->tstate, h->bk_tstate, sizeof(double) * TS_COUNT, cudaMemcpyDeviceToDevice, h->stream));
+    HB_CK(launch_state_copy(h, true));
     HB_CK(launch_rtag(h));
     HB_TRY(clear_need_flags(h));
     // forces and virials are not saved: the rebuild that follows a restore changes the order, they are recomputed
@@ -1222,7 +1213,9 @@ static int run_md(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, 
         }
         int64_t n = std::min<int64_t>(h->tun.graph_steps, nsteps - done);
         if (sort_period > 0) n = std::min<int64_t>(n, sort_period - h->since_sort);
-        if (n < h->tun.graph_steps) {          // a remainder: the largest power of two that fits (graphs exist for those)
+        if (n < h->tun.graph_steps && !h->graphs.count(n) && h->graphs.size() >= 24 && h->tun.graph_mode != 0 && h->tun.graph_mode != 3) {
+            // a remainder runs as ONE chunk with a graph of exactly its length, captured the first time that length is
+            // met and kept; once two dozen lengths are cached, the largest power of two that fits (those exist)
             int64_t p2 = 1;
             while (2 * p2 <= n) p2 *= 2;
             n = p2;

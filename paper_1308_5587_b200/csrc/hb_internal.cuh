@@ -275,6 +275,7 @@ size_t force_smem_bytes(const hb_system *h);
 cudaError_t launch_nve(hb_system *h, const NveArgs &a);
 cudaError_t launch_disp_check(hb_system *h);
 cudaError_t launch_thermo(hb_system *h);
+cudaError_t launch_state_copy(hb_system *h, bool restore);   // chunk backup of hb_run_nve (restore: the way back)
 // sort.cu
 cudaError_t launch_sfc_keys(hb_system *h);
 cudaError_t launch_radix_sort(hb_system *h, int key_bits);  // keys/sperm -> sorted in keys/sperm

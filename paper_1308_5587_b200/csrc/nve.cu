@@ -207,3 +207,33 @@ cudaError_t launch_mass(hb_system *h, const float *mass_in, float *mass_out)
     mass_kernel<<<(unsigned)cdiv(h->N, 256), 256, 0, h->stream>>>(h->vel, h->tag, (int)h->N, mass_in, mass_out, h->flags);
     return cudaGetLastError();
 }
+
+// The state a chunk of hb_run_nve can be rolled back to (positions, velocities, image flags, tags, thermostat state):
+// ONE kernel instead of five device-to-device copies (a chunk of 20 steps is 600 us; five copy launches were 15 of them).
+__global__ void __launch_bounds__(256)
+state_copy_kernel(const float4 *__restrict__ pos, const float4 *__restrict__ vel, const int *__restrict__ image,
+                  const uint32_t *__restrict__ tag, const double *__restrict__ ts, int N, float4 *__restrict__ pos_o,
+                  float4 *__restrict__ vel_o, int *__restrict__ image_o, uint32_t *__restrict__ tag_o, double *__restrict__ ts_o)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < TS_COUNT) ts_o[i] = ts[i];
+    if (i >= N) return;
+    pos_o[i] = pos[i];
+    vel_o[i] = vel[i];
+    image_o[i] = image[i];
+    image_o[N + i] = image[N + i];
+    image_o[2 * (int64_t)N + i] = image[2 * (int64_t)N + i];
+    tag_o[i] = tag[i];
+}
+
+cudaError_t launch_state_copy(hb_system *h, bool restore)
+{
+    const unsigned grid = (unsigned)cdiv(h->N, 256);
+    if (!restore)
+        state_copy_kernel<<<grid, 256, 0, h->stream>>>(h->pos(), h->vel, h->image, h->tag, h->tstate, (int)h->N, h->bk_pos, h->bk_vel,
+                                                       h->bk_image, h->bk_tag, h->bk_tstate);
+    else
+        state_copy_kernel<<<grid, 256, 0, h->stream>>>(h->bk_pos, h->bk_vel, h->bk_image, h->bk_tag, h->bk_tstate, (int)h->N, h->pos(),
+                                                       h->vel, h->image, h->tag, h->tstate);
+    return cudaGetLastError();
+}

@@ -334,7 +334,7 @@ int dp_force(hb_system *h)
     A.vir = h->dp.vir;
     A.flags = h->flags;
     const size_t smem = (size_t)h->geom.cap * 4;
-    HB_CK(cudaFuncSetAttribute(dp_force_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    HB_CK(cudaFuncSetAttribute(dp_force_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_attr(h)));
     dp_force_kernel<<<(unsigned)h->geom.ntiles, TILE_THREADS, smem, h->stream>>>(A);
     HB_CK(cudaGetLastError());
     h->stats.kernel_launches++;

@@ -542,7 +542,7 @@ static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
     if (nve) A.nv = *nve;
     cudaError_t e;
 #define LJ_LAUNCH(ONE)                                                                                                      \
-    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, FN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);        \
+    e = cudaFuncSetAttribute(lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, FN>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_attr(h));        \
     if (e != cudaSuccess) return e;                                                                                         \
     lj_tile_kernel<TPP, EPL, ONE, THERMO, SCALED, FN><<<grid, force_block_of(h), smem, h->stream>>>(A);
     if (h->ntypes == 1) { LJ_LAUNCH(true) } else { LJ_LAUNCH(false) }

@@ -115,7 +115,7 @@ int stage_cap_max(const hb_system *h)
     // what is left of the opt-in shared memory after the static tables (TileShared and the scan scratch, < 4 KB) and
     // the larger of the two kernels' extras beside the staging area itself (both functions count cap * 16 bytes)
     const size_t extra = std::max(nlist_smem_bytes(h), force_smem_bytes(h)) - (size_t)h->geom.cap * 16;
-    const int64_t left = (int64_t)h->smem_max - 4096 - (int64_t)extra;
+    const int64_t left = (int64_t)h->smem_max - 8192 - (int64_t)extra;      // smem_attr(): the dynamic shared memory a launch may ask for
     return (int)std::max<int64_t>(64, std::min<int64_t>(65535, left / 16));
 }
 

@@ -224,6 +224,11 @@ struct hb_system {
 
 static inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is state of the FUNCTION, shared by every handle and host thread of the
+// process: it is always set to the same value (all the opt-in shared memory but 8 KB for the kernels' static tables,
+// which is also what stage_cap_max budgets with), so that concurrent handles cannot lower it under each other.
+static inline int smem_attr(const hb_system *h) { return h->smem_max - 8192; }
+
 // threads per particle of the step kernel actually launched (the smoothed functor exists in the default layout only)
 static inline int force_tpp(const hb_system *h) { return (h->shift_mode == HB_XPLOR || h->pot != HB_POT_LJ) ? 2 : h->tun.tpp; }
 

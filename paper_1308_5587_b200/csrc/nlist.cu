@@ -335,7 +335,7 @@ cudaError_t launch_nlist(hb_system *h, const int *pred, bool copyback)
     const ListArgs la = make_list_args(h, copyback);
     cudaError_t e;
 #define NL_LAUNCH(PPI, TYPED)                                                                                           \
-    e = cudaFuncSetAttribute(nlist_tile_kernel<PPI, TYPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
+    e = cudaFuncSetAttribute(nlist_tile_kernel<PPI, TYPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_attr(h));    \
     if (e != cudaSuccess) return e;                                                                                     \
     nlist_tile_kernel<PPI, TYPED><<<grid, h->tun.nlist_block, smem, h->stream>>>(la, pred);
     if (list_typed(h)) { NL_LAUNCH(4, true) }      // the typed build comes with four particles per candidate load only
@@ -354,7 +354,7 @@ template <int PPI, bool WITH_LIST, bool TYPED>
 static cudaError_t launch_rebuild_coop_t(hb_system *h, const int *pred)
 {
     const size_t smem = WITH_LIST ? nlist_smem_bytes(h) : 0;
-    cudaError_t e = cudaFuncSetAttribute(rebuild_coop_kernel<PPI, WITH_LIST, TYPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(rebuild_coop_kernel<PPI, WITH_LIST, TYPED>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_attr(h));
     if (e != cudaSuccess) return e;
     int per_sm = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rebuild_coop_kernel<PPI, WITH_LIST, TYPED>, TILE_THREADS, smem);
@@ -465,7 +465,7 @@ cudaError_t launch_nlist_counts_by_tag(hb_system *h, int *counts)
 cudaError_t launch_nlist_fill_by_tag(hb_system *h, const int64_t *row_start, uint32_t *out)
 {
     const size_t smem = (size_t)h->geom.cap * 4;
-    cudaError_t e = cudaFuncSetAttribute(nlist_fill_by_tag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(nlist_fill_by_tag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_attr(h));
     if (e != cudaSuccess) return e;
     nlist_fill_by_tag_kernel<<<(unsigned)h->geom.ntiles, TILE_THREADS, smem, h->stream>>>(
         h->geom, h->cell_start, h->nlist, h->nlistn, h->row_pitch, h->tag, row_start, out, h->flags);

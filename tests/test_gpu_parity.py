@@ -459,3 +459,40 @@ def test_overflow_inside_a_graph_chunk_is_redone(hb):
     assert abs(Ea - Eb) <= 2e-4 * K0 and abs(Ea - Ea0) <= 5e-3 * K0 and abs(Eb - Eb0) <= 5e-3 * K0, (Ea, Eb, Ea0, K0)
     for t in (ta, tb):
         assert max(abs(t["px"]), abs(t["py"]), abs(t["pz"])) / N < 1e-5
+
+
+def test_two_handles_from_two_host_threads(hb):
+    """Nothing in the library is process-global: two systems, each created, driven and read by its own host thread on
+    its own CUDA stream (ctypes releases the GIL during the calls), give bit for bit what each gives alone."""
+    import threading
+    import torch
+    cfgs = [CASES["lj_20k"], wl.scaled(wl.CONFIGS["ka_1m"], 10_001)]
+
+    def drive(w, out, key, stream):
+        s = wl.make_state(w)
+        with hb.System(w.N, w.L, w.ntypes, w.eps, w.sigma, stream=stream) as g:
+            g.set_rcut_pair(w.rcut)
+            g.set_state(s.pos, s.type, s.vel, s.image)
+            g.build_nlist(0.0, w.r_buff)
+            g.compute_lj(w.shift)
+            for _ in range(3):
+                g.run_nve(w.dt, 37, 20)
+                rs, nbr = g.get_nlist()
+            st = g.get_state()
+            f4, w6 = g.get_forces()
+            out[key] = (st["pos"].copy(), st["vel"].copy(), f4.copy(), w6.copy(), rs.copy(), g.thermo())
+
+    alone, together = {}, {}
+    for k, w in enumerate(cfgs):
+        drive(w, alone, k, torch.cuda.current_stream().cuda_stream)
+    streams = [torch.cuda.Stream() for _ in cfgs]
+    threads = [threading.Thread(target=drive, args=(w, together, k, streams[k].cuda_stream)) for k, w in enumerate(cfgs)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert set(together) == {0, 1}
+    for k in (0, 1):
+        for a, b in zip(alone[k][:5], together[k][:5]):
+            assert np.array_equal(a, b)
+        assert alone[k][5] == together[k][5]

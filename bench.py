@@ -201,8 +201,11 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="skip the short N=1M measurement")
     ap.add_argument("--tune", default="", help="comma list name=value of hb tunables")
+    ap.add_argument("--n", type=int, default=0, help="run the config's fluid at another particle number (scaling studies)")
     args = ap.parse_args()
     w = wl.CONFIGS[args.config]
+    if args.n > 0:
+        w = wl.scaled(w, args.n)
     if args.impl == "reference":
         run_reference(args, w)
         return

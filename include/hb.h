@@ -255,6 +255,8 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *   "graph_steps"    steps per graph launch
  *   "nlist_pair_rcut" 1 = the list keeps pair (i, j) iff d < r_cut(type i, type j) + r_buff (reading t1; up to 8 types);
  *                    0 = (default) one list cutoff, the largest (reading c2.iii)
+ *   "dbg"            timing experiments only (the physics is WRONG with it): 1 = the step kernel skips its pair loop,
+ *                    2 = it stops after the tile tables, 4 = it returns at once (latency breakdown)
  *   "precision"      32 = (default) binary32 arithmetic (the paper's GPU precision);
  *                    64 = force sums and velocity Verlet in binary64 (NVE, hb_step_nve / hb_run_nve one step per host
  *                         iteration; hb_run_nvt / hb_run_langevin return HB_EINVAL): what the arithmetic conserves

@@ -346,7 +346,12 @@ def main():
 
     # ---- end to end through the C ABI with HOST buffers ----
     s_now = g.get_state()
-    pos_h, vel_h, typ_h, img_h = (np.ascontiguousarray(s_now[k]) for k in ("pos", "vel", "type", "image"))
+    def pinned(a):      # page-locked host buffers (the copies in and out of the timed call are DMA transfers)
+        t = torch.empty(a.shape, dtype={np.dtype(np.float32): torch.float32, np.dtype(np.int32): torch.int32}[a.dtype]).pin_memory()
+        v = t.numpy()
+        v[...] = a
+        return v, t
+    (pos_h, _p0), (vel_h, _p1), (typ_h, _p2), (img_h, _p3) = (pinned(np.ascontiguousarray(s_now[k])) for k in ("pos", "vel", "type", "image"))
     Ke = max(1, min(args.steps, 2000))
     g.set_state(pos_h, typ_h, vel_h, img_h)
     g.run_nve(w.dt, Ke, w.sort_period)                           # rehearsal: the timed call below repeats it
@@ -364,7 +369,7 @@ def main():
     e2e = {"value": world * Ke / el, "unit": UNIT, "steps_per_call": Ke, "h2d_bytes_per_step": w.N * 40 / Ke,
            "d2h_bytes_per_step": (w.N * 40 + 96) / Ke, "h2d_bytes_per_call": w.N * 40, "d2h_bytes_per_call": w.N * 40 + 96,
            "graph_builds_in_timed_region": g.stats()["graph_builds"] - builds_e,
-           "note": "hb_set_state(host) + hb_run_nve + hb_get_state(host) + hb_thermo, wall clock"}
+           "note": "hb_set_state(pinned host buffers) + hb_run_nve + hb_get_state(pinned host buffers) + hb_thermo, wall clock"}
     g.close()
 
     also = {}

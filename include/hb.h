@@ -8,7 +8,10 @@
  *      reused until a particle has moved more than r_buff/2
  *   -> Lennard-Jones pair force, energy and virial per particle
  *   -> velocity-Verlet NVE half-steps with image flags
- *   +  periodic space-filling-curve sort of the particles.
+ *   +  periodic space-filling-curve sort of the particles
+ *   +   XPLOR smoothing, Nose-Hoover and Langevin integration,
+ *      Gaussian / Yukawa / Morse pair functors, per-particle mass,
+ *      per-type-pair list cutoffs and a binary64 variant.
  *
  * Every step runs in CUDA kernels; there is no CPU fallback.  One GPU, one
  * stream, no collectives.  Citations are PAPER.md:<line>; "reading" refers to
@@ -22,7 +25,10 @@
  *   - Tables are row-major [ntypes][ntypes] and must be symmetric.
  *   - L, eps, sigma, r_cut, r_buff, dt are taken as double and rounded ONCE to
  *     binary32; all device arithmetic is binary32 (the paper's GPU precision,
- *     PAPER.md:308); hb_thermo accumulates in binary64.
+ *     PAPER.md:308) unless the tunable "precision" is 64; hb_thermo accumulates
+ *     in binary64.
+ *   - A handle is not thread-safe; different handles may be used from different
+ *     host threads at the same time.
  *   - Work is enqueued on the cudaStream_t given to hb_create.  Calls that
  *     return data to the host synchronise that stream; the others may not.
  *   - Pointers passed in are caller-owned and never retained.  `on_device`

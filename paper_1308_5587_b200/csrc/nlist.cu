@@ -100,8 +100,13 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
         }
     }
     if (!fits) return;
-    tile_stage_positions_by_cell(g, t, s, pos_build, stage, nullptr);
-    __syncthreads();
+    __shared__ alignas(8) uint64_t stage_bar;
+    if (g.fast) {
+        tile_stage_positions_bulk(g, t, s, pos_build, stage, &stage_bar);
+    } else {
+        tile_stage_positions_by_cell(g, t, s, pos_build, stage, nullptr);
+        __syncthreads();
+    }
 
     int wmax = 0;
     const int ncell_own = t.ex * t.ey * t.ez;

@@ -19,6 +19,39 @@
 #pragma once
 #include "hb_internal.cuh"
 
+// TMA bulk copy global -> shared (UBLKCP), completion counted in bytes on an mbarrier: one instruction moves a whole
+// piece of the halo (a contiguous run of positions), no per-particle instruction at all.
+__device__ __forceinline__ void mbar_inval(uint64_t *bar)
+{
+    asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     (unsigned)__cvta_generic_to_shared(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
+
+
 struct TileCtx {
     int x0, y0, z0;   // first own cell
     int ex, ey, ez;   // own extent in cells (clipped tile)
@@ -265,6 +298,47 @@ __device__ __forceinline__ void tile_stage_positions_by_cell(const TileGeom &g, 
                 }
         }
     }
+}
+
+// The same result for the FAST geometry with the TMA unit: consecutive halo cells of a row that are consecutive in the
+// cell-ordered position array (all of them, unless the row wraps around the box) go as ONE bulk copy, issued by the
+// thread that owns the halo row; then the tiles whose halo touches a face of the box fix the periodic image in place.
+// `bar` is a shared-memory mbarrier used for this one staging (initialised and invalidated here).
+__device__ __forceinline__ void tile_stage_positions_bulk(const TileGeom &g, const TileCtx &t, const TileShared &s,
+                                                          const float4 *__restrict__ pos, float4 *__restrict__ stage, uint64_t *bar)
+{
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        stage[0] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+        mbar_expect_tx(bar, (unsigned)(t.nslots - 1) * 16u);
+    }
+    __syncthreads();
+    const int hrows = t.hy * t.hz;
+    for (int r = threadIdx.x; r < hrows; r += blockDim.x) {
+        const int h0 = r * t.hx;
+        int first = h0;                                   // first cell of the running piece
+        for (int h = h0; h < h0 + t.hx; h++) {
+            const bool last = h + 1 == h0 + t.hx;
+            const int cnt_h = s.hslot[h + 1] - s.hslot[h];
+            if (last || s.hg[h + 1] != s.hg[h] + cnt_h) {     // the piece ends with cell h
+                const int len = s.hslot[h + 1] - s.hslot[first];
+                if (len > 0) bulk_g2s(stage + s.hslot[first], pos + s.hg[first], (unsigned)len * 16u, bar);
+                first = h + 1;
+            }
+        }
+    }
+    mbar_wait(bar, 0);
+    const bool fix = t.x0 <= 1 || t.x0 + t.ex >= g.m - 1 || t.y0 <= 1 || t.y0 + t.ey >= g.m - 1 || t.z0 <= 1 || t.z0 + t.ez >= g.m - 1;
+    if (fix) {
+        const float L = g.L, hL = 0.5f * g.L, cx = s.d.cx, cy = s.d.cy, cz = s.d.cz;
+        for (int sl = 1 + threadIdx.x; sl < t.nslots; sl += blockDim.x) {
+            float4 p = stage[sl];
+            p.x = tile_image(p.x, cx, L, hL); p.y = tile_image(p.y, cy, L, hL); p.z = tile_image(p.z, cz, L, hL);
+            stage[sl] = p;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) mbar_inval(bar);
 }
 
 // The same staging from the tables the list build left behind (fast geometry only): per slot one

@@ -196,28 +196,36 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                     const int ks = self0 + i0 + p - k0;
                     if (ks >= 0 && ks < Tc && (ks & 31) == lane) hits[p] &= ~(1u << (ks >> 5));
                 }
-                // compact: warp scan of the per-lane hit counts gives every lane its positions (l.18-19)
+                // compact: warp scans of the per-lane hit counts give every lane its positions (l.18-19); the counts of
+                // two particles share one scan (16 bits each: a chunk has at most 1024 candidates)
+                int at[PPI], total[PPI];
 #pragma unroll
-                for (int p = 0; p < PPI; p++) {
-                    if (gidx[p] < 0) continue;   // warp-uniform
-                    const int cn = __popc(hits[p]);
-                    int inc = cn;
+                for (int p = 0; p < PPI; p += 2) {
+                    const int x = __popc(hits[p]) | (p + 1 < PPI ? __popc(hits[p + 1]) << 16 : 0);
+                    int inc = x;
 #pragma unroll
                     for (int o = 1; o < 32; o <<= 1) {
                         const int y = __shfl_up_sync(0xffffffffu, inc, o);
                         if (lane >= o) inc += y;
                     }
-                    const int total = cnt0[p] + __shfl_sync(0xffffffffu, inc, 31);
-                    int at = cnt0[p] + inc - cn;
+                    const int tot = __shfl_sync(0xffffffffu, inc, 31), exc = inc - x;   // no borrow: inclusive >= own, field by field
+                    at[p] = cnt0[p] + (exc & 0xffff);
+                    total[p] = cnt0[p] + (tot & 0xffff);
+                    if (p + 1 < PPI) { at[p + 1] = cnt0[p + 1] + (exc >> 16); total[p + 1] = cnt0[p + 1] + (tot >> 16); }
+                }
+#pragma unroll
+                for (int p = 0; p < PPI; p++) {
+                    if (gidx[p] < 0) continue;   // warp-uniform
                     uint16_t *row = nlist + (int64_t)gidx[p] * pitch;
                     unsigned hm = hits[p];
+                    int a = at[p];
                     while (hm) {
                         const int gq = __ffs(hm) - 1;
                         hm &= hm - 1;
-                        if (at < pitch) row[at] = (uint16_t)(clist[(gq << 5) + lane] << eshift);
-                        at++;
+                        if (a < pitch) row[a] = (uint16_t)(clist[(gq << 5) + lane] << eshift);
+                        a++;
                     }
-                    const int nw = min(total, pitch);
+                    const int nw = min(total[p], pitch);
                     // at least 32 dummy entries end the row: the force kernel stops at the first one it meets
                     // (pad_end is even and the row is 128-byte aligned: one 16-bit store if nw is odd, then 32-bit words)
                     const int pad_end = min(pitch, (nw & ~(ROW_PAD - 1)) + 2 * ROW_PAD);
@@ -225,7 +233,7 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                     if (lane == 0 && e0 != nw && nw < pad_end) row[nw] = 0;
                     if (e0 + 2 * lane < pad_end) reinterpret_cast<uint32_t *>(row)[(e0 >> 1) + lane] = 0u;
                     if (lane == 0) nlistn[gidx[p]] = nw;                      // l.22
-                    wmax = max(wmax, total);
+                    wmax = max(wmax, total[p]);
                 }
             }
         }

@@ -178,9 +178,10 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                     }
                 }
                 // lane l tests candidates l, l+32, ...; bit gq of hits[p] records candidate 32 gq + l (Alg. 3 l.16-17)
+                const uint16_t *const clist_lane = clist + lane;
 #pragma unroll 2
                 for (int gq = 0; gq < ngroups; gq++) {
-                    const float4 e = stage[clist[(gq << 5) + lane]];
+                    const float4 e = stage[clist_lane[gq << 5]];
                     const unsigned bit = 1u << gq;
 #pragma unroll
                     for (int p = 0; p < PPI; p++) {
@@ -218,12 +219,22 @@ __device__ __forceinline__ void nlist_tile_body(const ListArgs &la, const int ti
                     if (gidx[p] < 0) continue;   // warp-uniform
                     uint16_t *row = nlist + (int64_t)gidx[p] * pitch;
                     unsigned hm = hits[p];
-                    int a = at[p];
-                    while (hm) {
-                        const int gq = __ffs(hm) - 1;
-                        hm &= hm - 1;
-                        if (a < pitch) row[a] = (uint16_t)(clist[(gq << 5) + lane] << eshift);
-                        a++;
+                    uint16_t *w = row + at[p];
+                    const uint16_t *cl = clist + lane;
+                    if (total[p] <= pitch) {       // warp-uniform, the rule: no bound to test per entry
+                        while (hm) {
+                            const int gq = __ffs(hm) - 1;
+                            hm &= hm - 1;
+                            *w++ = (uint16_t)(cl[gq << 5] << eshift);
+                        }
+                    } else {                       // the row overflows: keep what fits, the host grows the rows
+                        int a = at[p];
+                        while (hm) {
+                            const int gq = __ffs(hm) - 1;
+                            hm &= hm - 1;
+                            if (a < pitch) row[a] = (uint16_t)(cl[gq << 5] << eshift);
+                            a++;
+                        }
                     }
                     const int nw = min(total[p], pitch);
                     // at least 32 dummy entries end the row: the force kernel stops at the first one it meets

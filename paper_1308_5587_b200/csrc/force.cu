@@ -65,6 +65,13 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// Depth of the per-thread ring of list copies (cp.async): how many iterations ahead a thread asks for its list entries.
+// Measured on B200 (us per time step, N = 64,000 / 10^6 / Kob-Andersen 2^20): depth 4: 27.4 / 237.7 / 400; 2: 27.1 / 229.2 /
+// 380; 1: 27.3 / 227.1 / 368.  The kernel is bound by the shared-memory pipe, and every copy of a warp costs 16 wavefronts
+// (its 32 lanes read 16 different rows): the copies issued past the end of a row are pure cost, and a shallower ring
+// leaves more shared memory for resident blocks.
+constexpr int LIST_PF = 2;
+
 struct Acc {
     float fx, fy, fz, u, wxx, wxy, wxz, wyy, wyz, wzz;
 };
@@ -269,7 +276,7 @@ lj_tile_kernel(const ForceArgs A)
     const int nthreads = blockDim.x;
     const int PPB = nthreads / TPP;              // particles per block per pass
     constexpr int G = TPP * EPL;                 // entries per particle per iteration
-    constexpr int PF = 4;                        // depth of the ring of list copies
+    constexpr int PF = LIST_PF;                  // depth of the ring of list copies
     using EntryVec = decltype(Entries<EPL>::v);
 
     // dynamic shared memory: staging area | pair table | ring | own data of a pass (v, x, x_build; one buffer: a
@@ -487,7 +494,7 @@ size_t force_smem_bytes(const hb_system *h)
     // and forces of a pass
     return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? ((sizeof(PairParam) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
            (h->ntypes > 1 ? ((sizeof(PairParamX) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
-           (size_t)4 * 16 * force_block_of(h) + (size_t)3 * 16 * force_ppb(h) + (h->geom.fast ? 0 : sizeof(TileShared));
+           (size_t)LIST_PF * 16 * force_block_of(h) + (size_t)3 * 16 * force_ppb(h) + (h->geom.fast ? 0 : sizeof(TileShared));
 }
 
 template <int TPP, int EPL, bool THERMO, bool SCALED, int FN>

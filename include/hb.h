@@ -220,6 +220,47 @@ HB_API int hb_sort(hb_system *h);
  * hb_build_cells, hb_sort) the list is rebuilt if needed and the forces are evaluated first. */
 HB_API int hb_thermo(hb_system *h, hb_thermo_t *out);
 
+/* The same sums for a caller that is not allowed to allocate device memory.
+ *
+ * Who that is: code that runs when the GPU's memory has already been handed out and must stay that way.  A host
+ * program that gave the whole device to its own pool at start-up (a framework's caching allocator with a fixed
+ * budget, a simulation whose arrays were sized to fill HBM) can see cudaMalloc fail, or has a rule against going
+ * round the pool.  A logger or analysis hook that somebody else's time-step loop calls between steps must not
+ * stall that loop, and cudaMalloc / cudaFree synchronise the whole device.  hb_create and hb_thermo are no use to
+ * such a caller: the first allocates every array of the system, the second reads them.
+ *
+ * So this call takes no handle and allocates nothing, on the device or through any CUDA library: no cudaMalloc,
+ * cudaFree, stream-ordered or pool allocation, pinned host memory.  The caller passes its own arrays, all DEVICE
+ * pointers on the current device, in the layouts hb_get_state / hb_get_mass / hb_get_forces write:
+ *   vel_xyz    [N][3]                     (required)
+ *   mass       [N]      NULL = every mass is 1
+ *   f_xyz_u    [N][4]   (Fx, Fy, Fz, U_i); only U_i is read.  NULL = U is reported as 0
+ *   virial6    [N][6]   xx, xy, xz, yy, yz, zz.  NULL = W is reported as 0 (P is then the ideal-gas part)
+ *   out_device          one hb_thermo_t in device memory, written by the last kernel
+ * The order of the particles does not matter (these are plain sums).  L is the box edge, for P = (2K + tr W) / (3 L^3).
+ * Two kernels are enqueued on cuda_stream (a cudaStream_t of the current device, NULL = the legacy default
+ * stream); the call does not wait for them: order your read of out_device after them on that stream.
+ *
+ * The only memory the reduction needs besides inputs and output -- 11 binary64 partial sums per block of 4096
+ * particles -- is a fixed array of 360,448 bytes compiled into the library.  Consequences to know about:
+ *   - Limit: N <= HB_THERMO_STATIC_MAX_N (16,777,216).  A larger N is refused with HB_EINVAL and a message that
+ *     names the limit; nothing is launched.  (Sums are additive: split the particles over several calls, or use
+ *     hb_thermo.)
+ *   - Every GPU on which this library is loaded holds those 360,448 bytes until the process exits.
+ *   - The first call made on each device looks up that device's address of the array (cudaGetSymbolAddress, with
+ *     that device current; the runtime may load the library's GPU code at that moment).  It is remembered per
+ *     device afterwards.  Make that first call at set-up time, before any stream capture is begun.
+ *   - All calls on one device share the one array.  Calls whose kernels can run at the same time on that device
+ *     (different streams, different host threads) overwrite each other's partial sums: keep them ordered, e.g. on
+ *     one stream.  Nothing needs clearing between calls: a call writes every partial sum before it reads it.
+ * Accumulation is binary64, and which particles share a partial sum depends on N only, so the result does not
+ * depend on the GPU model.  It can differ from hb_thermo's in the last bits (another summation order).
+ * errbuf (nullable) receives a NUL-terminated message when the return value is not HB_OK; there is no handle to
+ * ask.  Returns HB_OK, HB_EINVAL (NULL vel_xyz / out_device, N < 1, N over the limit, L <= 0) or HB_ECUDA. */
+#define HB_THERMO_STATIC_MAX_N 16777216LL
+HB_API int hb_thermo_static(const float *vel_xyz, const float *mass, const float *f_xyz_u, const float *virial6,
+                     int64_t N, double L, hb_thermo_t *out_device, void *cuda_stream, char *errbuf, size_t errbuf_len);
+
 /* Cell list: m_out [3]; cell_start [m^3+1]; cell_tags [N] = tags of the members
  * of each cell in CSR order (order inside a cell is undefined).
  * Pass NULL to skip an output.  Sizes: call once with only m_out. */

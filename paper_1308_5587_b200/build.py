@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhb.so")
-SOURCES = ["hb_api.cu", "cells.cu", "nlist.cu", "force.cu", "nve.cu", "sort.cu", "peaks.cu", "dp.cu"]
+SOURCES = ["hb_api.cu", "cells.cu", "nlist.cu", "force.cu", "nve.cu", "sort.cu", "peaks.cu", "dp.cu", "thermo_static.cu"]
 HEADERS = [os.path.join(CSRC, n) for n in ("hb_internal.cuh", "tile.cuh", "cells_dev.cuh", "integrate_dev.cuh")] + \
           [os.path.join(os.path.dirname(HERE), "include", "hb.h")]
 

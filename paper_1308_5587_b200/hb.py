@@ -22,13 +22,14 @@ HB_OK, HB_EINVAL, HB_ECUDA, HB_ENOMEM, HB_EBOX, HB_ESTATE, HB_ENAN = 0, -1, -2, 
 HB_SHIFT_NONE, HB_SHIFT_ENERGY, HB_XPLOR = 0, 1, 2
 HB_POT_LJ, HB_POT_GAUSS, HB_POT_YUKAWA, HB_POT_MORSE = 0, 1, 2, 3
 POTS = {"lj": HB_POT_LJ, "gauss": HB_POT_GAUSS, "yukawa": HB_POT_YUKAWA, "morse": HB_POT_MORSE}
+THERMO_STATIC_MAX_N = 16_777_216   # HB_THERMO_STATIC_MAX_N
 _ERR_NAMES = {-1: "HB_EINVAL", -2: "HB_ECUDA", -3: "HB_ENOMEM", -4: "HB_EBOX", -5: "HB_ESTATE", -6: "HB_ENAN"}
 
 EXPORTS = ["hb_create", "hb_destroy", "hb_set_state", "hb_get_state", "hb_set_state_f64", "hb_get_state_f64", "hb_get_forces_f64", "hb_set_rcut_pair", "hb_set_ron_pair",
            "hb_set_pair_potential", "hb_set_mass", "hb_get_mass", "hb_build_cells",
            "hb_build_nlist", "hb_needs_rebuild", "hb_compute_lj", "hb_step_nve", "hb_run_nve", "hb_run_nvt", "hb_run_langevin",
            "hb_get_thermostat", "hb_set_thermostat", "hb_sort",
-           "hb_thermo", "hb_get_cells", "hb_get_nlist", "hb_get_forces", "hb_stats", "hb_set_tunable",
+           "hb_thermo", "hb_thermo_static", "hb_get_cells", "hb_get_nlist", "hb_get_forces", "hb_stats", "hb_set_tunable",
            "hb_get_tunable", "hb_time_stage", "hb_measure_peak", "hb_last_error", "hb_version"]
 
 
@@ -91,6 +92,7 @@ def load():
     L.hb_set_thermostat.argtypes = [vp, dbl, dbl, i64]
     L.hb_sort.argtypes = [vp]
     L.hb_thermo.argtypes = [vp, C.POINTER(hb_thermo_t)]
+    L.hb_thermo_static.argtypes = [vp, vp, vp, vp, i64, dbl, vp, vp, C.c_char_p, C.c_size_t]
     L.hb_get_cells.argtypes = [vp, vp, vp, vp, i32]
     L.hb_get_nlist.argtypes = [vp, vp, vp, i32]
     L.hb_get_forces.argtypes = [vp, vp, vp, i32]
@@ -332,6 +334,32 @@ class System:
         t = hb_thermo_t()
         self._ck(self._lib.hb_thermo(self._h, C.byref(t)))
         return dict(K=t.K, U=t.U, W=list(t.W), P=t.P, px=t.px, py=t.py, pz=t.pz)
+
+    @staticmethod
+    def thermo_static(vel, mass, f_xyz_u, virial6, L, out, stream=None):
+        """hb_thermo_static: the sums of thermo() from the caller's own CUDA tensors, for callers that must not
+        allocate device memory (include/hb.h says who and why).  No handle is involved.  vel float32 [N][3];
+        mass [N], f_xyz_u [N][4], virial6 [N][6] float32 or None; out: a CUDA float64 tensor of 12 elements that
+        receives (K, U, W[6], P, px, py, pz) once the two kernels enqueued on `stream` (default: torch's current
+        stream) have run -- this call does not wait for them.  N <= THERMO_STATIC_MAX_N."""
+        lib = load()
+        N = int(vel.shape[0])
+        ptrs = []
+        for a in (vel, mass, f_xyz_u, virial6):
+            p, d = _ptr(a, np.float32)
+            if d == 0:
+                raise TypeError("hb_thermo_static takes device arrays (torch CUDA tensors) only")
+            ptrs.append(p)
+        o, d = _ptr(out, np.float64)
+        if d != 1 or out.numel() != 12:
+            raise TypeError("out must be a CUDA float64 tensor of 12 elements")
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        err = C.create_string_buffer(512)
+        rc = lib.hb_thermo_static(*ptrs, N, float(L), o, C.c_void_p(stream or 0), err, len(err))
+        if rc != HB_OK:
+            raise HBError(rc, err.value.decode())
 
     # ---- accessors (BY TAG) ----
     def get_cells(self):

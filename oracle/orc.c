@@ -748,8 +748,8 @@ double orc_uniform_pm1(uint64_t seed, uint64_t stream, uint64_t index)
 /* nsteps of thermostatted dynamics with the list rebuilt on buffer exceedance (same loop as orc_run_nve).
  * mode 1: Nose-Hoover, par = tau, state[0..1] = (xi, eta) in and out.
  * mode 2: Langevin, par = gamma, state[0] = number of the first time step (stream of the generator), advanced.
- * log (nullable) [nsteps+1][4]: K, U, xi, eta at every step incl. step 0.  tag[i] = identity of particle i for
- * the generator (NULL: i). */
+ * log (nullable) [nsteps+1][4]: K, U, xi, eta at every step incl. step 0.  The generator identifies a particle by
+ * its index i (the oracle never reorders particles). */
 int orc_run_thermostat(int mode, double *pos, double *vel, int32_t *image, const int32_t *type, int64_t N, double L,
                        int ntypes, const double *eps, const double *sigma, const double *rcut, const double *ron, int shift,
                        double r_buff, double dt, int64_t nsteps, double T, double par, uint64_t seed, double *state,

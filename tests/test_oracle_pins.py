@@ -407,6 +407,22 @@ def test_rebuild_rule_keeps_list_complete(orc):
     assert 2 <= builds < 60
 
 
+def test_max_disp2_by_hand_including_a_face_crossing(orc):
+    """c3, pinned directly: hand values with no formula of the oracle in between.  Particle 0 moved by (0.3, -0.4, 0):
+    0.25.  Particle 1 left through the +x face and came back in at -x (wrapped coordinate 4.95 -> -4.95 in a box of
+    10): its displacement is 0.1, squared 0.01, NOT (L - 0.1)^2 = 98.01 -- a missing minimum image would give that.
+    Particle 2 did not move.  The maximum is particle 0's; with particle 0 at rest it is particle 1's 0.01."""
+    L = 10.0
+    build = np.array([[1.0, 2.0, -3.0], [4.95, 0.0, 0.0], [-2.0, -2.0, 2.0]])
+    now = np.array([[1.3, 1.6, -3.0], [-4.95, 0.0, 0.0], [-2.0, -2.0, 2.0]])
+    assert orc.max_disp2(now, build, L) == pytest.approx(0.25, rel=1e-14)
+    now[0] = build[0]
+    assert orc.max_disp2(now, build, L) == pytest.approx(0.01, rel=1e-12)
+    # a diagonal crossing of two faces at once: (4.9, -4.9) -> (-4.9, 4.9) is a move of (0.2, -0.2): 0.08
+    assert orc.max_disp2(np.array([[-4.9, 4.9, 0.0]]), np.array([[4.9, -4.9, 0.0]]), L) == pytest.approx(0.08, rel=1e-12)
+    assert orc.max_disp2(build, build, L) == 0.0
+
+
 def test_run_nve_matches_hand_driven_loop(orc):
     """orc_run_nve is the same loop as the pieces called one by one."""
     w = wl.CONFIGS["lj_1k"]

@@ -210,6 +210,7 @@ int configure_geometry(hb_system *h)
     }
     h->r_max = r_max;
     h->m = m;
+    h->geometry_dirty = false;
     h->ncells = (int64_t)m * m * m;
     if (h->ncells > h->ncells_alloc) {
         dev_free_t(h, h->cell_count);
@@ -312,6 +313,7 @@ int enqueue_rebuild(hb_system *h, const int *pred)
 int build_nlist_sync(hb_system *h)
 {
     if (!h->have_state) { h->err = "no state: call hb_set_state first"; return HB_ESTATE; }
+    if (h->geometry_dirty || h->m == 0) HB_TRY(configure_geometry(h));   // hb_set_rcut_pair after a build: new r_max, m, table
     if (h->row_pitch == 0) HB_TRY(ensure_rows(h, initial_pitch(h)));
     for (int attempt = 0; attempt < 16; attempt++) {
         HB_TRY(enqueue_rebuild(h, nullptr));
@@ -475,9 +477,11 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     HB_CK(cudaGraphCreate(&g, 0));
     cudaStream_t saved = h->stream;
     const int64_t saved_launches = h->stats.kernel_launches;
-    const int saved_cur = h->cur, saved_parity = h->parity;
+    const int saved_cur = h->cur, saved_parity = h->parity, saved_parity0 = h->parity0;
     h->cur = 0;       // every chunk starts from posbuf[0] and drift parity 0 (run_chunk sees to it): one graph per n
     h->parity = 0;
+    h->parity0 = 0;   // make_nve bakes kick_step = parity - parity0 - 1 into the captured kernel parameters: a value left
+                      // by hb_step_nve (step_sync) would shift the Langevin generator's step number by the call history
     int rc = HB_OK;
     auto fail = [&](const char *what, cudaError_t e) {
         h->err = std::string(what) + ": " + cudaGetErrorString(e);
@@ -559,6 +563,7 @@ int build_graph(hb_system *h, int n, float dt, hb_system::GraphEntry *out)
     h->stats.kernel_launches = saved_launches;
     h->cur = saved_cur;
     h->parity = saved_parity;
+    h->parity0 = saved_parity0;
     cudaGraphExec_t ex = nullptr;
     if (rc == HB_OK) {
         e = cudaGraphInstantiate(&ex, g, 0);
@@ -1038,6 +1043,7 @@ int hb_set_rcut_pair(hb_system *h, const double *rcut)
             if (rcut[a * nt + b] != rcut[b * nt + a] || !(rcut[a * nt + b] > 0.0)) { h->err = "r_cut table must be symmetric and positive"; return HB_EINVAL; }
     for (int p = 0; p < nt * nt; p++) h->rcut[p] = (double)(float)rcut[p];
     h->rcut_user = true;
+    h->geometry_dirty = true;     // r_cut,max and with it r_max, m and the per-pair list cutoffs may have changed
     h->nlist_valid = h->cells_valid = h->forces_valid = false;
     destroy_graphs(h);
     return upload_params(h);

@@ -101,6 +101,8 @@ struct hb_system {
     int64_t N = 0;
     int ntypes = 1;
     float L = 0, r_cut_max = 0, r_buff = 0, r_max = 0;
+    bool geometry_dirty = false;  // a cutoff changed since configure_geometry last ran: r_max, m, the tiles and the typed-list
+                                  // table are out of date; build_nlist_sync reconfigures before it builds
     int shift_mode = HB_SHIFT_ENERGY;
     int pot = HB_POT_LJ;     // pair potential (hb_set_pair_potential)
     bool rcut_user = false;  // hb_set_rcut_pair was called

@@ -95,6 +95,28 @@ def test_langevin_trajectory_matches_the_oracle(hb, orc, tun):
     assert np.abs(ref["vel"] - nve["vel"]).max() > 0.05   # the noise is not a no-op
 
 
+@pytest.mark.parametrize("tun", [dict(), dict(fuse_nve=0), dict(graph_mode=2)])
+def test_langevin_after_a_graph_run_and_a_single_step(hb, orc, tun):
+    """hb_run_nve, then hb_step_nve, then hb_run_langevin: the single step leaves its own step offset in the handle,
+    and the graphs captured for the new ensemble must not inherit it -- the generator's stream is the number of the
+    Langevin step since hb_set_state (hb.h), whatever was called before."""
+    w = wl.CONFIGS["lj_1k"]
+    s = wl.make_state(w)
+    p = orc.Params.of(w)
+    T, gamma, seed = 0.8, 2.0, 99
+    nve = orc.run_nve(s.pos, s.vel, s.image, s.type, s.L, p, w.r_buff, w.dt, 4)
+    ref = orc.run_langevin(nve["pos"], nve["vel"], nve["image"], s.type, s.L, p, w.r_buff, w.dt, 10, T, gamma, seed)
+    with _system(hb, w, s, **tun) as g:
+        g.run_nve(w.dt, 3, 0)
+        g.step_nve(w.dt)
+        g.run_langevin(w.dt, 10, T, gamma, seed)
+        out = g.get_state()
+        ts = g.get_thermostat()
+    assert ts["langevin_steps"] == 10
+    assert np.abs(_unwrapped(out, s.L) - (ref["pos"] + ref["image"] * s.L)).max() <= 2e-5
+    assert np.abs(out["vel"].astype(np.float64) - ref["vel"]).max() <= 2e-5 * max(1.0, np.abs(ref["vel"]).max())
+
+
 def test_langevin_free_particles_and_thermalisation(hb, orc):
     """eps = 0: stationary <v^2> = T / (1 - gamma dt / 2) per component (the closed form that pins the oracle);
     the interacting fluid settles at the set temperature."""

@@ -102,3 +102,44 @@ def test_one_type_ignores_the_tunable(hb, orc):
     pos64 = s.pos.astype(np.float64)
     c, r, n = orc.nlist_cells(pos64, s.L, w.r_max)
     parity.assert_nlist_equal(pos64, s.L, w.r_max, r, n, rs, nbr)
+
+
+@pytest.mark.parametrize("typed", [0, 1])
+def test_raising_rcut_after_a_build_rebuilds_with_the_new_radius(hb, orc, typed):
+    """hb_set_rcut_pair on a handle that already has a list, then straight to hb_thermo / hb_run_nve with no explicit
+    hb_build_nlist: the list the library rebuilds on its own must use the NEW r_max, cell count and per-pair table,
+    or the pairs between the old list radius and the new cutoff are silently missing from the forces."""
+    w = wl.scaled(wl.CONFIGS["ka_1m"], 20_000)
+    s = wl.make_state(w)
+    pos64 = s.pos.astype(np.float64)
+    short = tuple(0.8 * rc for rc in w.rcut)             # the first list: every cutoff 20 % shorter
+    with hb.System(w.N, w.L, w.ntypes, w.eps, w.sigma) as g:
+        g.set_tunable("nlist_pair_rcut", typed)
+        g.set_rcut_pair(short)
+        g.set_state(s.pos, s.type, s.vel, s.image)
+        g.build_nlist(0.0, w.r_buff)
+        g.compute_lj(w.shift)
+        m_short = g.stats()["cells_per_axis"]
+        g.set_rcut_pair(w.rcut)                          # raise them; no hb_build_nlist after this
+        th = g.thermo()                                  # rebuilds the list and the forces by itself
+        m_full = g.stats()["cells_per_axis"]
+        rs, nbr = g.get_nlist()
+        f4, w6 = g.get_forces()
+        g.run_nve(w.dt, 20, 0)                           # and the graphs are captured for the new geometry
+        E1 = g.thermo()
+    assert m_full < m_short                              # wider cells: the geometry was reconfigured
+    rl = _rlist(w)
+    if typed:
+        c, r, n = orc.nlist_cells_typed(pos64, s.type, s.L, w.ntypes, rl)
+        parity.assert_nlist_equal(pos64, s.L, _per_pair(s.type, rl, w.ntypes), r, n, rs, nbr)
+    else:
+        c, r, n = orc.nlist_cells(pos64, s.L, w.r_max)
+        parity.assert_nlist_equal(pos64, s.L, w.r_max, r, n, rs, nbr)
+    p = orc.Params.of(w)
+    F, U, W, A = orc.compute_lj_nlist(pos64, s.type, s.L, p, c, r, n, band=parity.BAND)
+    parity.assert_forces_close(F, U, W, A, f4, w6)
+    parity.assert_energy_close(U.sum(), th["U"], A[:, 1].sum())
+    # the dense lattice start melts violently: same bound as test_typed_list_through_run_nve (the velocity-Verlet error
+    # of that transient); a run whose graphs still held the short cutoff would lose far more than this
+    E0 = th["K"] + th["U"]
+    assert abs(E1["K"] + E1["U"] - E0) <= 2e-3 * E1["K"]

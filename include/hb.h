@@ -198,11 +198,12 @@ HB_API int hb_step_nve(hb_system *h, double dt);
 HB_API int hb_run_nve(hb_system *h, double dt, int64_t nsteps, int64_t sort_period);
 
 /* The same loop with a thermostat (the paper names the integrators, PAPER.md:87, 99, 324,
- * and prints no equations: readings n1, n2 of DESIGN.md).  k_B = 1, m = 1.
- * hb_run_nvt: Nose-Hoover, dv/dt = F - xi v, dxi/dt = (T_k / T - 1) / tau^2 with T_k = 2K / (3N - 3); the
+ * and prints no equations: readings n1, n2, m1 of DESIGN.md).  k_B = 1; m is the particle's mass (1 unless hb_set_mass).
+ * hb_run_nvt: Nose-Hoover, dv/dt = F / m - xi v, dxi/dt = (T_k / T - 1) / tau^2 with T_k = 2K / (3N - 3); the
  *   thermostat variable xi and its time integral eta live in the handle (hb_get_thermostat / hb_set_thermostat;
  *   hb_set_state zeroes them); K + U + (3N - 3) T (tau^2 xi^2 / 2 + eta) is conserved.
- * hb_run_langevin: after every velocity-Verlet step v <- v (1 - gamma dt) + sqrt(6 gamma T dt) u, u uniform in
+ * hb_run_langevin: after every velocity-Verlet step v <- v (1 - gamma dt / m) + sqrt(6 gamma T dt) / m u (friction and
+ *   noise are forces: both divided by the mass), u uniform in
  *   (-1, 1) from the counter-based generator splitmix64(seed, time step number, 3 tag + component); the time step
  *   number counts the Langevin steps since hb_set_state (hb_get_thermostat reports it). */
 HB_API int hb_run_nvt(hb_system *h, double dt, int64_t nsteps, int64_t sort_period, double T, double tau);
@@ -327,7 +328,8 @@ HB_API int hb_time_stage(hb_system *h, const char *stage, int reps, int64_t flus
 /* Measured roofline denominators on this device, with kernels of this library:
  *   "fp32_tflops"  FFMA throughput, 8 independent chains per thread, all SMs        -> TFLOP/s
  *   "l2_gbs"       read bandwidth of a 32 MB buffer resident in L2, 16 B per load   -> GB/s
- *   "smem_gbs"     conflict-free 16-byte shared-memory loads, all SMs               -> GB/s
+ *   "smem_gbs"     conflict-free 16-byte shared-memory loads, 4 independent address
+ *                  streams per thread (no load feeds an address), all SMs           -> GB/s
  * Best of five timed launches (CUDA events on the system's stream); synchronises. */
 HB_API int hb_measure_peak(hb_system *h, const char *which, double *value);
 

@@ -2,7 +2,8 @@
 // and L2 peaks"): three small kernels, timed with CUDA events on the system's stream.
 //   fp32_tflops  eight independent FFMA chains per thread, every SM full of warps
 //   l2_gbs       a 32 MB buffer (resident in the 126 MB L2 after the first pass) read again and again, 16 B per load
-//   smem_gbs     conflict-free 16-byte shared-memory loads: the crossbar the force kernel's neighbor gathers go through
+//   smem_gbs     conflict-free 16-byte shared-memory loads, four independent address streams per thread: the crossbar
+//                the force kernel's neighbor gathers go through
 #include "hb_internal.cuh"
 
 constexpr int PK_THREADS = 256;
@@ -37,22 +38,31 @@ __global__ void __launch_bounds__(PK_THREADS) peak_l2_kernel(const float4 *__res
     if (acc == 12345.678f) out[0] = acc;
 }
 
-__global__ void __launch_bounds__(PK_THREADS) peak_smem_kernel(float *out, int iters)
+// Four address streams per thread, none of which depends on a loaded value (the index advances by a kernel argument,
+// so the loads can neither be hoisted nor chained): the loads of one thread are independent and the pipe, not the
+// load latency, is what limits the rate.  Consecutive lanes read consecutive 16-byte words: no bank conflict, four
+// 128-byte wavefronts per warp instruction.
+__global__ void __launch_bounds__(PK_THREADS) peak_smem_kernel(float *out, int iters, int step)
 {
     __shared__ int4 tile[PK_THREADS * 4];
     for (int k = threadIdx.x; k < PK_THREADS * 4; k += PK_THREADS) tile[k] = make_int4(k, 1, 0, 3);
     __syncthreads();
-    int acc = 0;
-    int idx = threadIdx.x;
+    constexpr int MASK = PK_THREADS * 4 - 1;
+    int acc0 = 0, acc1 = 0, acc2 = 0, acc3 = 0;
+    int i0 = threadIdx.x, i1 = threadIdx.x + PK_THREADS, i2 = threadIdx.x + 2 * PK_THREADS, i3 = threadIdx.x + 3 * PK_THREADS;
 #pragma unroll 1
     for (int k = 0; k < iters; k++) {
 #pragma unroll
-        for (int u = 0; u < 8; u++) {
-            const int4 v = tile[idx];                   // consecutive lanes, consecutive 16-byte words: no bank conflict
-            acc += v.y;
-            idx = (idx + PK_THREADS + v.z) & (PK_THREADS * 4 - 1);   // depends on the load: it cannot be hoisted
+        for (int u = 0; u < 2; u++) {
+            const int4 v0 = tile[i0], v1 = tile[i1], v2 = tile[i2], v3 = tile[i3];
+            acc0 += (v0.x ^ v0.y) + (v0.z ^ v0.w);
+            acc1 += (v1.x ^ v1.y) + (v1.z ^ v1.w);
+            acc2 += (v2.x ^ v2.y) + (v2.z ^ v2.w);
+            acc3 += (v3.x ^ v3.y) + (v3.z ^ v3.w);
+            i0 = (i0 + step) & MASK; i1 = (i1 + step) & MASK; i2 = (i2 + step) & MASK; i3 = (i3 + step) & MASK;
         }
     }
+    const int acc = (acc0 + acc1) + (acc2 + acc3);
     if (acc == 123456789) out[0] = (float)acc;
 }
 
@@ -87,7 +97,7 @@ int measure_peak(hb_system *h, const char *which, double *value)
             peak_l2_kernel<<<grid, PK_THREADS, 0, st>>>(buf, n4, passes, out);
             work = (double)n4 * 16.0 * passes / 1e9;                                  // GB
         } else {
-            peak_smem_kernel<<<grid, PK_THREADS, 0, st>>>(out, iters);
+            peak_smem_kernel<<<grid, PK_THREADS, 0, st>>>(out, iters, PK_THREADS);
             work = (double)grid * PK_THREADS * iters * 8.0 * 16.0 / 1e9;              // GB
         }
         cudaEventRecord(e1, st);

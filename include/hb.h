@@ -284,7 +284,11 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *   "stage_cap"      shared-memory slots per tile (0 = from the density); grown on overflow
  *   "row_pitch"      initial entries per list row (rounded up to 64; 0 = estimate)
  *   "grow_pct"       head room in percent when rows / the staging area are grown after an overflow (25)
- *   "cell_sort"      1 = members of a cell ordered by index (deterministic lists)
+ *   "cell_sort"      1 = members of a cell ordered by index: the same lists, in the same order, run after run, FOR GIVEN
+ *                    tile sizes, "stage_cap" and "row_pitch".  The order inside a row follows the slot numbering of the
+ *                    staged tile, so after an overflow has grown the rows or the staging area the redone
+ *                    work sums the same pairs in another order: results then agree with a run that had room from the
+ *                    start to rounding (1e-4 relative in the tests), not bit for bit
  *   "force_block"    threads per block of the force kernel: 128, 256
  *   "nlist_block"    threads per block of the stand-alone list kernel: 128, 256
  *   "thermo_every"   0 = (default) inside hb_run_nve U_i and W_i are computed by the last step of every chunk only:
@@ -303,8 +307,6 @@ HB_API int hb_stats(hb_system *h, hb_stats_t *out);
  *   "graph_steps"    steps per graph launch
  *   "nlist_pair_rcut" 1 = the list keeps pair (i, j) iff d < r_cut(type i, type j) + r_buff (reading t1; up to 8 types);
  *                    0 = (default) one list cutoff, the largest (reading c2.iii)
- *   "dbg"            timing experiments only (the physics is WRONG with it): 1 = the step kernel skips its pair loop,
- *                    2 = it stops after the tile tables, 4 = it returns at once (latency breakdown)
  *   "precision"      32 = (default) binary32 arithmetic (the paper's GPU precision);
  *                    64 = force sums and velocity Verlet in binary64 (NVE, hb_step_nve / hb_run_nve one step per host
  *                         iteration; hb_run_nvt / hb_run_langevin return HB_EINVAL): what the arithmetic conserves

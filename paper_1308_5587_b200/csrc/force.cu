@@ -17,7 +17,7 @@
 //     position array ("piece", two where the row wraps around the box): the block
 //     reads cell_start at the ends of its (ty+2)(tz+2) halo rows, prefix-sums the
 //     lengths (that IS the slot numbering the list build used) and copies each piece
-//     with cp.async, 16 bytes per lane, straight into the staging area.  No per-tile
+//     with one cp.async.bulk (TMA bulk copy, completion on an mbarrier) straight into the staging area.  No per-tile
 //     table is read (round 1 read a 4-byte source index per staged slot per step).
 //     Only tiles whose halo touches a face of the box fix the periodic image, in place;
 //   * list entries are 16-bit BYTE OFFSETS into the staging area (slot * 16 when the
@@ -170,7 +170,7 @@ struct ForceArgs {
     const int *cell_start;
     const float4 *pos;
     const uint16_t *nlist;
-    int pitch, N, ntypes, pot, dbg;
+    int pitch, N, ntypes, pot;
     const PairParam *params;
     const PairParamX *paramsx;
     float4 *force, *virial;
@@ -292,7 +292,6 @@ lj_tile_kernel(const ForceArgs A)
     const NveArgs &nv = A.nv;
     const bool nve = A.do_nve != 0, drift = nve && nv.kick_drift;
     const bool block0 = (blockIdx.x | blockIdx.y | blockIdx.z) == 0;
-    if (A.dbg & 4) return;
 
     if (threadIdx.x == 0 && g.fast) mbar_init(&s.mbar, 1);
     if (!ONE_TYPE)
@@ -306,7 +305,7 @@ lj_tile_kernel(const ForceArgs A)
     bool fits;
     if (g.fast) {
         fits = force_tile_tables(g, A.cell_start, s);
-        if (fits && !(A.dbg & 2) && threadIdx.x < 32) {
+        if (fits && threadIdx.x < 32) {
             // warp 0 hands the pieces to the TMA unit: one bulk copy per contiguous run of positions
             const int lane = threadIdx.x;
             if (lane == 0) {
@@ -327,8 +326,7 @@ lj_tile_kernel(const ForceArgs A)
         __syncthreads();
         if (fits) tile_stage_positions(g, t, sgen, A.pos, stage, nullptr);
     }
-    const int nown = (fits && !(A.dbg & 2)) ? s.d.nown : 0;
-    if (A.dbg & 2) return;
+    const int nown = fits ? s.d.nown : 0;
 
     const int sub = threadIdx.x % TPP;
     const int ql = threadIdx.x / TPP;            // particle of the pass this thread group works for
@@ -396,17 +394,13 @@ lj_tile_kernel(const ForceArgs A)
             cp_async_wait<PF - 1>();
             Entries<EPL> ent;
             ent.v = ring[0];
-            for (int k = 0; k < ((A.dbg & 1) ? 0 : A.pitch); k += G) {
+            for (int k = 0; k < A.pitch; k += G) {
                 if ((ent.v.x & 0xffffu) == 0u) break;                    // padding: the row is over for this thread
                 cp_async<EPL * 2>(ring + c * ring_stride, row + k + PF * G);   // refill PF iterations ahead (reads past the
                 cp_async_commit();                                       // row's end are harmless: the array has slack)
                 c = (c + 1 == PF) ? 0 : c + 1;
                 unsigned off[EPL];
                 unpack_entries<EPL, SCALED>(ent, off);
-#ifdef HB_EXPERIMENT_BANKS   // timing experiment only (wrong physics): force the bank group of every gather to the conflict-free pattern
-#pragma unroll
-                for (int e = 0; e < EPL; e++) off[e] = (off[e] & ~0x70u) | ((unsigned)((ql + sub * EPL + e) & 7) << 4);
-#endif
                 float4 pj[EPL];
 #pragma unroll
                 for (int e = 0; e < EPL; e++) pj[e] = *reinterpret_cast<const float4 *>(stage_b + off[e]);
@@ -490,7 +484,7 @@ static int force_ppb(const hb_system *h) { return force_block_of(h) / force_tpp(
 
 size_t force_smem_bytes(const hb_system *h)
 {
-    // staged positions, pair table, ring of 4 async list copies (16 B at most) per thread, own data (2 buffers x 3 arrays)
+    // staged positions, pair table, ring of PF (2) async list copies (16 B at most) per thread, own data (2 buffers x 3 arrays)
     // and forces of a pass
     return (size_t)h->geom.cap * 16 + (h->ntypes > 1 ? ((sizeof(PairParam) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
            (h->ntypes > 1 ? ((sizeof(PairParamX) * h->ntypes * h->ntypes + 15) & ~(size_t)15) : 0) +
@@ -511,7 +505,6 @@ static cudaError_t launch_force_tts(hb_system *h, const NveArgs *nve)
     A.N = (int)h->N;
     A.ntypes = h->ntypes;
     A.pot = h->pot;
-    A.dbg = h->tun.dbg;
     A.params = h->params;
     A.paramsx = h->paramsx;
     A.force = h->force;

@@ -1519,7 +1519,6 @@ static int *tunable_slot(hb_system *h, const char *name)
     if (!strcmp(name, "nlist_ppi")) return &h->tun.nlist_ppi;
     if (!strcmp(name, "nlist_block")) return &h->tun.nlist_block;
     if (!strcmp(name, "nlist_pair_rcut")) return &h->tun.nlist_pair_rcut;
-    if (!strcmp(name, "dbg")) return &h->tun.dbg;
     if (!strcmp(name, "precision")) return &h->tun.precision;
     if (!strcmp(name, "tile_x")) return &h->tun.tile_x;
     if (!strcmp(name, "tile_y")) return &h->tun.tile_y;

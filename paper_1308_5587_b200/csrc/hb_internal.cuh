@@ -85,7 +85,6 @@ struct Tunables {
     int graph_mode = 1;    // measured on B200: five early-exit kernels per step cost less than one conditional node
     int graph_steps = 100;
     int precision = 32;    // 64: the binary64 variant of the force sums and the integration (dp.cu)
-    int dbg = 0;           // timing experiments only (wrong physics): 1 skip the pair loop, 2 stop after the tile tables, 4 empty kernel
 };
 
 enum { TS_XI = 0, TS_ETA = 1, TS_KSUM = 2, TS_LBASE = 3, TS_COUNT = 8 };

@@ -62,9 +62,8 @@ struct TileCtx {
     int nrows;        // own (y, z) rows = ey * ez
 };
 
-// What the force kernel needs to know about a tile.  It depends on cell_start only, so the list
-// build writes it once per build (one per tile, in global memory) and the force kernel, which
-// runs every step, just loads it.
+// What a kernel needs to know about its tile.  It depends on cell_start only; every block derives it
+// from cell_start at its start (tile_tables / force_tile_tables) and keeps it in shared memory.
 struct TileDesc {
     int nslots;       // 1 + staged particles (1 = nothing staged: the build found the tile too big)
     int nown;         // own particles
@@ -75,7 +74,7 @@ struct TileDesc {
     int own_slot[TILE_ROWS_MAX];     // its slot
     int pad;
 };
-static_assert(sizeof(TileDesc) == 416, "hb_api.cu sizes the descriptor array with this number");
+static_assert(sizeof(TileDesc) == 416, "force.cu copies it word by word; keep it a multiple of 4 bytes");
 
 struct TileShared {
     int hslot[TILE_HMAX + 1];   // first slot of halo cell h
@@ -339,35 +338,6 @@ __device__ __forceinline__ void tile_stage_positions_bulk(const TileGeom &g, con
     }
     __syncthreads();
     if (threadIdx.x == 0) mbar_inval(bar);
-}
-
-// The same staging from the tables the list build left behind (fast geometry only): per slot one
-// coalesced index load, one position load, the image nearest to the tile centre.
-__device__ __forceinline__ void tile_stage_from_table(const TileDesc &d, const int *__restrict__ src_tab,
-                                                      const float4 *__restrict__ pos, float4 *__restrict__ stage, float L)
-{
-    constexpr int U = 4;
-    const int nt = blockDim.x;
-    const float hL = 0.5f * L;
-    const int nslots = d.nslots;
-    if (threadIdx.x == 0) stage[0] = make_float4(1e18f, 1e18f, 1e18f, 0.f);
-    for (int s0 = 1 + threadIdx.x; s0 < nslots; s0 += U * nt) {
-        int src[U];
-#pragma unroll
-        for (int u = 0; u < U; u++) {
-            const int sl = s0 + u * nt;
-            src[u] = sl < nslots ? __ldg(&src_tab[sl]) : -1;
-        }
-        float4 p[U];
-#pragma unroll
-        for (int u = 0; u < U; u++)
-            if (src[u] >= 0) p[u] = pos[src[u]];
-#pragma unroll
-        for (int u = 0; u < U; u++)
-            if (src[u] >= 0)
-                stage[s0 + u * nt] = make_float4(tile_image(p[u].x, d.cx, L, hL), tile_image(p[u].y, d.cy, L, hL),
-                                                 tile_image(p[u].z, d.cz, L, hL), p[u].w);
-    }
 }
 
 // tile-local own particle q -> own row r (rows are few: linear scan)
